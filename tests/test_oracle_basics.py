@@ -1,0 +1,281 @@
+"""Pins for the oracle's building blocks: Philox, the U(w) map, the single-link heatbath law,
+staples, overrelaxation, the sweep schedule and the slab mask.  CPU only.
+
+Each test names the passage of the paper / SURVEY.md section 8(c) it pins.
+"""
+import os
+
+import numpy as np
+import pytest
+from scipy import special, stats
+
+from tests import inputs
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def test_philox_known_answers(ulo):
+    # S8(c)-O4; vectors in tests/golden/philox4x32_10_kat.txt
+    n = 0
+    for line in open(os.path.join(GOLD, "philox4x32_10_kat.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        w = [int(v, 16) for v in line.split() if v != "->"]
+        out = ulo.philox4x32_10(w[0:4], w[4:6])
+        assert [int(v) for v in out] == w[6:10]
+        n += 1
+    assert n == 3
+
+
+def test_paper_accumulator_sizing(ulo):
+    # 2*8*volume*area/step = 972 MB for 24^3x16, step 2; bare lattice 1.7 MB
+    vals = {}
+    for line in open(os.path.join(GOLD, "paper_values.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        name, v = line.split()[:2]
+        vals[name] = int(v)
+    b = ulo.paper_accumulator_bytes(24, 16, 2)
+    assert b == vals["accumulator_bytes_24c16_step2"]
+    assert round(b / 2 ** 20) == 972
+    assert 8 * 24 ** 3 * 16 == vals["lattice_bytes_24c16"]
+    assert 550 < b / (8 * 24 ** 3 * 16) < 600          # "almost 600 times more"
+
+
+def _draws(ulo, a, n, seed=12345):
+    phi = np.empty(n)
+    att = np.empty(n, dtype=np.int64)
+    for i in range(n):
+        phi[i], att[i] = ulo.heatbath_phi(a, seed, i, 7, 0, 0)
+    return phi, att
+
+
+@pytest.mark.parametrize("a", [0.0, 0.01, 0.5, 1.0, 3.0, 6.0, 30.0])
+def test_heatbath_law_ks(ulo, a):
+    # BJ check (a): single-link heatbath histogram against exp(a cos phi) by a KS test (S8(c)-O3)
+    n = 40000
+    phi, att = _draws(ulo, a, n)
+    assert np.all(np.abs(phi) <= np.pi)
+    if a == 0.0:
+        cdf = lambda x: (x + np.pi) / (2 * np.pi)
+        assert np.all(att == 1)                       # a = 0: always accept
+    else:
+        cdf = stats.vonmises(kappa=a).cdf             # library cross-check of the law, not of the stream
+    d, p = stats.kstest(phi, cdf)
+    assert p > 1e-3, (a, d, p)
+    # <cos phi> = I1(a)/I0(a)
+    want = special.ive(1, a) / special.ive(0, a)
+    var = np.var(np.cos(phi)) / n
+    assert abs(np.cos(phi).mean() - want) < 4.5 * np.sqrt(var) + 1e-12
+    # odd moment vanishes (sign bit is fair)
+    assert abs(np.sin(phi).mean()) < 4.5 * np.sqrt(np.var(np.sin(phi)) / n)
+    assert att.max() < 64 and att.mean() < 1.7
+
+
+def test_heatbath_wrong_law_is_rejected(ulo):
+    # the KS pin has teeth: samples for a=1 must fail against a=1.15
+    phi, _ = _draws(ulo, 1.0, 40000)
+    _, p = stats.kstest(phi, stats.vonmises(kappa=1.15).cdf)
+    assert p < 1e-3
+
+
+def test_heatbath_stream_is_counter_based(ulo):
+    # same (seed, counter) -> same draw; different site word -> different draw
+    a = ulo.heatbath_phi(2.0, 9, 5, 1, 0, 3)
+    b = ulo.heatbath_phi(2.0, 9, 5, 1, 0, 3)
+    c = ulo.heatbath_phi(2.0, 9, 6, 1, 0, 3)
+    assert a == b and a != c
+
+
+def test_hot_start_matches_keying(ulo):
+    # S8(c)-O4: theta = fp32(2 pi w0 2^-32 - pi), ctr = (site, 0, 0, (1<<3)|mu), key = seed words
+    seed = (0x1234 << 32) | 0xABCDEF01
+    o = ulo.Oracle(4, 4, 1.0, seed)
+    th = o.get_links().reshape(4, -1)
+    for mu, site in [(0, 0), (1, 17), (3, 255), (2, 100)]:
+        w = ulo.philox4x32_10([site, 0, 0, (1 << 3) | mu], [seed & 0xffffffff, seed >> 32])
+        want = np.float32(2 * np.pi * float(w[0]) * 2.0 ** -32 - np.pi)
+        assert th[mu, site] == want
+    assert abs(th.mean()) < 0.2 and abs(th.std() - np.pi / np.sqrt(3)) < 0.1
+
+
+def _plaq_sum_numpy(links):
+    """sum over all plaquettes of cos theta_P, straight from P:99, with np.roll (independent of the oracle)."""
+    th = links.astype(np.float64)
+    tot = 0.0
+    for a in range(4):
+        for b in range(a + 1, 4):
+            thP = th[a] + inputs.shift(th[b], a) - inputs.shift(th[a], b) - th[b]
+            tot += np.cos(thP).sum()
+    return tot
+
+
+def test_staple_identity(ulo):
+    # sum_links k cos(theta - alpha) = 4 sum_plaq cos theta_P on any configuration (each plaquette has 4 links)
+    Ns, Nt = 4, 6
+    links = inputs.hot_links(Ns, Nt, 3)
+    o = ulo.Oracle(Ns, Nt, 1.0, 1)
+    o.set_links(links)
+    flat = links.reshape(4, -1).astype(np.float64)
+    tot = 0.0
+    for mu in range(4):
+        for site in range(o.V):
+            k, alpha = o.staple(mu, site)
+            tot += k * np.cos(flat[mu, site] - alpha)
+    assert abs(tot - 4 * _plaq_sum_numpy(links)) < 1e-9 * o.V
+
+
+def test_staple_single_link_numpy(ulo):
+    # S = sum_nu [e^{-i sigma+} + e^{-i sigma-}] re-derived with np.roll for every link of one direction
+    Ns, Nt = 4, 4
+    links = inputs.hot_links(Ns, Nt, 11)
+    th = links.astype(np.float64)
+    o = ulo.Oracle(Ns, Nt, 1.0, 1)
+    o.set_links(links)
+    for mu in range(4):
+        S = np.zeros(th[mu].shape, dtype=complex)
+        for nu in range(4):
+            if nu == mu:
+                continue
+            sp = inputs.shift(th[nu], mu) - inputs.shift(th[mu], nu) - th[nu]
+            down = lambda f: inputs.shift(f, nu, -1)
+            sm = -down(inputs.shift(th[nu], mu)) - down(th[mu]) + down(th[nu])
+            S += np.exp(-1j * sp) + np.exp(-1j * sm)
+        S = S.reshape(-1)
+        for site in [0, 5, 77, o.V - 1]:
+            k, alpha = o.staple(mu, site)
+            assert abs(k * np.exp(1j * alpha) - S[site]) < 1e-12
+
+
+def test_overrelaxation_preserves_action(ulo):
+    # P:101 / refs P:479-480: an OR sweep leaves sum cos theta_P unchanged up to fp32 storage rounding
+    Ns, Nt = 6, 4
+    o = ulo.Oracle(Ns, Nt, 1.0, 5)
+    o.sweep(3, 0)
+    before = _plaq_sum_numpy(o.get_links())
+    links0 = o.get_links().copy()
+    o.sweep(0, 1)
+    after = _plaq_sum_numpy(o.get_links())
+    assert not np.array_equal(links0, o.get_links())
+    assert abs(after - before) < 2e-6 * 6 * o.V
+
+
+def test_overrelaxation_substep_is_involution(ulo):
+    # applying the OR map twice with frozen neighbours is the identity (up to fp32 storage rounding)
+    Ns, Nt = 4, 4
+    o = ulo.Oracle(Ns, Nt, 1.0, 6)
+    a = o.get_links().astype(np.float64)
+    o.substep(1, 0, 2)
+    mid = o.get_links().astype(np.float64)
+    o.substep(1, 0, 2)
+    b = o.get_links().astype(np.float64)
+    diff = np.abs(np.angle(np.exp(1j * (a - b))))
+    assert diff.max() < 2e-6
+    assert np.abs(np.angle(np.exp(1j * (a - mid)))).max() > 0.1
+    # only links of direction 2 on even sites moved
+    moved = np.abs(np.angle(np.exp(1j * (a - mid)))) > 0
+    assert not moved[[0, 1, 3]].any()
+    t, x3, x2, x1 = np.meshgrid(np.arange(Nt), np.arange(Ns), np.arange(Ns), np.arange(Ns), indexing="ij")
+    assert not moved[2][(t + x1 + x2 + x3) % 2 == 1].any()
+
+
+def test_beta_zero_heatbath_is_uniform_and_forgets(ulo):
+    # beta = 0: new angles uniform, independent of the configuration
+    Ns, Nt = 6, 6
+    o = ulo.Oracle(Ns, Nt, 0.0, 7)
+    o.init(0)
+    o.sweep(1, 0)
+    th = o.get_links().reshape(-1).astype(np.float64)
+    _, p = stats.kstest(th, lambda x: (x + np.pi) / (2 * np.pi))
+    assert p > 1e-3
+    assert abs(np.cos(th).mean()) < 5 / np.sqrt(th.size)
+
+
+def test_sweep_equals_substeps_and_counter(ulo):
+    # S8(c)-O5 / P:374: parity outer (even, odd), direction inner; counter advances once per HB sweep only
+    Ns, Nt = 4, 4
+    a = ulo.Oracle(Ns, Nt, 0.9, 21)
+    b = ulo.Oracle(Ns, Nt, 0.9, 21)
+    a.sweep(1, 2)
+    assert a.get_counter() == 1
+    for parity in (0, 1):
+        for mu in range(4):
+            b.substep(0, parity, mu)
+    b.set_counter(b.get_counter() + 1)
+    for _ in range(2):
+        for parity in (0, 1):
+            for mu in range(4):
+                b.substep(1, parity, mu)
+    assert np.array_equal(a.get_links(), b.get_links())
+    # a different order is a different chain
+    c = ulo.Oracle(Ns, Nt, 0.9, 21)
+    for mu in range(4):
+        for parity in (0, 1):
+            c.substep(0, parity, mu)
+    assert not np.array_equal(a.get_links(), c.get_links())
+
+
+def test_checkpoint_resume_is_exact(ulo):
+    # state = links + counter + seed (counter-based RNG): resume reproduces the chain bit for bit
+    a = ulo.Oracle(4, 4, 1.0, 33)
+    a.sweep(2, 1)
+    links, ctr = a.get_links().copy(), a.get_counter()
+    a.sweep(2, 3)
+    b = ulo.Oracle(4, 4, 1.0, 33)
+    b.set_links(links)
+    b.set_counter(ctr)
+    b.sweep(2, 3)
+    assert np.array_equal(a.get_links(), b.get_links())
+
+
+@pytest.mark.parametrize("d", [2, 4])
+def test_slab_mask_freezes_boundary_layers(ulo, d):
+    # row a6: spatial links on layers t = 0 mod d stay bit-identical; everything else moves
+    Ns, Nt = 4, 8
+    o = ulo.Oracle(Ns, Nt, 1.0, 8)
+    before = o.get_links().copy()
+    o.set_subupdate(1, 2, 1)
+    o.multilevel(d, 3, 2)
+    after = o.get_links()
+    for t in range(Nt):
+        for mu in range(4):
+            same = np.array_equal(before[mu, t], after[mu, t])
+            assert same == (mu != 0 and t % d == 0), (mu, t)
+
+
+def test_slabs_are_dynamically_independent(ulo):
+    # with the boundary layers frozen, changing a link strictly inside another slab leaves
+    # this slab's trajectory bit-identical (same seed, same counters)
+    Ns, Nt, d = 4, 8, 2
+    base = inputs.hot_links(Ns, Nt, 4)
+    pert = base.copy()
+    pert[2, 5, 1, 2, 3] += 0.7          # spatial link at t = 5: interior of slab s = 2 (t = 4,5)
+    pert[0, 4, 0, 0, 1] -= 0.3          # temporal link at t = 4: also slab 2
+    outs = []
+    for cfg in (base, pert):
+        o = ulo.Oracle(Ns, Nt, 1.0, 99)
+        o.set_links(cfg)
+        o.multilevel(d, 4, 1)
+        outs.append(o.get_links())
+    a, b = outs
+    for t in range(Nt):
+        for mu in range(4):
+            in_slab2 = (t in (4, 5))
+            if not in_slab2:
+                assert np.array_equal(a[mu, t], b[mu, t]), (mu, t)
+    assert not np.array_equal(a[0, 4], b[0, 4])
+
+
+def test_error_codes(ulo):
+    import ctypes as C
+    L = ulo.lib()
+    h = C.c_void_p()
+    assert L.ulo_create(C.byref(h), 3, 4, 1.0, 1) == -1       # odd extent
+    assert L.ulo_create(C.byref(h), 4, 4, -1.0, 1) == -1      # beta < 0
+    o = ulo.Oracle(4, 4, 1.0, 1)
+    with pytest.raises(ulo.OracleError):
+        o.multilevel(3, 1, 1)                                  # Nt % d != 0
+    with pytest.raises(ulo.OracleError):
+        o.multilevel(2, 1, 3)                                  # r_max > Ns/2
+    with pytest.raises(ulo.OracleError):
+        o.read_correlators()                                   # nothing measured yet
