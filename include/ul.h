@@ -1,0 +1,157 @@
+/* ul.h -- C ABI of libul.so: the B200-native hot path of arXiv:1309.3859
+ * (Amado, Cardoso, Bicudo): compact U(1) Wilson-action lattice gauge theory in 3+1 d,
+ * heatbath + overrelaxation checkerboard sweeps, slab-masked sub-updates and the
+ * Luescher-Weisz multilevel estimator of <P^dagger P> and <P^dagger P O>.
+ *
+ * Citations: "P:<n>" = line n of the paper text; "S8" = SURVEY.md section 8;
+ * "DESIGN R<k>" = reading k in DESIGN.md.
+ *
+ * Conventions (S8): directions mu = 0 (time), 1,2,3 = x,y,z.  Site index
+ * i = x1 + Ns*(x2 + Ns*(x3 + Ns*t)); parity (x1+x2+x3+t) mod 2.  "Canonical" link arrays
+ * at this boundary are HOST pointers to float[4][Nt][Ns][Ns][Ns] (mu slowest, x1 fastest),
+ * fp32 radians in [-pi, pi].  Inside the library the links live in HBM as fp32 angles in a
+ * parity-split, direction-split structure of arrays.
+ *
+ * Ownership: the library owns the handle.  Every host pointer passed in is caller-owned and
+ * only read or written during the call.  With ul_create_ext the caller also owns the device
+ * buffers (e.g. torch.empty) and the stream (e.g. torch.cuda.Stream.cuda_stream); they must
+ * outlive the handle and the library never frees them.  With ul_create the library
+ * cudaMallocs and frees its own buffers and uses its own stream.
+ *
+ * Errors: every call returns UL_OK (0) or a negative code; nothing aborts or throws.
+ * ul_last_error(h) returns a static / handle-owned string describing the last failure.
+ * All calls are synchronous with respect to the host unless stated (ul_sweep and the
+ * multilevel calls only enqueue on the handle's stream; reads synchronise).
+ * There is no CPU fallback: without a CUDA device every call that touches the lattice
+ * returns UL_ECUDA.
+ */
+#ifndef UL_H
+#define UL_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ul_ctx ul_ctx;
+enum { UL_OK = 0, UL_EINVAL = -1, UL_ENOMEM = -2, UL_ECUDA = -3, UL_ESTATE = -4 };
+
+/* ---- set-up ------------------------------------------------------------------ */
+
+/* Lattice Ns^3 x Nt (both even, >= 2; the checkerboard of P:374 needs even extents), Wilson
+ * coupling beta >= 0, 64-bit seed.  Makes a hot start theta ~ U[-pi,pi) from the seed
+ * (Philox tag 1, S8(c)-O4) and sets the sweep counter to 0.  UL_EINVAL on bad sizes/beta,
+ * UL_ECUDA if no device, UL_ENOMEM if the link array cannot be allocated. */
+int ul_create(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed);
+
+/* Same, on caller-owned DEVICE memory and stream.  dev_links: >= 4*V*4 bytes, 256-byte
+ * aligned.  dev_work: workspace for the multilevel accumulators and reduction scratch, may
+ * be NULL/0 (then measurement calls cudaMalloc what they need), else it must hold
+ * ul_workspace_bytes(...) of the measurement that will be requested (UL_ENOMEM otherwise).
+ * cuda_stream: a cudaStream_t (NULL = default stream). */
+int ul_create_ext(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed,
+                  void* dev_links, size_t links_bytes,
+                  void* dev_work, size_t work_bytes, void* cuda_stream);
+
+/* Bytes of device workspace a measurement needs: accumulators of rows a7-a9 of S8(a)
+ * (Ns^3*(Nt/d)*3*r_max complex fp64, times (1 + 12*n_fp) with field points, for each level)
+ * plus per-configuration scratch.  d_out = 0 for a single-level measurement. */
+size_t ul_workspace_bytes(int Ns, int Nt, int d_in, int d_out, int r_max, int n_fp);
+
+int ul_destroy(ul_ctx* h);
+
+/* mode 0: cold start theta = 0; mode 1: hot start from the seed (same as ul_create). */
+int ul_init(ul_ctx* h, int mode);
+int ul_set_beta(ul_ctx* h, double beta);
+
+/* Canonical HOST array in / out (see top).  ul_set_links returns UL_EINVAL if any angle is
+ * NaN or has |theta| > 3.2 (angles must already be wrapped; the fixed-point staple sums of
+ * DESIGN.md "Arithmetic" assume |theta| <= pi up to rounding). */
+int ul_set_links(ul_ctx* h, const float* host_links);
+int ul_get_links(ul_ctx* h, float* host_links);
+
+/* 64-bit count of heatbath sweeps issued so far = the Philox counter words 1,2 (S8(c)-O4).
+ * State = links + counter + seed: restoring both resumes a run bit for bit. */
+int ul_get_counter(ul_ctx* h, uint64_t* sweep_counter);
+int ul_set_counter(ul_ctx* h, uint64_t sweep_counter);
+
+/* ---- updates (S8(a) rows a2-a6) -------------------------------------------- */
+
+/* n_hb heatbath sweeps, then n_or overrelaxation sweeps, of the whole lattice.  One sweep =
+ * 8 sub-steps: parity outer (even, odd: P:374), direction inner (0..3), in place.  Heatbath
+ * draws theta' = alpha + phi, phi ~ exp(beta k cos phi), from the staple sum k e^{i alpha}
+ * (DESIGN R2: Best-Fisher rejection, Philox4x32-10 keyed by (seed; site, sweep, attempt,
+ * parity, mu)); overrelaxation sets theta' = 2 alpha - theta.  Asynchronous on the stream. */
+int ul_sweep(ul_ctx* h, int n_hb, int n_or);
+
+/* Test hook: one sub-step.  kind 0 = heatbath (draws with the current sweep counter, does
+ * not advance it), 1 = overrelaxation.  slab_d > 0 freezes spatial links (mu != 0) on time
+ * layers t % slab_d == 0; 0 = no mask.  Nt % slab_d must be 0. */
+int ul_substep(ul_ctx* h, int kind, int parity, int mu, int slab_d);
+
+/* Sub-update recipe used inside the multilevel calls: k_sweeps x (n_hb HB + n_or OR) masked
+ * sweeps between measurements.  Default 1 HB + 3 OR, k_sweeps = 1 (DESIGN R4, R5). */
+int ul_set_subupdate(ul_ctx* h, int n_hb, int n_or, int k_sweeps);
+
+/* ---- multilevel measurement (Alg. 1; S8(a) rows a6-a10, a13) -------- */
+
+/* Single level.  Repeats n_sub times { sub-update with spatial links frozen on layers
+ * t % slab_thickness == 0; accumulate T^(d)(x,s,mu,r) (Eq. 22, Eq. 25) for
+ * mu = 1..3, r = 1..r_max and, for each field point, T^(d) * sum_{t in slab} O_ch (Eq. 31
+ * P:340) }, then forms the slab averages, their product over slabs and the lattice average
+ * (Eq. 26, Eq. 34).  n_sub = 0 measures the current configuration once
+ * without updating (naive estimator).  field_points: HOST int[n_fp][3] = (a,b,c) in the
+ * charge-aligned frame of S8(b): y = x + (floor(r/2)+a) mu + b nu + c rho, nu = 1+(mu mod 3),
+ * rho = 1+((mu+1) mod 3); may be NULL with n_fp = 0.
+ * UL_EINVAL: Nt % slab_thickness != 0, r_max < 1 or > Ns/2, n_sub < 0, bad field points.
+ * UL_ENOMEM: accumulators exceed the caller's workspace / device memory. */
+int ul_multilevel(ul_ctx* h, int slab_thickness, int n_sub, int r_max,
+                  const int* field_points, int n_fp);
+
+/* Two levels (Eq. 27, Eqs. 32-33 P:343-347 with DESIGN R7, Alg. 1 lines 5-18):
+ * n_out x { sub-update masked with d_out; n_in x { sub-update masked with d_in; accumulate
+ * T^(d_in), TO^(d_in) }; combine the m = d_out/d_in inner slab averages of each outer slab
+ * and accumulate }.  Needs d_in | d_out | Nt, n_in >= 1, n_out >= 1. */
+int ul_multilevel2(ul_ctx* h, int d_in, int n_in, int d_out, int n_out, int r_max,
+                   const int* field_points, int n_fp);
+
+/* Test hooks: open a single-level measurement, add the current configuration to the slab
+ * sums (rows a7, a8), close (row a10).  ul_accumulate returns UL_ESTATE if none is open. */
+int ul_measure_begin(ul_ctx* h, int slab_thickness, int r_max, const int* field_points, int n_fp);
+int ul_accumulate(ul_ctx* h);
+int ul_measure_end(ul_ctx* h);
+
+/* Mean of cos theta_P (Eq. 6) over all 6V plaquettes, over the 3V time-like and the
+ * 3V space-like ones: HOST double[3].  Synchronises. */
+int ul_plaquette(ul_ctx* h, double* mean_cos);
+
+/* Results of the last measurement, HOST buffers (any may be NULL):
+ * corr[r_max][2]           C(r) = (1/3Ns^3) sum_x sum_mu prod_s [T](x,s,mu,r)       (re, im)
+ * field[r_max][n_fp][12][2] G(r,fp,ch) of Eq. 34; ch = 2*comp + kind, comp 0..5 = plaquette
+ *                          orientations (0,mu) (0,nu) (0,rho) (nu,rho) (rho,mu) (mu,nu),
+ *                          kind 0 = 1 - cos theta_P, 1 = sin theta_P (Eqs. 28-29
+ *                          without the beta factors)
+ * vacuum[12]               <O_ch> over all sites, times and the three frames.
+ * UL_ESTATE before any measurement.  Synchronises. */
+int ul_read_correlators(ul_ctx* h, double* corr, double* field, double* vacuum);
+
+/* Slab averages [T] of the last measurement (outer level for two levels), HOST
+ * double[3][r_max][n_slab][Ns^3][2], xs = x1 + Ns*(x2 + Ns*x3).  Test hook for parity P2. */
+int ul_read_slab_averages(ul_ctx* h, double* out);
+
+/* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
+int ul_get_launch_count(ul_ctx* h, uint64_t* n);
+
+/* Philox4x32-10 known-answer hook: runs the DEVICE generator on n (ctr[4], key[2]) tuples.
+ * HOST pointers: ctr uint32[n][4], key uint32[n][2], out uint32[n][4]. */
+int ul_philox_selftest(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int n);
+
+/* Blocks until everything enqueued on the handle's stream has finished. */
+int ul_sync(ul_ctx* h);
+
+const char* ul_last_error(ul_ctx* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

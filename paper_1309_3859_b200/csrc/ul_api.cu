@@ -1,0 +1,505 @@
+// ul_api.cu -- host driver and C ABI of libul.so (include/ul.h).
+//
+// The host only enqueues kernels: the sweep schedule (S8(c)-O5), the sub-update recipe
+// and the nesting of Algorithm 1.  Every arithmetic step of the hot
+// path runs in the kernels of ul_update.cuh / ul_measure.cuh.  There is no CPU fallback.
+#include "../../include/ul.h"
+
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "ul_measure.cuh"
+#include "ul_update.cuh"
+
+namespace {
+
+constexpr int NBLK = 592;   // blocks of the two-stage reductions: 4 per SM on 148 SMs
+
+struct Workspace {           // byte offsets into the measurement workspace
+    size_t Th = 0, Ot = 0, fps = 0, A2 = 0, B2 = 0, A4 = 0, B4 = 0, partial = 0, result = 0, total = 0;
+};
+
+size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
+
+Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_fp) {
+    Workspace w;
+    const size_t Vs = (size_t)Ns * Ns * Ns;
+    const size_t n_in = (size_t)(Nt / d_in), n_out = d_out > 0 ? (size_t)(Nt / d_out) : 0;
+    const size_t F12 = (size_t)n_fp * 12, R = (size_t)r_max;
+    size_t o = 0;
+    w.Th = o;  o = align_up(o + n_in * Vs * sizeof(int));
+    w.Ot = o;  o = align_up(o + 12 * n_in * Vs * sizeof(float));
+    w.fps = o; o = align_up(o + (size_t)(n_fp > 0 ? n_fp : 1) * 3 * sizeof(int));
+    w.A2 = o;  o = align_up(o + 3 * R * n_in * Vs * 16);
+    w.B2 = o;  o = align_up(o + 3 * R * n_in * F12 * Vs * 16);
+    w.A4 = o;  o = align_up(o + 3 * R * n_out * Vs * 16);
+    w.B4 = o;  o = align_up(o + 3 * R * n_out * F12 * Vs * 16);
+    const size_t n_entries = R * (1 + F12);
+    size_t np = 2 * n_entries;
+    if (np < 12) np = 12;
+    w.partial = o; o = align_up(o + np * NBLK * sizeof(double));
+    w.result = o;  o = align_up(o + (2 * n_entries + 12 + 12) * sizeof(double));   // corr|field, vacuum, column sums
+    w.total = o;
+    return w;
+}
+
+}  // namespace
+
+struct ul_ctx {
+    int Ns = 0, Nt = 0, Nh = 0;
+    long long Vs = 0, V = 0, Vh = 0;
+    double beta = 0;
+    uint64_t seed = 0, sweep = 0, launches = 0;
+    cudaStream_t stream = nullptr;
+    bool own_stream = false;
+    float* th = nullptr;
+    bool own_th = false;
+    char* work = nullptr;      // measurement workspace in use
+    size_t work_bytes = 0;
+    bool own_work = false;     // library-allocated (grown on demand) vs caller-owned
+    float* staging = nullptr;  // canonical device copy for set/get links
+    double* scratch = nullptr; // [2*NBLK + 4] plaquette partials and sums
+    int* d_bad = nullptr;
+    int vec = 1, bx = 1, by = 1, bz = 1;
+    int sub_hb = 1, sub_or = 3, sub_k = 1;
+    // open measurement
+    bool open = false;
+    int d = 0, r_max = 0, n_fp = 0, n_slab = 0, d_out = 0, n_outer = 0;
+    long long n_acc = 0;
+    Workspace ws;
+    // last result
+    bool have = false;
+    int res_r_max = 0, res_n_fp = 0, res_n_slab = 0;
+    const double2* res_A = nullptr;
+    double res_inv = 1.0;
+    std::vector<double> corr, field, vacuum;
+    std::string err;
+};
+
+namespace {
+
+std::string g_err;   // errors without a handle
+
+int fail(ul_ctx* c, int code, const std::string& msg) {
+    if (c) c->err = msg; else g_err = msg;
+    return code;
+}
+#define UL_CUDA(c, call)                                                                       \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess)                                                                 \
+            return fail((c), e_ == cudaErrorMemoryAllocation ? UL_ENOMEM : UL_ECUDA,           \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                   \
+    } while (0)
+
+ulk::Geom geom(const ul_ctx* c) {
+    ulk::Geom g;
+    g.Ns = c->Ns; g.Nh = c->Nh; g.Nt = c->Nt; g.Vs = c->Vs; g.V = c->V; g.Vh = c->Vh;
+    return g;
+}
+
+int largest_divisor_le(int n, int cap) {
+    int best = 1;
+    for (int v = 1; v <= n && v <= cap; ++v)
+        if (n % v == 0) best = v;
+    return best;
+}
+
+template <int KIND, int MU>
+cudaError_t launch_update_vec(const ul_ctx* c, const ulk::UpdateArgs& a, dim3 grid, dim3 block) {
+    switch (c->vec) {
+        case 4: ulk::k_update<KIND, MU, 4><<<grid, block, 0, c->stream>>>(a); break;
+        case 2: ulk::k_update<KIND, MU, 2><<<grid, block, 0, c->stream>>>(a); break;
+        default: ulk::k_update<KIND, MU, 1><<<grid, block, 0, c->stream>>>(a); break;
+    }
+    return cudaGetLastError();
+}
+template <int KIND>
+cudaError_t launch_update_mu(const ul_ctx* c, int mu, const ulk::UpdateArgs& a, dim3 grid, dim3 block) {
+    switch (mu) {
+        case 0: return launch_update_vec<KIND, 0>(c, a, grid, block);
+        case 1: return launch_update_vec<KIND, 1>(c, a, grid, block);
+        case 2: return launch_update_vec<KIND, 2>(c, a, grid, block);
+        default: return launch_update_vec<KIND, 3>(c, a, grid, block);
+    }
+}
+
+// one sub-step (kind, parity, mu), optionally slab-masked: rows a3-a6
+int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
+    int n_t = c->Nt;
+    if (slab_d > 0 && mu != 0) n_t = c->Nt / slab_d * (slab_d - 1);
+    if (n_t == 0) return UL_OK;                       // thickness 1: every spatial link is frozen
+    ulk::UpdateArgs a;
+    a.th = c->th; a.Vh = c->Vh; a.Ns = c->Ns; a.Nh = c->Nh; a.Nt = c->Nt;
+    a.parity = parity; a.slab_d = slab_d; a.beta = (float)c->beta;
+    a.key0 = (uint32_t)(c->seed & 0xffffffffu); a.key1 = (uint32_t)(c->seed >> 32);
+    a.sweep_lo = (uint32_t)(c->sweep & 0xffffffffu); a.sweep_hi = (uint32_t)(c->sweep >> 32);
+    const dim3 block(c->bx, c->by, c->bz), grid(c->Ns / c->by, c->Ns / c->bz, n_t);
+    const cudaError_t e = kind == 0 ? launch_update_mu<0>(c, mu, a, grid, block) : launch_update_mu<1>(c, mu, a, grid, block);
+    if (e != cudaSuccess) return fail(c, UL_ECUDA, std::string("k_update launch: ") + cudaGetErrorString(e));
+    c->launches += 1;
+    return UL_OK;
+}
+int one_sweep(ul_ctx* c, int kind, int slab_d) {      // O5: parity outer, direction inner
+    for (int parity = 0; parity < 2; ++parity)
+        for (int mu = 0; mu < 4; ++mu) {
+            const int rc = substep(c, kind, parity, mu, slab_d);
+            if (rc) return rc;
+        }
+    if (kind == 0) c->sweep += 1;
+    return UL_OK;
+}
+int compound(ul_ctx* c, int n_hb, int n_or, int slab_d) {
+    for (int i = 0; i < n_hb; ++i) { const int rc = one_sweep(c, 0, slab_d); if (rc) return rc; }
+    for (int i = 0; i < n_or; ++i) { const int rc = one_sweep(c, 1, slab_d); if (rc) return rc; }
+    return UL_OK;
+}
+
+int check_meas_args(ul_ctx* c, int d, int r_max, const int* fps, int n_fp) {
+    if (d < 1 || c->Nt % d != 0) return fail(c, UL_EINVAL, "Nt % slab_thickness != 0");
+    if (r_max < 1 || r_max > c->Ns / 2) return fail(c, UL_EINVAL, "r_max out of range [1, Ns/2]");
+    if (n_fp < 0 || (n_fp > 0 && !fps)) return fail(c, UL_EINVAL, "bad field points");
+    return UL_OK;
+}
+
+template <typename T> T* wsp(ul_ctx* c, size_t off) { return reinterpret_cast<T*>(c->work + off); }
+
+// reserve the workspace, upload the field points, zero the accumulators
+int open_measurement(ul_ctx* c, int d_in, int d_out, int r_max, const int* fps, int n_fp) {
+    const Workspace w = plan_workspace(c->Ns, c->Nt, d_in, d_out, r_max, n_fp);
+    if (w.total > c->work_bytes) {
+        if (!c->own_work && c->work) return fail(c, UL_ENOMEM, "accumulators exceed the caller's workspace");
+        if (c->work) { UL_CUDA(c, cudaStreamSynchronize(c->stream)); cudaFree(c->work); c->work = nullptr; c->work_bytes = 0; }
+        void* p = nullptr;
+        UL_CUDA(c, cudaMalloc(&p, w.total));
+        c->work = (char*)p; c->work_bytes = w.total; c->own_work = true;
+    }
+    c->ws = w;
+    c->d = d_in; c->d_out = d_out; c->r_max = r_max; c->n_fp = n_fp;
+    c->n_slab = c->Nt / d_in; c->n_outer = d_out > 0 ? c->Nt / d_out : 0;
+    c->n_acc = 0;
+    c->have = false;
+    if (n_fp > 0) UL_CUDA(c, cudaMemcpyAsync(c->work + w.fps, fps, sizeof(int) * 3 * (size_t)n_fp, cudaMemcpyHostToDevice, c->stream));
+    UL_CUDA(c, cudaMemsetAsync(c->work + w.A2, 0, w.partial - w.A2, c->stream));           // A2, B2, A4, B4
+    UL_CUDA(c, cudaMemsetAsync(c->work + w.result, 0, w.total - w.result, c->stream));
+    if (n_fp > 0) UL_CUDA(c, cudaStreamSynchronize(c->stream));                            // fps is a caller-owned host buffer
+    c->open = true;
+    return UL_OK;
+}
+
+double* res_colsum(ul_ctx* c) { return wsp<double>(c, c->ws.result) + 2 * (size_t)c->r_max * (1 + 12 * (size_t)c->n_fp) + 12; }
+double* res_vacuum(ul_ctx* c) { return wsp<double>(c, c->ws.result) + 2 * (size_t)c->r_max * (1 + 12 * (size_t)c->n_fp); }
+
+// rows a7, a8 on the current configuration
+int accumulate(ul_ctx* c) {
+    const ulk::Geom g = geom(c);
+    const long long n = (long long)c->n_slab * c->Vs;
+    const int nb = (int)((n + 255) / 256);
+    ulk::k_slab_tables<<<nb, 256, 0, c->stream>>>(g, c->th, c->d, c->n_slab, wsp<int>(c, c->ws.Th), wsp<float>(c, c->ws.Ot));
+    ulk::AccumArgs a;
+    a.g = g; a.d = c->d; a.n_slab = c->n_slab; a.r_max = c->r_max; a.n_fp = c->n_fp;
+    a.Th = wsp<int>(c, c->ws.Th); a.Ot = wsp<float>(c, c->ws.Ot); a.fps = wsp<int>(c, c->ws.fps);
+    a.A = wsp<double2>(c, c->ws.A2); a.B = wsp<double2>(c, c->ws.B2);
+    ulk::k_accumulate<<<nb, 256, 0, c->stream>>>(a);
+    ulk::k_ot_colsum<<<dim3(NBLK, 12), 256, 0, c->stream>>>(wsp<float>(c, c->ws.Ot), n, wsp<double>(c, c->ws.partial));
+    ulk::k_sum_partials<<<12, 256, 0, c->stream>>>(wsp<double>(c, c->ws.partial), NBLK, res_colsum(c), 1.0, 1);
+    UL_CUDA(c, cudaGetLastError());
+    c->launches += 4;
+    c->n_acc += 1;
+    return UL_OK;
+}
+
+// row a10 on accumulators (A, B) with n_slab slabs, scaled by inv; results to the host vectors
+int finish(ul_ctx* c, const double2* A, const double2* B, int n_slab, double inv, double vac_inv) {
+    const int R = c->r_max, F = c->n_fp;
+    const int n_entries = R * (1 + 12 * F);
+    ulk::ReduceArgs a;
+    a.Vs = c->Vs; a.r_max = R; a.n_fp = F; a.n_slab = n_slab; a.inv = inv; a.A = A; a.B = B;
+    a.partial = wsp<double>(c, c->ws.partial);
+    ulk::k_slab_product<<<dim3(NBLK, n_entries), 256, 0, c->stream>>>(a);
+    double* res = wsp<double>(c, c->ws.result);
+    // C /= 3 Vs ; G /= 3 Vs Nt (DESIGN R9)
+    ulk::k_sum_partials<<<2 * R, 256, 0, c->stream>>>(a.partial, NBLK, res, 1.0 / (3.0 * (double)c->Vs), 0);
+    c->launches += 2;
+    if (F > 0) {
+        ulk::k_sum_partials<<<2 * (n_entries - R), 256, 0, c->stream>>>(a.partial + (size_t)2 * R * NBLK, NBLK, res + 2 * R,
+                                                                        1.0 / (3.0 * (double)c->Vs * (double)c->Nt), 0);
+        c->launches += 1;
+    }
+    ulk::k_vacuum<<<1, 32, 0, c->stream>>>(res_colsum(c), vac_inv / (3.0 * (double)c->V), res_vacuum(c));
+    c->launches += 1;
+    UL_CUDA(c, cudaGetLastError());
+    std::vector<double> host((size_t)2 * n_entries + 12);
+    UL_CUDA(c, cudaMemcpyAsync(host.data(), res, sizeof(double) * host.size(), cudaMemcpyDeviceToHost, c->stream));
+    UL_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->corr.assign(host.begin(), host.begin() + 2 * R);
+    c->field.assign(host.begin() + 2 * R, host.begin() + 2 * n_entries);
+    c->vacuum.assign(host.begin() + 2 * n_entries, host.end());
+    c->res_r_max = R; c->res_n_fp = F; c->res_n_slab = n_slab; c->res_A = A; c->res_inv = inv;
+    c->have = true;
+    c->open = false;
+    return UL_OK;
+}
+
+int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* dev_links, size_t links_bytes,
+                  void* dev_work, size_t work_bytes, void* stream, bool ext) {
+    if (!h) return fail(nullptr, UL_EINVAL, "null handle pointer");
+    *h = nullptr;
+    if (Ns < 2 || Nt < 2 || (Ns & 1) || (Nt & 1) || !(beta >= 0.0)) return fail(nullptr, UL_EINVAL, "need even Ns, Nt >= 2 and beta >= 0");
+    const int Nh = Ns / 2;
+    const int vec = (Nh % 4 == 0) ? 4 : ((Nh % 2 == 0) ? 2 : 1);
+    if (Nh / vec > 256 || (double)Ns * Ns * Ns * Nt > 4.0e9) return fail(nullptr, UL_EINVAL, "lattice too large for this build");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(nullptr, UL_ECUDA, "no CUDA device");
+    ul_ctx* c = new (std::nothrow) ul_ctx;
+    if (!c) return fail(nullptr, UL_ENOMEM, "host allocation failed");
+    c->Ns = Ns; c->Nt = Nt; c->Nh = Nh;
+    c->Vs = (long long)Ns * Ns * Ns; c->V = c->Vs * Nt; c->Vh = c->V / 2;
+    c->beta = beta; c->seed = seed;
+    c->vec = vec; c->bx = Nh / vec;
+    c->by = largest_divisor_le(Ns, 256 / c->bx);
+    c->bz = largest_divisor_le(Ns, 256 / (c->bx * c->by));
+    const size_t need = sizeof(float) * 4 * (size_t)c->V;
+    if (ext) {
+        if (!dev_links || links_bytes < need || ((uintptr_t)dev_links & 255)) { delete c; return fail(nullptr, UL_EINVAL, "dev_links too small or misaligned"); }
+        c->th = (float*)dev_links;
+        c->stream = (cudaStream_t)stream;
+        if (dev_work && work_bytes) { c->work = (char*)dev_work; c->work_bytes = work_bytes; c->own_work = false; }
+        else c->own_work = true;
+    } else {
+        void* p = nullptr;
+        cudaError_t e = cudaMalloc(&p, need);
+        if (e != cudaSuccess) { delete c; return fail(nullptr, UL_ENOMEM, std::string("cudaMalloc links: ") + cudaGetErrorString(e)); }
+        c->th = (float*)p; c->own_th = true;
+        e = cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) { cudaFree(p); delete c; return fail(nullptr, UL_ECUDA, std::string("cudaStreamCreate: ") + cudaGetErrorString(e)); }
+        c->own_stream = true; c->own_work = true;
+    }
+    void* s = nullptr;
+    if (cudaMalloc(&s, sizeof(double) * (2 * NBLK + 4) + 256) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ENOMEM, "cudaMalloc scratch"); }
+    c->scratch = (double*)s;
+    c->d_bad = (int*)((char*)s + sizeof(double) * (2 * NBLK + 4));
+    *h = c;
+    const int rc = ul_init(c, 1);
+    if (rc) { g_err = c->err; ul_destroy(c); *h = nullptr; }
+    return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ul_create(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed) {
+    return create_common(h, Ns, Nt, beta, seed, nullptr, 0, nullptr, 0, nullptr, false);
+}
+int ul_create_ext(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* dev_links, size_t links_bytes,
+                  void* dev_work, size_t work_bytes, void* cuda_stream) {
+    return create_common(h, Ns, Nt, beta, seed, dev_links, links_bytes, dev_work, work_bytes, cuda_stream, true);
+}
+size_t ul_workspace_bytes(int Ns, int Nt, int d_in, int d_out, int r_max, int n_fp) {
+    if (Ns < 2 || Nt < 2 || d_in < 1 || Nt % d_in != 0 || d_out < 0 || (d_out > 0 && (d_out % d_in != 0 || Nt % d_out != 0)) ||
+        r_max < 1 || n_fp < 0)
+        return 0;
+    return plan_workspace(Ns, Nt, d_in, d_out, r_max, n_fp).total;
+}
+int ul_destroy(ul_ctx* c) {
+    if (!c) return UL_OK;
+    cudaStreamSynchronize(c->stream);
+    if (c->own_th && c->th) cudaFree(c->th);
+    if (c->own_work && c->work) cudaFree(c->work);
+    if (c->staging) cudaFree(c->staging);
+    if (c->scratch) cudaFree(c->scratch);
+    if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
+    delete c;
+    return UL_OK;
+}
+
+int ul_init(ul_ctx* c, int mode) {
+    if (!c || (mode != 0 && mode != 1)) return fail(c, UL_EINVAL, "mode must be 0 or 1");
+    if (mode == 0) {
+        UL_CUDA(c, cudaMemsetAsync(c->th, 0, sizeof(float) * 4 * (size_t)c->V, c->stream));
+        return UL_OK;
+    }
+    const long long n = 4 * c->V;
+    ulk::k_hot_start<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(geom(c), c->th, (uint32_t)(c->seed & 0xffffffffu),
+                                                                         (uint32_t)(c->seed >> 32));
+    UL_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    return UL_OK;
+}
+int ul_set_beta(ul_ctx* c, double beta) {
+    if (!c || !(beta >= 0.0)) return fail(c, UL_EINVAL, "beta must be >= 0");
+    c->beta = beta;
+    return UL_OK;
+}
+
+static int ensure_staging(ul_ctx* c) {
+    if (c->staging) return UL_OK;
+    void* p = nullptr;
+    UL_CUDA(c, cudaMalloc(&p, sizeof(float) * 4 * (size_t)c->V));
+    c->staging = (float*)p;
+    return UL_OK;
+}
+int ul_set_links(ul_ctx* c, const float* host) {
+    if (!c || !host) return fail(c, UL_EINVAL, "null pointer");
+    int rc = ensure_staging(c);
+    if (rc) return rc;
+    const long long n = 4 * c->V;
+    UL_CUDA(c, cudaMemsetAsync(c->d_bad, 0, sizeof(int), c->stream));
+    UL_CUDA(c, cudaMemcpyAsync(c->staging, host, sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
+    ulk::k_repack<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(geom(c), c->th, c->staging, 1, c->d_bad);
+    UL_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    int bad = 0;
+    UL_CUDA(c, cudaMemcpyAsync(&bad, c->d_bad, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    UL_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (bad) return fail(c, UL_EINVAL, "link angles must be finite with |theta| <= 3.2 (wrap them to [-pi, pi] first)");
+    return UL_OK;
+}
+int ul_get_links(ul_ctx* c, float* host) {
+    if (!c || !host) return fail(c, UL_EINVAL, "null pointer");
+    int rc = ensure_staging(c);
+    if (rc) return rc;
+    const long long n = 4 * c->V;
+    ulk::k_repack<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(geom(c), c->th, c->staging, 0, c->d_bad);
+    UL_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    UL_CUDA(c, cudaMemcpyAsync(host, c->staging, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, c->stream));
+    UL_CUDA(c, cudaStreamSynchronize(c->stream));
+    return UL_OK;
+}
+int ul_get_counter(ul_ctx* c, uint64_t* v) { if (!c || !v) return fail(c, UL_EINVAL, "null pointer"); *v = c->sweep; return UL_OK; }
+int ul_set_counter(ul_ctx* c, uint64_t v) { if (!c) return fail(c, UL_EINVAL, "null handle"); c->sweep = v; return UL_OK; }
+
+int ul_sweep(ul_ctx* c, int n_hb, int n_or) {
+    if (!c || n_hb < 0 || n_or < 0) return fail(c, UL_EINVAL, "n_hb, n_or must be >= 0");
+    return compound(c, n_hb, n_or, 0);
+}
+int ul_substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
+    if (!c || (kind != 0 && kind != 1) || (parity != 0 && parity != 1) || mu < 0 || mu > 3 || slab_d < 0)
+        return fail(c, UL_EINVAL, "bad sub-step arguments");
+    if (slab_d > 0 && c->Nt % slab_d != 0) return fail(c, UL_EINVAL, "Nt % slab_d != 0");
+    return substep(c, kind, parity, mu, slab_d);
+}
+int ul_set_subupdate(ul_ctx* c, int n_hb, int n_or, int k_sweeps) {
+    if (!c || n_hb < 0 || n_or < 0 || k_sweeps < 1) return fail(c, UL_EINVAL, "bad sub-update recipe");
+    c->sub_hb = n_hb; c->sub_or = n_or; c->sub_k = k_sweeps;
+    return UL_OK;
+}
+
+int ul_measure_begin(ul_ctx* c, int d, int r_max, const int* fps, int n_fp) {
+    if (!c) return fail(c, UL_EINVAL, "null handle");
+    const int rc = check_meas_args(c, d, r_max, fps, n_fp);
+    if (rc) return rc;
+    return open_measurement(c, d, 0, r_max, fps, n_fp);
+}
+int ul_accumulate(ul_ctx* c) {
+    if (!c) return fail(c, UL_EINVAL, "null handle");
+    if (!c->open) return fail(c, UL_ESTATE, "no open measurement");
+    return accumulate(c);
+}
+int ul_measure_end(ul_ctx* c) {
+    if (!c) return fail(c, UL_EINVAL, "null handle");
+    if (!c->open || c->n_acc == 0) return fail(c, UL_ESTATE, "nothing accumulated");
+    const double inv = 1.0 / (double)c->n_acc;
+    return finish(c, wsp<double2>(c, c->ws.A2), wsp<double2>(c, c->ws.B2), c->n_slab, inv, inv);
+}
+
+int ul_multilevel(ul_ctx* c, int d, int n_sub, int r_max, const int* fps, int n_fp) {
+    if (!c || n_sub < 0) return fail(c, UL_EINVAL, "n_sub must be >= 0");
+    int rc = ul_measure_begin(c, d, r_max, fps, n_fp);
+    if (rc) return rc;
+    if (n_sub == 0) { rc = accumulate(c); if (rc) return rc; }
+    for (int j = 0; j < n_sub; ++j) {
+        for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d); if (rc) return rc; }
+        rc = accumulate(c);
+        if (rc) return rc;
+    }
+    return ul_measure_end(c);
+}
+
+int ul_multilevel2(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, int r_max, const int* fps, int n_fp) {
+    if (!c || n_in < 1 || n_out < 1) return fail(c, UL_EINVAL, "n_in, n_out must be >= 1");
+    int rc = check_meas_args(c, d_in, r_max, fps, n_fp);
+    if (rc) return rc;
+    if (d_out < d_in || d_out % d_in != 0 || c->Nt % d_out != 0) return fail(c, UL_EINVAL, "need d_in | d_out | Nt");
+    rc = open_measurement(c, d_in, d_out, r_max, fps, n_fp);
+    if (rc) return rc;
+    const Workspace& w = c->ws;
+    ulk::CombineArgs a;
+    a.Vs = c->Vs; a.r_max = r_max; a.n_fp = n_fp; a.n_inner = c->n_slab; a.n_outer = c->n_outer; a.m = d_out / d_in;
+    a.inv = 1.0 / (double)n_in;
+    a.A2 = wsp<double2>(c, w.A2); a.B2 = wsp<double2>(c, w.B2); a.A4 = wsp<double2>(c, w.A4); a.B4 = wsp<double2>(c, w.B4);
+    const long long total = 3LL * r_max * c->n_outer * c->Vs;
+    for (int J = 0; J < n_out; ++J) {
+        for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d_out); if (rc) return rc; }
+        if (J > 0) UL_CUDA(c, cudaMemsetAsync(c->work + w.A2, 0, w.A4 - w.A2, c->stream));   // A2, B2 <- 0
+        for (int j = 0; j < n_in; ++j) {
+            for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d_in); if (rc) return rc; }
+            rc = accumulate(c);
+            if (rc) return rc;
+        }
+        ulk::k_combine<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>(a);          // Eqs. 32-33
+        UL_CUDA(c, cudaGetLastError());
+        c->launches += 1;
+    }
+    return finish(c, a.A4, a.B4, c->n_outer, 1.0 / (double)n_out, 1.0 / ((double)n_in * (double)n_out));
+}
+
+int ul_plaquette(ul_ctx* c, double* out) {
+    if (!c || !out) return fail(c, UL_EINVAL, "null pointer");
+    ulk::k_plaquette<<<NBLK, 256, 0, c->stream>>>(geom(c), c->th, c->scratch);
+    ulk::k_sum_partials<<<2, 256, 0, c->stream>>>(c->scratch, NBLK, c->scratch + 2 * NBLK, 1.0 / (3.0 * (double)c->V), 0);
+    UL_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    double v[2];
+    UL_CUDA(c, cudaMemcpyAsync(v, c->scratch + 2 * NBLK, sizeof(v), cudaMemcpyDeviceToHost, c->stream));
+    UL_CUDA(c, cudaStreamSynchronize(c->stream));
+    out[0] = 0.5 * (v[0] + v[1]); out[1] = v[0]; out[2] = v[1];
+    return UL_OK;
+}
+int ul_read_correlators(ul_ctx* c, double* corr, double* field, double* vacuum) {
+    if (!c) return fail(c, UL_EINVAL, "null handle");
+    if (!c->have) return fail(c, UL_ESTATE, "no measurement yet");
+    if (corr) std::memcpy(corr, c->corr.data(), sizeof(double) * c->corr.size());
+    if (field && !c->field.empty()) std::memcpy(field, c->field.data(), sizeof(double) * c->field.size());
+    if (vacuum) std::memcpy(vacuum, c->vacuum.data(), sizeof(double) * 12);
+    return UL_OK;
+}
+int ul_read_slab_averages(ul_ctx* c, double* out) {
+    if (!c || !out) return fail(c, UL_EINVAL, "null pointer");
+    if (!c->have) return fail(c, UL_ESTATE, "no measurement yet");
+    const size_t n = (size_t)3 * c->res_r_max * c->res_n_slab * (size_t)c->Vs * 2;
+    UL_CUDA(c, cudaMemcpyAsync(out, c->res_A, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
+    UL_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (size_t i = 0; i < n; ++i) out[i] *= c->res_inv;
+    return UL_OK;
+}
+int ul_get_launch_count(ul_ctx* c, uint64_t* n) { if (!c || !n) return fail(c, UL_EINVAL, "null pointer"); *n = c->launches; return UL_OK; }
+
+int ul_philox_selftest(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int n) {
+    if (!ctr || !key || !out || n < 1) return fail(nullptr, UL_EINVAL, "bad arguments");
+    uint32_t* d = nullptr;
+    UL_CUDA(nullptr, cudaMalloc((void**)&d, sizeof(uint32_t) * 10 * (size_t)n));
+    uint32_t *dc = d, *dk = d + 4 * (size_t)n, *dout = d + 6 * (size_t)n;
+    cudaError_t e = cudaMemcpy(dc, ctr, sizeof(uint32_t) * 4 * (size_t)n, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(dk, key, sizeof(uint32_t) * 2 * (size_t)n, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) { ulk::k_philox_test<<<(n + 127) / 128, 128>>>(dc, dk, dout, n); e = cudaGetLastError(); }
+    if (e == cudaSuccess) e = cudaMemcpy(out, dout, sizeof(uint32_t) * 4 * (size_t)n, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(nullptr, UL_ECUDA, cudaGetErrorString(e));
+    return UL_OK;
+}
+int ul_sync(ul_ctx* c) {
+    if (!c) return fail(c, UL_EINVAL, "null handle");
+    UL_CUDA(c, cudaStreamSynchronize(c->stream));
+    return UL_OK;
+}
+const char* ul_last_error(ul_ctx* c) { return c ? c->err.c_str() : g_err.c_str(); }
+
+}  // extern "C"
