@@ -1,0 +1,306 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the U(1) multilevel hot path on B200 (BASELINE.json config 5).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+One STEP = one pass of the whole hot path over a 64^4 lattice (beta = 0.98, hot start seed 5):
+    ul_sweep(1 HB, 4 OR)                      full compound sweep          (rows a2-a5)
+    ul_multilevel(d=2, n_sub, r_max=16)       n_sub x {slab-masked compound sub-update (1 HB + 4 OR)
+                                              + T^(2) accumulation}, slab product, reduction (a6, a7, a10, a13)
+    ul_plaquette()                                                          (row a11)
+metric = link updates per second (full + masked updates) over the whole step, inputs resident in HBM.
+`e2e` = the same step through the C ABI with HOST link buffers (ul_set_links + step + ul_get_links).
+`roofline` = the overrelaxation sub-step kernel (4 of every 5 sweeps), timed with CUDA events inside
+the timed region, against its algorithmic 36 B per link update.
+`cpu_baseline` = the oracle (oracle/ulo.cpp, single thread) on a bounded sample of the same workload.
+
+N > 1 (torchrun): every rank runs an independent lattice (seed 5 + rank), no data-path collective;
+times are the max over ranks ("weak" scaling).
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+WORKLOAD = dict(name="cfg5_64^4", Ns=64, Nt=64, beta=0.98, seed=5, n_hb=1, n_or=4, slab_d=2, n_sub=2, r_max=16)
+METRIC = "link_updates_per_s"
+UNIT = "link updates/s"
+BYTES_PER_UPDATE_OR = 36.0     # DESIGN.md / SURVEY 8(d): 3V + V/2 + V/2 reads, V/2 writes per V/2 updates, fp32
+
+
+def updates_per_step(w):
+    V = w["Ns"] ** 3 * w["Nt"]
+    sweeps = w["n_hb"] + w["n_or"]
+    full = sweeps * 4 * V
+    d = w["slab_d"]
+    masked = sweeps * (V + 3 * V * (d - 1) // d)
+    return full + w["n_sub"] * masked, full, masked
+
+
+def rank_seed(base_seed, rank):
+    """Independent problems per rank (weak scaling): rank r runs the lattice seeded base + r."""
+    return int(base_seed) + int(rank)
+
+
+def distributed_max(value, dist, device=None):
+    """max over ranks of a python float through torch.distributed (nccl on GPUs, gloo in CPU tests)."""
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.02):
+        self.index, self.period = index, period
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4),
+            "hw_power_brake": getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80),
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def start(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def measured_peak_hbm():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic():
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary, or None."""
+    p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    try:
+        return float(json.load(open(p))["k_update_or_dram_bytes_per_launch"])
+    except Exception:
+        return None
+
+
+# ------------------------------------------------------------------------------------------- oracle arm
+def oracle_sample(w, budget_s):
+    """Times the oracle, as it stands, on a bounded sample: a 64^3 x Nt_s sub-lattice of the workload
+    (same Ns, beta, seed), one heatbath + one overrelaxation sub-step (parity 0, mu 0).  Returns
+    (updates/s, description, seconds)."""
+    from oracle import ulo
+    per_update = 1.2e-6                                     # rough single-core cost, only to size the sample
+    Ns = w["Ns"]
+    nt = int(budget_s / (per_update * Ns ** 3)) // 2 * 2
+    nt = max(2, min(w["Nt"], nt))
+    o = ulo.Oracle(Ns, nt, w["beta"], w["seed"])
+    V = Ns ** 3 * nt
+    t0 = time.perf_counter()
+    o.substep(0, 0, 0, 0)
+    o.substep(1, 0, 0, 0)
+    dt = time.perf_counter() - t0
+    o.close()
+    return V / dt, f"{Ns}^3x{nt} sub-lattice of the workload, 1 HB + 1 OR sub-step (parity 0, mu 0) = {V} link updates", dt
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    w = WORKLOAD
+    total = args.steps + args.warmup
+    budget = max(0.3, min(20.0, 150.0 / max(1, total)))
+    vals, sample, secs = [], "", []
+    for i in range(total):
+        v, sample, dt = oracle_sample(w, budget)
+        if i >= args.warmup:
+            vals.append(v)
+            secs.append(dt)
+    value = sum(vals) / len(vals)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * sum(secs) / len(secs), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w["name"], "lattice": f"{w['Ns']}^3x{w['Nt']}", "beta": w["beta"], "seed": w["seed"],
+                   "note": "oracle (single-threaded C++, fp64) on a bounded sample per step"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------- our arm
+def run_ours(args, rank, local_rank, world):
+    import torch
+    from paper_1309_3859_b200 import build, ul
+    if rank == 0:
+        build.build()
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist.barrier()
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    w = WORKLOAD
+    Ns, Nt = w["Ns"], w["Nt"]
+    V = Ns ** 3 * Nt
+    ws = ul.workspace_bytes(Ns, Nt, w["slab_d"], 0, w["r_max"], 0)
+    lat = ul.Lattice(Ns, Nt, w["beta"], rank_seed(w["seed"], rank), workspace_bytes=ws, device=dev)
+    lat.set_subupdate(w["n_hb"], w["n_or"], 1)
+    n_upd, n_full, n_masked = updates_per_step(w)
+
+    ev_or = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+
+    def step(i=None):
+        lat.sweep(w["n_hb"], 0)
+        if i is not None:
+            ev_or[i][0].record()
+        lat.sweep(0, w["n_or"])
+        if i is not None:
+            ev_or[i][1].record()
+        lat.multilevel(w["slab_d"], w["n_sub"], w["r_max"])
+        return lat.plaquette()[0]
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    l0 = lat.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(args.steps):
+        plaq = step(i)
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = lat.launch_count() - l0
+    ms = e0.elapsed_time(e1)
+    or_ms = sum(a.elapsed_time(b) for a, b in ev_or) / args.steps          # 4 OR sweeps = 32 launches per step
+    if dist is not None:
+        ms = distributed_max(ms, dist, dev)
+    ms_per_step = ms / args.steps
+    value = world * n_upd / (ms_per_step * 1e-3)
+
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region
+    host_in = torch.empty(4 * V, dtype=torch.float32).pin_memory()
+    host_out = torch.empty(4 * V, dtype=torch.float32).pin_memory()
+    lat.get_links(host_in)
+    e2e_steps = max(2, min(args.steps, 5))
+    for _ in range(2):
+        lat.set_links(host_in); step(); lat.get_links(host_out)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        lat.set_links(host_in)
+        step()
+        lat.get_links(host_out)
+        lat.read_correlators()
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    if dist is not None:
+        e2e_ms = distributed_max(e2e_ms, dist, dev)
+    e2e_value = world * n_upd / (e2e_ms / e2e_steps * 1e-3)
+
+    if rank != 0:
+        return
+    peak, peak_src = measured_peak_hbm()
+    n_or_launches = 8 * w["n_or"]
+    or_launch_s = or_ms * 1e-3 / n_or_launches
+    or_bytes = BYTES_PER_UPDATE_OR * (V / 2)
+    achieved = or_bytes / or_launch_s / 1e9
+    cpu_v, cpu_sample, _ = oracle_sample(w, 12.0)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": w["name"], "lattice": f"{Ns}^3x{Nt}", "beta": w["beta"], "seed": w["seed"],
+                   "step": f"ul_sweep({w['n_hb']},{w['n_or']}) + ul_multilevel(d={w['slab_d']}, n_sub={w['n_sub']}, "
+                           f"r_max={w['r_max']}) with sub-update ({w['n_hb']} HB + {w['n_or']} OR) + ul_plaquette",
+                   "link_updates_per_step": n_upd, "slab_sweeps_per_step": w["n_sub"],
+                   "l2": "inputs larger than L2 (links 268 MB + accumulators 6.4 GB vs 126 MB L2)",
+                   "parallelism": f"replicas x{world}, independent seeds, no collective"},
+        "slab_sweeps_per_s": world * w["n_sub"] / (ms_per_step * 1e-3),
+        "plaquette": plaq,
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 16 * V, "d2h_bytes_per_step": 16 * V + 8 * (2 * w["r_max"] + 12 + 3),
+                "steps": e2e_steps},
+        "gpu_launches": int(launches),
+        "roofline": {"kernel": "k_update<OR> (overrelaxation sub-step, 32 launches per step)", "bound": "hbm",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic(),
+                     "algorithmic_bytes_per_launch": or_bytes, "avg_launch_us": or_launch_s * 1e6,
+                     "link_updates_per_s": (V / 2) / or_launch_s, "peak_source": peak_src},
+        "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": cpu_sample},
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    main()

@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(256) k_plaquette(Geom g, const float* __restri
 #pragma unroll
             for (int b = a + 1; b < 4; ++b) {
                 float c, sn;
-                ulm::sincos_fx(plaq_fx(g, th, a, b, x), c, sn);
+                ulm::sincos_fx<true>(plaq_fx(g, th, a, b, x), c, sn);
                 if (a == 0) v[0] += (double)c; else v[1] += (double)c;
             }
     }
@@ -186,7 +186,7 @@ __global__ void __launch_bounds__(256) k_slab_tables(Geom g, const float* __rest
 #pragma unroll
             for (int b = a + 1; b < 4; ++b) {
                 float c, sn;
-                ulm::sincos_fx(plaq_fx(g, th, a, b, x), c, sn);
+                ulm::sincos_fx<true>(plaq_fx(g, th, a, b, x), c, sn);
                 o_c[o] += 1.0f - c;
                 o_s[o] += sn;
                 ++o;
@@ -266,7 +266,7 @@ __global__ void __launch_bounds__(256) k_accumulate(const AccumArgs P) {
             const long long ys = y[1] + (long long)Ns * (y[2] + (long long)Ns * y[3]);
             // T^(d)(x,s,r mu) = exp(i sum_{t in slab} [theta_0(x + r mu, t) - theta_0(x, t)])  (Eq. 22, 25)
             float c, sn;
-            ulm::sincos_fx(Ths[ys] - th0, c, sn);
+            ulm::sincos_fx<true>(Ths[ys] - th0, c, sn);
             const double Tr = (double)c, Ti = (double)sn;
             const long long a_idx = (((long long)(mu - 1) * P.r_max + (r - 1)) * P.n_slab + s) * g.Vs + xs;
             double2 a = P.A[a_idx];

@@ -85,9 +85,9 @@ __device__ __forceinline__ void staple_pair(const float* __restrict__ th, long l
 #pragma unroll
     for (int i = 0; i < VEC; ++i) {
         float c, s;
-        ulm::sincos_fx(A[i] + B[i] - C[i], c, s);
+        ulm::sincos_fx<false>(A[i] + B[i] - C[i], c, s);
         Sx[i] += c; Sy[i] += s;
-        ulm::sincos_fx(D[i] + E[i] - F[i], c, s);
+        ulm::sincos_fx<false>(D[i] + E[i] - F[i], c, s);
         Sx[i] += c; Sy[i] += s;
     }
 }

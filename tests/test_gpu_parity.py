@@ -1,0 +1,446 @@
+"""GPU-vs-oracle parity (protocols P1-P3), through the C ABI.
+
+P1  link level: per sub-step and per whole sweep, |theta_gpu - theta_cpu| mod 2pi <= 2e-5 rad
+    except accept/reject flips (< 1e-5 of links) and the ill-conditioned class k < 0.05.
+P2  frozen configuration: slab averages, correlators, fields, plaquette to relative 1e-5
+    (DESIGN R17: abs <= 1e-5 * max(|cpu|, rms_term / sqrt(N))).
+P3  ensemble: independent chains agree within 3 combined standard errors.
+"""
+import numpy as np
+import pytest
+
+from tests import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL = 2e-5
+
+
+@pytest.fixture(scope="module")
+def ul():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_1309_3859_b200 import build, ul as _ul
+    build.build()
+    return _ul
+
+
+def wrapdiff(a, b):
+    d = a.astype(np.float64) - b.astype(np.float64)
+    return np.abs(d - 2 * np.pi * np.round(d / (2 * np.pi)))
+
+
+def staple_k(o, mu, flat_sites):
+    return np.array([o.staple(mu, int(s))[0] for s in flat_sites])
+
+
+def check_links(got, want, before, o_before, label, allow_frac=1e-5):
+    """P1 criterion.  o_before: oracle holding the configuration BEFORE the update (for k)."""
+    diff = wrapdiff(got, want)
+    untouched = (want == before)
+    assert np.array_equal(got[untouched & (diff == 0)], want[untouched & (diff == 0)])
+    bad = np.argwhere(diff > TOL)
+    n_links = got.size
+    n_ill = 0
+    n_other = 0
+    for idx in bad:
+        mu = int(idx[0])
+        site = int(np.ravel_multi_index(tuple(idx[1:]), got.shape[1:]))
+        k, _ = o_before.staple(mu, site)
+        if k < 0.05:
+            n_ill += 1
+        else:
+            n_other += 1          # accept/reject flip (heatbath) -- or a real bug
+    assert n_other <= max(1, allow_frac * n_links), (label, n_other, n_ill, diff.max())
+    assert n_ill <= max(2, 1e-4 * n_links), (label, n_ill)
+    return n_other, n_ill, float(diff.max())
+
+
+# ----------------------------------------------------------------------------- building blocks
+def test_philox_known_answers_on_device(ul, ulo):
+    import os
+    rows = []
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "philox4x32_10_kat.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        rows.append([int(v, 16) for v in line.split() if v != "->"])
+    rows = np.array(rows, dtype=np.uint64)
+    out = ul.philox_selftest(rows[:, 0:4], rows[:, 4:6])
+    assert np.array_equal(out, rows[:, 6:10].astype(np.uint32))
+    rng = np.random.default_rng(0)
+    ctr = rng.integers(0, 2 ** 32, size=(1000, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2 ** 32, size=(1000, 2), dtype=np.uint64).astype(np.uint32)
+    out = ul.philox_selftest(ctr, key)
+    for i in range(0, 1000, 37):
+        assert np.array_equal(out[i], ulo.philox4x32_10(ctr[i], key[i]))
+
+
+@pytest.mark.parametrize("Ns,Nt", [(2, 2), (4, 4), (6, 4), (8, 6), (16, 4)])
+def test_hot_start_and_layout_roundtrip(ul, ulo, Ns, Nt):
+    seed = (0x51 << 32) | 0xC0FFEE
+    g = ul.Lattice(Ns, Nt, 1.0, seed)
+    o = ulo.Oracle(Ns, Nt, 1.0, seed)
+    assert np.array_equal(g.get_links(), o.get_links())          # same Philox stream, bit for bit
+    links = inputs.hot_links(Ns, Nt, 3)
+    g.set_links(links)
+    assert np.array_equal(g.get_links(), links)
+    g.init(0)
+    assert not g.get_links().any()
+    g.init(1)
+    assert np.array_equal(g.get_links(), o.get_links())
+
+
+def test_set_links_rejects_unwrapped_angles(ul):
+    g = ul.Lattice(4, 4, 1.0, 1)
+    links = inputs.hot_links(4, 4, 3)
+    links[2, 1, 0, 3, 2] = 7.0
+    with pytest.raises(ul.UlError) as e:
+        g.set_links(links)
+    assert e.value.code == ul.UL_EINVAL
+    links[2, 1, 0, 3, 2] = np.nan
+    with pytest.raises(ul.UlError):
+        g.set_links(links)
+
+
+def test_error_codes(ul):
+    g = ul.Lattice(4, 4, 1.0, 1)
+    for call in (lambda: g.multilevel(3, 0, 1), lambda: g.multilevel(2, 0, 3), lambda: g.multilevel(2, -1, 1),
+                 lambda: g.multilevel2(2, 1, 3, 1, 1), lambda: g.substep(0, 0, 4), lambda: g.substep(2, 0, 0)):
+        with pytest.raises(ul.UlError) as e:
+            call()
+        assert e.value.code == ul.UL_EINVAL
+    with pytest.raises(ul.UlError) as e:
+        g.read_correlators()
+    assert e.value.code == ul.UL_ESTATE
+    with pytest.raises(ul.UlError) as e:
+        g.accumulate()
+    assert e.value.code == ul.UL_ESTATE
+    small = ul.Lattice(4, 4, 1.0, 1, workspace_bytes=4096)
+    with pytest.raises(ul.UlError) as e:
+        small.multilevel(2, 0, 2)
+    assert e.value.code == ul.UL_ENOMEM
+
+
+# ----------------------------------------------------------------------------- P1 link level
+@pytest.mark.parametrize("Ns,Nt,therm", [(4, 4, 0), (6, 4, 0), (8, 6, 0), (16, 4, 0), (16, 4, 30)])
+def test_p1_per_substep(ul, ulo, Ns, Nt, therm):
+    """P1(i): every sub-step of a HB and an OR sweep, full and slab-masked, from the oracle's configuration."""
+    beta, seed = 0.99, 2
+    o = ulo.Oracle(Ns, Nt, beta, seed)
+    ob = ulo.Oracle(Ns, Nt, beta, seed)
+    g = ul.Lattice(Ns, Nt, beta, seed)
+    if therm:
+        o.sweep(0, 0)
+        for _ in range(therm):
+            o.sweep(1, 4)
+    tot_flip = tot_ill = 0
+    n_upd = 0
+    for kind in (0, 1):
+        for d in (0, 2):
+            for parity in (0, 1):
+                for mu in range(4):
+                    before = o.get_links()
+                    ob.set_links(before)
+                    g.set_links(before)
+                    g.set_counter(o.get_counter())
+                    o.substep(kind, parity, mu, d)
+                    g.substep(kind, parity, mu, d)
+                    f, i, _ = check_links(g.get_links(), o.get_links(), before, ob, (kind, d, parity, mu), allow_frac=1e-4)
+                    tot_flip += f
+                    tot_ill += i
+                    n_upd += 1
+            if kind == 0:
+                o.set_counter(o.get_counter() + 1)
+    V4 = 4 * Ns ** 3 * Nt
+    assert tot_flip <= max(2, 1e-5 * V4 * n_upd / 8), (tot_flip, tot_ill)
+
+
+@pytest.mark.parametrize("Ns,Nt,beta,seed,n_therm,n_hb,n_or", [(4, 4, 0.95, 1, 20, 1, 3), (16, 4, 0.99, 2, 60, 1, 4)])
+def test_p1_whole_sweep_thermalised(ul, ulo, Ns, Nt, beta, seed, n_therm, n_hb, n_or):
+    """P1(ii): BJ's criterion literally, one heatbath sweep from a thermalised configuration."""
+    o = ulo.Oracle(Ns, Nt, beta, seed)
+    for _ in range(n_therm):
+        o.sweep(n_hb, n_or)
+    before = o.get_links()
+    ob = ulo.Oracle(Ns, Nt, beta, seed)
+    ob.set_links(before)
+    g = ul.Lattice(Ns, Nt, beta, seed)
+    g.set_links(before)
+    g.set_counter(o.get_counter())
+    o.sweep(1, 0)
+    g.sweep(1, 0)
+    assert g.get_counter() == o.get_counter()
+    diff = wrapdiff(g.get_links(), o.get_links())
+    frac = (diff > TOL).mean()
+    assert frac < (1e-5 if diff.size > 2e5 else 2.0 / diff.size), (frac, diff.max())
+
+
+def test_p1_masked_links_are_frozen_bit_for_bit(ul):
+    Ns, Nt = 8, 8
+    g = ul.Lattice(Ns, Nt, 1.0, 5)
+    g.sweep(2, 2)
+    before = g.get_links()
+    g.multilevel(4, 3, 2)
+    after = g.get_links()
+    for t in (0, 4):
+        assert np.array_equal(after[1:, t], before[1:, t])
+    assert not np.array_equal(after[0, 0], before[0, 0])          # temporal links on the boundary layer do move
+    assert not np.array_equal(after[1:, 1], before[1:, 1])
+
+
+def test_runs_are_bitwise_reproducible(ul):
+    res = []
+    for _ in range(2):
+        g = ul.Lattice(8, 4, 1.0, 9)
+        g.sweep(3, 2)
+        g.multilevel(2, 4, 3, [(0, 0, 0), (0, 1, 0)])
+        res.append((g.get_links(), g.read_correlators(), g.plaquette()))
+    assert np.array_equal(res[0][0], res[1][0])
+    assert all(np.array_equal(a, b) for a, b in zip(res[0][1], res[1][1]))
+    assert np.array_equal(res[0][2], res[1][2])
+
+
+def test_counter_resume_is_exact(ul):
+    a = ul.Lattice(8, 4, 1.0, 11)
+    a.sweep(2, 1)
+    links, ctr = a.get_links(), a.get_counter()
+    a.sweep(1, 1)
+    b = ul.Lattice(8, 4, 1.0, 11)
+    b.set_links(links)
+    b.set_counter(ctr)
+    b.sweep(1, 1)
+    assert np.array_equal(a.get_links(), b.get_links())
+
+
+# ----------------------------------------------------------------------------- P2 frozen configuration
+def rel_ok(got, want, n_terms, rms_term=1.0, tol=1e-5):
+    got, want = np.asarray(got), np.asarray(want)
+    bound = tol * np.maximum(np.abs(want), rms_term / np.sqrt(n_terms))
+    return np.all(np.abs(got - want) <= bound), float(np.max(np.abs(got - want) / bound))
+
+
+FPS = [(0, 0, 0), (0, 1, 0), (1, 0, 0), (0, 0, 1), (-1, 2, 1), (0, 3, 0)]
+
+
+@pytest.mark.parametrize("Ns,Nt,d", [(4, 4, 2), (8, 4, 2), (8, 8, 4), (6, 4, 1), (8, 4, 4)])
+def test_p2_frozen_configuration(ul, ulo, Ns, Nt, d):
+    beta = 1.0
+    o = ulo.Oracle(Ns, Nt, beta, 3)
+    for _ in range(10):
+        o.sweep(1, 3)
+    links = o.get_links()
+    g = ul.Lattice(Ns, Nt, beta, 3)
+    g.set_links(links)
+    ok, worst = rel_ok(g.plaquette(), o.plaquette(), 3 * Ns ** 3 * Nt)
+    assert ok, worst
+    R = Ns // 2
+    o.multilevel(d, 0, R, FPS)
+    g.multilevel(d, 0, R, FPS)
+    co, fo, vo = o.read_correlators()
+    cg, fg, vg = g.read_correlators()
+    Vs = Ns ** 3
+    assert np.abs(g.read_slab_averages() - o.read_slab_averages()).max() < 1e-5     # |T| = 1
+    ok, worst = rel_ok(cg, co, 3 * Vs)
+    assert ok, worst
+    ok, worst = rel_ok(fg, fo, 3 * Vs * Nt)
+    assert ok, worst
+    ok, worst = rel_ok(vg, vo, 3 * Vs * Nt)
+    assert ok, worst
+
+
+def test_p2_sequence_of_oracle_configurations(ul, ulo):
+    """Slab sums over several oracle sub-update configurations fed one by one (P2)."""
+    Ns, Nt, d, R = 8, 4, 2, 4
+    o = ulo.Oracle(Ns, Nt, 0.99, 4)
+    for _ in range(10):
+        o.sweep(1, 3)
+    g = ul.Lattice(Ns, Nt, 0.99, 4)
+    o.measure_begin(d, R, FPS)
+    g.measure_begin(d, R, FPS)
+    for _ in range(5):
+        for mu in range(4):
+            for par in range(2):
+                o.substep(1, par, mu, d)
+        o.substep(0, 0, 0, d)
+        g.set_links(o.get_links())
+        o.accumulate()
+        g.accumulate()
+    o.measure_end()
+    g.measure_end()
+    co, fo, vo = o.read_correlators()
+    cg, fg, vg = g.read_correlators()
+    assert np.abs(g.read_slab_averages() - o.read_slab_averages()).max() < 1e-5
+    Vs = Ns ** 3
+    for got, want, n in ((cg, co, 3 * Vs), (fg, fo, 3 * Vs * Nt), (vg, vo, 3 * Vs * Nt)):
+        ok, worst = rel_ok(got, want, n)
+        assert ok, worst
+
+
+def test_p2_two_level_one_iteration_matches_oracle_combine(ul, ulo):
+    """Two-level combine (Eqs. 32-33) on the same configurations: with n_in = n_out = 1 and a sub-update
+    recipe of zero sweeps both sides measure the SAME frozen configuration through the two-level code path."""
+    Ns, Nt, R = 8, 8, 3
+    o = ulo.Oracle(Ns, Nt, 1.0, 6)
+    for _ in range(8):
+        o.sweep(1, 3)
+    g = ul.Lattice(Ns, Nt, 1.0, 6)
+    g.set_links(o.get_links())
+    o.set_subupdate(0, 0, 1)
+    g.set_subupdate(0, 0, 1)
+    o.multilevel2(2, 1, 4, 1, R, FPS)
+    g.multilevel2(2, 1, 4, 1, R, FPS)
+    co, fo, vo = o.read_correlators()
+    cg, fg, vg = g.read_correlators()
+    Vs = Ns ** 3
+    assert np.abs(g.read_slab_averages() - o.read_slab_averages()).max() < 1e-5
+    for got, want, n in ((cg, co, 3 * Vs), (fg, fo, 3 * Vs * Nt), (vg, vo, 3 * Vs * Nt)):
+        ok, worst = rel_ok(got, want, n)
+        assert ok, worst
+    # and it equals the single-level result on the same configuration (factorisation, Eq. 24)
+    g.multilevel(2, 0, R, FPS)
+    c1, f1, _ = g.read_correlators()
+    assert np.allclose(c1, cg, atol=1e-12) and np.allclose(f1, fg, atol=1e-12)
+
+
+def test_p2_closed_forms_on_device(ul):
+    """Pins that need no oracle: cold start, constant flux, Polyakov winding (SURVEY 8(c) pins)."""
+    Ns, Nt = 8, 4
+    g = ul.Lattice(Ns, Nt, 1.0, 1)
+    g.init(0)
+    assert np.allclose(g.plaquette(), 1.0, atol=1e-7)
+    g.multilevel(2, 0, 4, FPS)
+    c, f, v = g.read_correlators()
+    assert np.allclose(c, 1.0, atol=1e-7) and np.allclose(f, 0, atol=1e-7) and np.allclose(v, 0, atol=1e-7)
+    links, phi = inputs.constant_flux_links(Ns, Nt, m=1)
+    g.set_links(links)
+    p = g.plaquette()
+    assert abs(p[0] - (5 + np.cos(phi)) / 6) < 1e-6 and abs(p[1] - 1) < 1e-6 and abs(p[2] - (2 + np.cos(phi)) / 3) < 1e-6
+    m = 1
+    links = np.zeros((4, Nt, Ns, Ns, Ns), dtype=np.float64)
+    links[0] = (2 * np.pi * m * np.arange(Ns) / Ns / Nt).reshape(1, 1, 1, Ns)
+    links = (links - 2 * np.pi * np.round(links / (2 * np.pi))).astype(np.float32)
+    g.set_links(links)
+    g.multilevel(2, 0, 4)
+    c, _, _ = g.read_correlators()
+    # C(r) = (e^{2 pi i m r / Ns} + 2)/3 : the winding shows only along mu = 1
+    want = (np.exp(2j * np.pi * m * np.arange(1, 5) / Ns) + 2) / 3
+    assert np.allclose(c, want, atol=2e-6)
+
+
+def test_gauge_invariance_on_device(ul):
+    """BJ check (b) on the GPU path: plaquette, C(r), G invariant under a random gauge transformation."""
+    Ns, Nt = 8, 4
+    g = ul.Lattice(Ns, Nt, 1.0, 21)
+    g.sweep(5, 5)
+    links = g.get_links()
+    g.multilevel(2, 0, 4, FPS)
+    c0, f0, v0 = g.read_correlators()
+    p0 = g.plaquette()
+    g.set_links(inputs.gauge_transform(links, inputs.gauge_function(Ns, Nt, 5)))
+    g.multilevel(2, 0, 4, FPS)
+    c1, f1, v1 = g.read_correlators()
+    assert np.allclose(g.plaquette(), p0, atol=2e-7)
+    assert np.allclose(c1, c0, atol=3e-7) and np.allclose(f1, f0, atol=3e-7) and np.allclose(v1, v0, atol=3e-7)
+
+
+# ----------------------------------------------------------------------------- P3 ensemble
+def binned_err(x, nbin=10):
+    x = np.asarray(x, dtype=np.float64)
+    n = len(x) // nbin * nbin
+    b = x[:n].reshape(nbin, -1).mean(axis=1)
+    return b.mean(), b.std(ddof=1) / np.sqrt(nbin)
+
+
+def test_p3_ensemble_config1(ul, ulo):
+    """BJ config 1 (4^3x4, beta=0.95, 1 HB + 3 OR): plaquette and multilevel C(r) of independent
+    GPU and oracle chains agree within 3 combined standard errors."""
+    Ns, Nt, beta = 4, 4, 0.95
+    n_meas = 120
+    g = ul.Lattice(Ns, Nt, beta, 1)
+    o = ulo.Oracle(Ns, Nt, beta, 101)
+    series = {}
+    for name, L in (("gpu", g), ("cpu", o)):
+        for _ in range(20):
+            L.sweep(1, 3)
+        P, C1, C2 = [], [], []
+        for _ in range(n_meas):
+            L.sweep(1, 3)
+            P.append(L.plaquette()[0])
+            L.multilevel(2, 10, 2, [(0, 0, 0)])
+            c, f, v = L.read_correlators()
+            C1.append(c[0].real)
+            C2.append(c[1].real)
+        series[name] = (P, C1, C2)
+    for k, label in enumerate(("plaquette", "C(1)", "C(2)")):
+        mg, eg = binned_err(series["gpu"][k])
+        mc, ec = binned_err(series["cpu"][k])
+        assert abs(mg - mc) <= 3.0 * np.hypot(eg, ec) + 1e-12, (label, mg, eg, mc, ec)
+
+
+def test_p3_strong_and_weak_coupling_on_device(ul):
+    """BJ checks (c), (d) on the GPU path: <cos theta_P> = I1/I0 at beta = 0.1; <1 - cos> ~ 1/(4 beta) at beta = 5."""
+    from scipy import special
+    g = ul.Lattice(8, 8, 0.1, 31)
+    for _ in range(20):
+        g.sweep(1, 1)
+    vals = []
+    for _ in range(200):
+        g.sweep(1, 1)
+        vals.append(g.plaquette()[0])
+    m, e = binned_err(vals)
+    want = special.iv(1, 0.1) / special.iv(0, 0.1)
+    assert abs(m - want) < 4 * e + 2e-5, (m, e, want)
+    g = ul.Lattice(8, 8, 5.0, 32)
+    g.init(0)
+    for _ in range(100):
+        g.sweep(1, 3)
+    vals = []
+    for _ in range(100):
+        g.sweep(1, 3)
+        vals.append(1 - g.plaquette()[0])
+    m, e = binned_err(vals)
+    assert abs(m - 0.05) < 0.05 * 0.05, (m, e)
+
+
+def test_multilevel_matches_naive_on_device(ul):
+    """BJ check (e) on the GPU path: multilevel C(r) vs the naive estimator (n_sub = 0) at strong coupling."""
+    Ns, Nt, beta = 4, 4, 0.6
+    g = ul.Lattice(Ns, Nt, beta, 41)
+    for _ in range(30):
+        g.sweep(1, 3)
+    naive, ml = [], []
+    for _ in range(300):
+        g.sweep(1, 3)
+        g.multilevel(2, 0, 1)
+        naive.append(g.read_correlators()[0][0].real)
+        g.multilevel(2, 8, 1)
+        ml.append(g.read_correlators()[0][0].real)
+    mn, en = binned_err(naive)
+    mm, em = binned_err(ml)
+    assert abs(mn - mm) < 3.5 * np.hypot(en, em), (mn, en, mm, em)
+    assert em < en                                               # the multilevel estimator is less noisy
+
+
+# ----------------------------------------------------------------------------- full size (BJ config 5)
+def test_full_size_64_sampled_against_oracle(ul, ulo):
+    """64^4 (the bench workload, same launch configuration): hot start bit-exact, then one HB and one
+    OR sub-step compared with the oracle on every updated link; plaquette to relative 1e-5."""
+    Ns = Nt = 64
+    seed, beta = 5, 0.98
+    g = ul.Lattice(Ns, Nt, beta, seed)
+    o = ulo.Oracle(Ns, Nt, beta, seed)
+    links = o.get_links()
+    assert np.array_equal(g.get_links(), links)
+    ok, worst = rel_ok(g.plaquette(), o.plaquette(), 3 * Ns ** 4, rms_term=0.7)
+    assert ok, worst
+    for kind, parity, mu, d in ((1, 0, 1, 0), (0, 1, 0, 0), (0, 0, 3, 2)):
+        before = o.get_links()
+        g.set_links(before)
+        g.set_counter(o.get_counter())
+        o.substep(kind, parity, mu, d)
+        g.substep(kind, parity, mu, d)
+        diff = wrapdiff(g.get_links(), o.get_links())
+        frac = (diff > TOL).sum() / (diff.size / 8)
+        # hot start: links with tiny staples (k < 0.05, P ~ 3e-4) amplify rounding; flips are rare
+        assert frac < 1e-4, (kind, parity, mu, d, frac, diff.max())
+        assert (diff > 1e-3).sum() / (diff.size / 8) < 1e-5
