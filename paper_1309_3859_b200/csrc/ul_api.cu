@@ -135,7 +135,7 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
     if (slab_d > 0 && mu != 0) n_t = c->Nt / slab_d * (slab_d - 1);
     if (n_t == 0) return UL_OK;                       // thickness 1: every spatial link is frozen
     ulk::UpdateArgs a;
-    a.th = c->th; a.Vh = c->Vh; a.Ns = c->Ns; a.Nh = c->Nh; a.Nt = c->Nt;
+    a.th = c->th; a.Vh = (int)c->Vh; a.Ns = c->Ns; a.Nh = c->Nh; a.Nt = c->Nt;
     a.parity = parity; a.slab_d = slab_d; a.beta = (float)c->beta;
     a.key0 = (uint32_t)(c->seed & 0xffffffffu); a.key1 = (uint32_t)(c->seed >> 32);
     a.sweep_lo = (uint32_t)(c->sweep & 0xffffffffu); a.sweep_hi = (uint32_t)(c->sweep >> 32);
@@ -253,7 +253,7 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     if (Ns < 2 || Nt < 2 || (Ns & 1) || (Nt & 1) || !(beta >= 0.0)) return fail(nullptr, UL_EINVAL, "need even Ns, Nt >= 2 and beta >= 0");
     const int Nh = Ns / 2;
     const int vec = (Nh % 4 == 0) ? 4 : ((Nh % 2 == 0) ? 2 : 1);
-    if (Nh / vec > 256 || (double)Ns * Ns * Ns * Nt > 4.0e9) return fail(nullptr, UL_EINVAL, "lattice too large for this build");
+    if (Nh / vec > 256 || 4.0 * (double)Ns * Ns * Ns * Nt >= 2147483648.0) return fail(nullptr, UL_EINVAL, "lattice too large for this build");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(nullptr, UL_ECUDA, "no CUDA device");
     ul_ctx* c = new (std::nothrow) ul_ctx;

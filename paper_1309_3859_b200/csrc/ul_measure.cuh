@@ -54,9 +54,9 @@ __global__ void __launch_bounds__(256) k_repack(Geom g, float* __restrict__ inte
     if (pack) {
         const float v = canonical[i];
         if (!(fabsf(v) <= 3.2f)) *bad = 1;
-        internal[j] = v;
+        internal[j] = ulm::to_units(v);               // exact power-of-two scaling
     } else {
-        canonical[i] = internal[j];
+        canonical[i] = ulm::to_rad(internal[j]);
     }
 }
 
@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(256) k_hot_start(Geom g, float* __restrict__ i
     uint32_t w[4];
     ulm::philox4x32_10(site, 0u, 0u, (1u << 3) | (uint32_t)mu, key0, key1, w);
     const double th = 6.28318530717958647692 * (double)w[0] * (1.0 / 4294967296.0) - 3.14159265358979323846;
-    internal[link_index(g, mu, t, x3, x2, x1)] = (float)th;
+    internal[link_index(g, mu, t, x3, x2, x1)] = ulm::to_units((float)th);
 }
 
 __global__ void k_philox_test(const uint32_t* __restrict__ ctr, const uint32_t* __restrict__ key, uint32_t* __restrict__ out, int n) {
