@@ -9,8 +9,11 @@
  * Conventions (S8): directions mu = 0 (time), 1,2,3 = x,y,z.  Site index
  * i = x1 + Ns*(x2 + Ns*(x3 + Ns*t)); parity (x1+x2+x3+t) mod 2.  "Canonical" link arrays
  * at this boundary are HOST pointers to float[4][Nt][Ns][Ns][Ns] (mu slowest, x1 fastest),
- * fp32 radians in [-pi, pi].  Inside the library the links live in HBM as fp32 angles in a
- * parity-split, direction-split structure of arrays.
+ * fp32 radians in [-pi, pi].  Inside the library the links live in HBM as 32-bit binary angles
+ * (int32 I, theta = I * 2 pi / 2^32: angle sums are exact wrapping adds) in a parity-split,
+ * direction-split structure of arrays.  fp32 radians -> binary angle ->
+ * fp32 radians returns the same fp32 for |theta| >= 2^-6 rad and differs by <= 1.2e-9 rad
+ * below that.
  *
  * Ownership: the library owns the handle.  Every host pointer passed in is caller-owned and
  * only read or written during the call.  With ul_create_ext the caller also owns the device
@@ -65,10 +68,14 @@ int ul_init(ul_ctx* h, int mode);
 int ul_set_beta(ul_ctx* h, double beta);
 
 /* Canonical HOST array in / out (see top).  ul_set_links returns UL_EINVAL if any angle is
- * NaN or has |theta| > 3.2 (angles must already be wrapped; the fixed-point staple sums of
- * DESIGN.md "Arithmetic" assume |theta| <= pi up to rounding). */
+ * NaN or has |theta| > 3.2 (angles must already be wrapped to [-pi, pi] up to rounding). */
 int ul_set_links(ul_ctx* h, const float* host_links);
 int ul_get_links(ul_ctx* h, float* host_links);
+
+/* The same arrays as raw binary angles, HOST int32[4][Nt][Ns][Ns][Ns], bit for bit: the exact
+ * state for checkpoint / resume (with ul_get_counter / ul_set_counter and the seed). */
+int ul_set_links_raw(ul_ctx* h, const int32_t* host_links);
+int ul_get_links_raw(ul_ctx* h, int32_t* host_links);
 
 /* 64-bit count of heatbath sweeps issued so far = the Philox counter words 1,2 (S8(c)-O4).
  * State = links + counter + seed: restoring both resumes a run bit for bit. */

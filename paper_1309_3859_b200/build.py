@@ -26,7 +26,7 @@ def build(force=False, verbose=False):
     deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]
     if not force and os.path.exists(SO) and all(os.path.getmtime(SO) >= os.path.getmtime(d) for d in deps):
         return SO
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+    cmd = [_nvcc()] + NVCC_FLAGS + os.environ.get("UL_NVCC_EXTRA", "").split() + (["-Xptxas", "-v"] if verbose else []) + \
           ["-o", SO + ".tmp"] + [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.run(cmd, check=True, cwd=CSRC)
     os.replace(SO + ".tmp", SO)

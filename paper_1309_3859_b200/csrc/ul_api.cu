@@ -57,7 +57,7 @@ struct ul_ctx {
     uint64_t seed = 0, sweep = 0, launches = 0;
     cudaStream_t stream = nullptr;
     bool own_stream = false;
-    float* th = nullptr;
+    int* th = nullptr;         // internal layout, binary angles
     bool own_th = false;
     char* work = nullptr;      // measurement workspace in use
     size_t work_bytes = 0;
@@ -267,7 +267,7 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     const size_t need = sizeof(float) * 4 * (size_t)c->V;
     if (ext) {
         if (!dev_links || links_bytes < need || ((uintptr_t)dev_links & 255)) { delete c; return fail(nullptr, UL_EINVAL, "dev_links too small or misaligned"); }
-        c->th = (float*)dev_links;
+        c->th = (int*)dev_links;
         c->stream = (cudaStream_t)stream;
         if (dev_work && work_bytes) { c->work = (char*)dev_work; c->work_bytes = work_bytes; c->own_work = false; }
         else c->own_work = true;
@@ -275,7 +275,7 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
         void* p = nullptr;
         cudaError_t e = cudaMalloc(&p, need);
         if (e != cudaSuccess) { delete c; return fail(nullptr, UL_ENOMEM, std::string("cudaMalloc links: ") + cudaGetErrorString(e)); }
-        c->th = (float*)p; c->own_th = true;
+        c->th = (int*)p; c->own_th = true;
         e = cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking);
         if (e != cudaSuccess) { cudaFree(p); delete c; return fail(nullptr, UL_ECUDA, std::string("cudaStreamCreate: ") + cudaGetErrorString(e)); }
         c->own_stream = true; c->own_work = true;
@@ -345,14 +345,14 @@ static int ensure_staging(ul_ctx* c) {
     c->staging = (float*)p;
     return UL_OK;
 }
-int ul_set_links(ul_ctx* c, const float* host) {
+static int links_in(ul_ctx* c, const void* host, int mode) {
     if (!c || !host) return fail(c, UL_EINVAL, "null pointer");
     int rc = ensure_staging(c);
     if (rc) return rc;
     const long long n = 4 * c->V;
     UL_CUDA(c, cudaMemsetAsync(c->d_bad, 0, sizeof(int), c->stream));
     UL_CUDA(c, cudaMemcpyAsync(c->staging, host, sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
-    ulk::k_repack<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(geom(c), c->th, c->staging, 1, c->d_bad);
+    ulk::k_repack<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(geom(c), c->th, c->staging, mode, c->d_bad);
     UL_CUDA(c, cudaGetLastError());
     c->launches += 1;
     int bad = 0;
@@ -361,18 +361,22 @@ int ul_set_links(ul_ctx* c, const float* host) {
     if (bad) return fail(c, UL_EINVAL, "link angles must be finite with |theta| <= 3.2 (wrap them to [-pi, pi] first)");
     return UL_OK;
 }
-int ul_get_links(ul_ctx* c, float* host) {
+static int links_out(ul_ctx* c, void* host, int mode) {
     if (!c || !host) return fail(c, UL_EINVAL, "null pointer");
     int rc = ensure_staging(c);
     if (rc) return rc;
     const long long n = 4 * c->V;
-    ulk::k_repack<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(geom(c), c->th, c->staging, 0, c->d_bad);
+    ulk::k_repack<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(geom(c), c->th, c->staging, mode, c->d_bad);
     UL_CUDA(c, cudaGetLastError());
     c->launches += 1;
     UL_CUDA(c, cudaMemcpyAsync(host, c->staging, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, c->stream));
     UL_CUDA(c, cudaStreamSynchronize(c->stream));
     return UL_OK;
 }
+int ul_set_links(ul_ctx* c, const float* host) { return links_in(c, host, 1); }
+int ul_get_links(ul_ctx* c, float* host) { return links_out(c, host, 0); }
+int ul_set_links_raw(ul_ctx* c, const int32_t* host) { return links_in(c, host, 3); }
+int ul_get_links_raw(ul_ctx* c, int32_t* host) { return links_out(c, host, 2); }
 int ul_get_counter(ul_ctx* c, uint64_t* v) { if (!c || !v) return fail(c, UL_EINVAL, "null pointer"); *v = c->sweep; return UL_OK; }
 int ul_set_counter(ul_ctx* c, uint64_t v) { if (!c) return fail(c, UL_EINVAL, "null handle"); c->sweep = v; return UL_OK; }
 

@@ -38,9 +38,10 @@ __device__ __forceinline__ int modc(int v, int L) {           // any v
 }
 
 // ---------------------------------------------------------------- layout (row a1)
-// canonical [mu][t][x3][x2][x1] <-> internal; dir = 1 pack (canonical -> internal), 0 unpack.
-// On pack, *bad is set if an angle is NaN or |theta| > 3.2.
-__global__ void __launch_bounds__(256) k_repack(Geom g, float* __restrict__ internal, float* __restrict__ canonical,
+// canonical [mu][t][x3][x2][x1] <-> internal; pack = 1 (fp32 radians -> internal), 0 (internal -> fp32
+// radians), 3 / 2 the same with raw int32 binary angles (bit copy).  On pack = 1, *bad is set if an angle
+// is NaN or |theta| > 3.2.
+__global__ void __launch_bounds__(256) k_repack(Geom g, int* __restrict__ internal, float* __restrict__ canonical,
                                                 int pack, int* __restrict__ bad) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;   // over 4V canonical elements
     if (i >= 4 * g.V) return;
@@ -51,17 +52,21 @@ __global__ void __launch_bounds__(256) k_repack(Geom g, float* __restrict__ inte
     const int x3 = (int)(s % g.Ns); s /= g.Ns;
     const int t = (int)s;
     const long long j = link_index(g, mu, t, x3, x2, x1);
-    if (pack) {
+    if (pack == 1) {
         const float v = canonical[i];
         if (!(fabsf(v) <= 3.2f)) *bad = 1;
-        internal[j] = ulm::to_units(v);               // exact power-of-two scaling
+        internal[j] = ulm::rad_to_bt(v);              // nearest binary angle (fp64 scaling)
+    } else if (pack == 0) {
+        canonical[i] = ulm::bt_to_rad(internal[j]);
+    } else if (pack == 3) {                           // raw binary angles in canonical order (exact checkpoint)
+        internal[j] = __float_as_int(canonical[i]);
     } else {
-        canonical[i] = ulm::to_rad(internal[j]);
+        canonical[i] = __int_as_float(internal[j]);
     }
 }
 
 // hot start (S8(c)-O4): theta = fp32(2 pi w0 2^-32 - pi), ctr = (site, 0, 0, (1<<3)|mu)
-__global__ void __launch_bounds__(256) k_hot_start(Geom g, float* __restrict__ internal, uint32_t key0, uint32_t key1) {
+__global__ void __launch_bounds__(256) k_hot_start(Geom g, int* __restrict__ internal, uint32_t key0, uint32_t key1) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= 4 * g.V) return;
     const int mu = (int)(i / g.V);
@@ -74,7 +79,7 @@ __global__ void __launch_bounds__(256) k_hot_start(Geom g, float* __restrict__ i
     uint32_t w[4];
     ulm::philox4x32_10(site, 0u, 0u, (1u << 3) | (uint32_t)mu, key0, key1, w);
     const double th = 6.28318530717958647692 * (double)w[0] * (1.0 / 4294967296.0) - 3.14159265358979323846;
-    internal[link_index(g, mu, t, x3, x2, x1)] = ulm::to_units((float)th);
+    internal[link_index(g, mu, t, x3, x2, x1)] = ulm::rad_to_bt((float)th);
 }
 
 __global__ void k_philox_test(const uint32_t* __restrict__ ctr, const uint32_t* __restrict__ key, uint32_t* __restrict__ out, int n) {
@@ -122,20 +127,20 @@ __global__ void __launch_bounds__(256) k_sum_partials(const double* __restrict__
 }
 
 // ---------------------------------------------------------------- plaquette angles
-// theta_P(a,b)(y) = theta_a(y) + theta_b(y+a) - theta_a(y+b) - theta_b(y), fixed point
-__device__ __forceinline__ int plaq_fx(const Geom& g, const float* __restrict__ th, int a, int b, const int x[4]) {
+// theta_P(a,b)(y) = theta_a(y) + theta_b(y+a) - theta_a(y+b) - theta_b(y), binary angle (exact mod 2 pi)
+__device__ __forceinline__ int plaq_fx(const Geom& g, const int* __restrict__ th, int a, int b, const int x[4]) {
     int xa[4] = {x[0], x[1], x[2], x[3]}, xb[4] = {x[0], x[1], x[2], x[3]};
     xa[a] = (x[a] + 1 == (a == 0 ? g.Nt : g.Ns)) ? 0 : x[a] + 1;
     xb[b] = (x[b] + 1 == (b == 0 ? g.Nt : g.Ns)) ? 0 : x[b] + 1;
-    const int t0 = ulm::to_fx(__ldg(th + link_index(g, a, x[0], x[3], x[2], x[1])));
-    const int t1 = ulm::to_fx(__ldg(th + link_index(g, b, xa[0], xa[3], xa[2], xa[1])));
-    const int t2 = ulm::to_fx(__ldg(th + link_index(g, a, xb[0], xb[3], xb[2], xb[1])));
-    const int t3 = ulm::to_fx(__ldg(th + link_index(g, b, x[0], x[3], x[2], x[1])));
-    return t0 + t1 - t2 - t3;                          // |.| <= 4 pi 2^27 < 2^31
+    const unsigned t0 = (unsigned)__ldg(th + link_index(g, a, x[0], x[3], x[2], x[1]));
+    const unsigned t1 = (unsigned)__ldg(th + link_index(g, b, xa[0], xa[3], xa[2], xa[1]));
+    const unsigned t2 = (unsigned)__ldg(th + link_index(g, a, xb[0], xb[3], xb[2], xb[1]));
+    const unsigned t3 = (unsigned)__ldg(th + link_index(g, b, x[0], x[3], x[2], x[1]));
+    return (int)(t0 + t1 - t2 - t3);
 }
 
 // row a11: partial[0*nblk + b] = sum of cos over time-like plaquettes, [1*nblk + b] space-like
-__global__ void __launch_bounds__(256) k_plaquette(Geom g, const float* __restrict__ th, double* __restrict__ partial) {
+__global__ void __launch_bounds__(256) k_plaquette(Geom g, const int* __restrict__ th, double* __restrict__ partial) {
     __shared__ double sm[2 * 32];
     double v[2] = {0.0, 0.0};
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.V; i += (long long)gridDim.x * blockDim.x) {
@@ -150,7 +155,7 @@ __global__ void __launch_bounds__(256) k_plaquette(Geom g, const float* __restri
 #pragma unroll
             for (int b = a + 1; b < 4; ++b) {
                 float c, sn;
-                ulm::sincos_fx<true>(plaq_fx(g, th, a, b, x), c, sn);
+                ulm::sincos_bt(plaq_fx(g, th, a, b, x), c, sn);
                 if (a == 0) v[0] += (double)c; else v[1] += (double)c;
             }
     }
@@ -159,9 +164,9 @@ __global__ void __launch_bounds__(256) k_plaquette(Geom g, const float* __restri
 }
 
 // ---------------------------------------------------------------- per-configuration slab tables
-// Th[s][xs] = sum_{t in slab s} theta_0(xs,t), fixed point, reduced to [-pi, pi]
+// Th[s][xs] = sum_{t in slab s} theta_0(xs,t), binary angle (wrapping sum = exact mod 2 pi)
 // Ot[o][kind][s][xs] = sum_{t in slab s} O(theta_P(o)(xs,t)),  O = 1 - cos (kind 0), sin (kind 1)
-__global__ void __launch_bounds__(256) k_slab_tables(Geom g, const float* __restrict__ th, int d, int n_slab,
+__global__ void __launch_bounds__(256) k_slab_tables(Geom g, const int* __restrict__ th, int d, int n_slab,
                                                      int* __restrict__ Th, float* __restrict__ Ot) {
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (long long)n_slab * g.Vs) return;
@@ -171,28 +176,26 @@ __global__ void __launch_bounds__(256) k_slab_tables(Geom g, const float* __rest
     x[1] = (int)(r % g.Ns); r /= g.Ns;
     x[2] = (int)(r % g.Ns); r /= g.Ns;
     x[3] = (int)r;
-    int acc = 0;
+    unsigned acc = 0u;
     float o_c[6], o_s[6];
 #pragma unroll
     for (int o = 0; o < 6; ++o) { o_c[o] = 0.0f; o_s[o] = 0.0f; }
     for (int t = s * d; t < (s + 1) * d; ++t) {
         x[0] = t;
-        acc += ulm::to_fx(__ldg(th + link_index(g, 0, t, x[3], x[2], x[1])));
-        acc -= (acc > ulm::FX_PI) ? ulm::FX_TWO_PI : 0;
-        acc += (acc < -ulm::FX_PI) ? ulm::FX_TWO_PI : 0;
+        acc += (unsigned)__ldg(th + link_index(g, 0, t, x[3], x[2], x[1]));
         int o = 0;
 #pragma unroll
         for (int a = 0; a < 4; ++a)
 #pragma unroll
             for (int b = a + 1; b < 4; ++b) {
                 float c, sn;
-                ulm::sincos_fx<true>(plaq_fx(g, th, a, b, x), c, sn);
+                ulm::sincos_bt(plaq_fx(g, th, a, b, x), c, sn);
                 o_c[o] += 1.0f - c;
                 o_s[o] += sn;
                 ++o;
             }
     }
-    Th[idx] = acc;
+    Th[idx] = (int)acc;
     const long long stride = (long long)n_slab * g.Vs;
 #pragma unroll
     for (int o = 0; o < 6; ++o) {
@@ -266,7 +269,7 @@ __global__ void __launch_bounds__(256) k_accumulate(const AccumArgs P) {
             const long long ys = y[1] + (long long)Ns * (y[2] + (long long)Ns * y[3]);
             // T^(d)(x,s,r mu) = exp(i sum_{t in slab} [theta_0(x + r mu, t) - theta_0(x, t)])  (Eq. 22, 25)
             float c, sn;
-            ulm::sincos_fx<true>(Ths[ys] - th0, c, sn);
+            ulm::sincos_bt((int)((unsigned)Ths[ys] - (unsigned)th0), c, sn);
             const double Tr = (double)c, Ti = (double)sn;
             const long long a_idx = (((long long)(mu - 1) * P.r_max + (r - 1)) * P.n_slab + s) * g.Vs + xs;
             double2 a = P.A[a_idx];

@@ -1,7 +1,7 @@
 // ul_update.cuh -- link-update kernels: staple gather + heatbath / overrelaxation sub-step,
 // full or slab-masked.
 //
-// Layout (row a1, BJ kernel 1): th[mu][par][row*Nh + h], fp32 angles in units of 2^-27 rad, where
+// Layout (row a1, BJ kernel 1): th[mu][par][row*Nh + h], int32 binary angles (ul_math.cuh), where
 //   row = (t*Ns + x3)*Ns + x2,  Nh = Ns/2,  par = (x1+x2+x3+t)&1,  x1 = 2h + ((par+x2+x3+t)&1).
 // One sub-step (parity p, direction MU) updates the array th[MU][p] in place and reads the
 // seven other arrays it depends on; it never reads an element another thread writes.
@@ -17,7 +17,7 @@
 namespace ulk {
 
 struct UpdateArgs {
-    float* th;            // internal layout, 8 arrays of Vh floats
+    int* th;              // internal layout, 8 arrays of Vh binary angles
     int Vh;               // V/2
     int Ns, Nh, Nt;
     int parity;           // sub-step parity p
@@ -35,44 +35,42 @@ struct Site {
     int off;              // x1 = 2h + off
 };
 
-// Loads, as fixed point, the VEC angles at element offset `idx` shifted by the x1-displacement D1
-// (-1, 0, +1): x1 + 1 lives at h + off, x1 - 1 at h - 1 + off of the other-parity row.
+// Loads the VEC angles at element offset `idx` shifted by the x1-displacement D1 (-1, 0, +1):
+// x1 + 1 lives at h + off, x1 - 1 at h - 1 + off of the other-parity row.
 template <int VEC, int D1>
-__device__ __forceinline__ void load_row(const float* __restrict__ th, int idx, const Site& st, int out[VEC]) {
-    float v[VEC];
+__device__ __forceinline__ void load_row(const int* __restrict__ th, int idx, const Site& st, int v[VEC]) {
     if (VEC == 4) {
-        const float4 q = __ldg(reinterpret_cast<const float4*>(th + idx));
+        const int4 q = __ldg(reinterpret_cast<const int4*>(th + idx));
         v[0] = q.x; v[1 % VEC] = q.y; v[2 % VEC] = q.z; v[3 % VEC] = q.w;
     } else if (VEC == 2) {
-        const float2 q = __ldg(reinterpret_cast<const float2*>(th + idx));
+        const int2 q = __ldg(reinterpret_cast<const int2*>(th + idx));
         v[0] = q.x; v[1 % VEC] = q.y;
     } else {
         v[0] = __ldg(th + idx);
     }
     if (D1 > 0) {
         if (st.off) {                                 // shift by +1: need element h0 + VEC
-            const float x = __ldg(th + idx + st.dxp);
+            const int x = __ldg(th + idx + st.dxp);
 #pragma unroll
             for (int i = 0; i < VEC - 1; ++i) v[i] = v[i + 1];
             v[VEC - 1] = x;
         }
     } else if (D1 < 0) {
         if (!st.off) {                                // shift by -1: need element h0 - 1
-            const float x = __ldg(th + idx + st.dxm);
+            const int x = __ldg(th + idx + st.dxm);
 #pragma unroll
             for (int i = VEC - 1; i > 0; --i) v[i] = v[i - 1];
             v[0] = x;
         }
     }
-#pragma unroll
-    for (int i = 0; i < VEC; ++i) out[i] = ulm::to_fx(v[i]);
 }
 
 // Adds the two staples of the (MU, NU) plane to S for the VEC links of one thread (row a2):
 //   S += e^{-i sigma+} + e^{-i sigma-},  -sigma+ = th_nu(x) + th_mu(x+nu) - th_nu(x+mu),
 //                                        -sigma- = th_nu(x+mu-nu) + th_mu(x-nu) - th_nu(x-nu).
+// The phase sums are wrapping int32 adds: exact and already reduced mod 2 pi.
 template <int MU, int NU, int VEC>
-__device__ __forceinline__ void staple_pair(const float* __restrict__ th, int Vh, int p, const Site& st,
+__device__ __forceinline__ void staple_pair(const int* __restrict__ th, int Vh, int p, const Site& st,
                                             float Sx[VEC], float Sy[VEC]) {
     constexpr int m1 = (MU == 1), n1 = (NU == 1);
     const int a_nu_p = (NU * 2 + p) * Vh, a_nu_q = (NU * 2 + 1 - p) * Vh, a_mu_q = (MU * 2 + 1 - p) * Vh;
@@ -85,9 +83,17 @@ __device__ __forceinline__ void staple_pair(const float* __restrict__ th, int Vh
     load_row<VEC, -n1>(th, a_nu_q + st.e0 + st.dm[NU], st, F);                     // theta_nu(x-nu)
 #pragma unroll
     for (int i = 0; i < VEC; ++i) {
-        ulm::cis_accumulate(A[i] + B[i] - C[i], Sx[i], Sy[i]);
-        ulm::cis_accumulate(D[i] + E[i] - F[i], Sx[i], Sy[i]);
+        ulm::cis_accumulate((int)((unsigned)A[i] + (unsigned)B[i] - (unsigned)C[i]), Sx[i], Sy[i]);
+        ulm::cis_accumulate((int)((unsigned)D[i] + (unsigned)E[i] - (unsigned)F[i]), Sx[i], Sy[i]);
     }
+}
+
+template <typename T, int VEC>
+__device__ __forceinline__ T pick(const T v[VEC], int j) {        // v[j] without dynamic register indexing
+    T r = v[0];
+#pragma unroll
+    for (int i = 1; i < VEC; ++i) r = (j == i) ? v[i] : r;
+    return r;
 }
 
 // KIND 0 = heatbath, 1 = overrelaxation.  Block (Nh/VEC, BY, BZ); grid (Ns/BY, Ns/BZ, n_t)
@@ -123,36 +129,58 @@ __global__ void __launch_bounds__(256) k_update(const UpdateArgs P) {
     staple_pair<MU, (MU + 2) & 3, VEC>(P.th, P.Vh, p, st, Sx, Sy);
     staple_pair<MU, (MU + 3) & 3, VEC>(P.th, P.Vh, p, st, Sx, Sy);
 
-    float* own = P.th + ((MU * 2 + p) * P.Vh + st.e0);
-    float out[VEC];
+    int* own = P.th + ((MU * 2 + p) * P.Vh + st.e0);
+    int out[VEC];
     if (KIND == 1) {
-        float old[VEC];
-        if (VEC == 4) { const float4 q = *reinterpret_cast<const float4*>(own); old[0] = q.x; old[1 % VEC] = q.y; old[2 % VEC] = q.z; old[3 % VEC] = q.w; }
-        else if (VEC == 2) { const float2 q = *reinterpret_cast<const float2*>(own); old[0] = q.x; old[1 % VEC] = q.y; }
+        int old[VEC];
+        if (VEC == 4) { const int4 q = *reinterpret_cast<const int4*>(own); old[0] = q.x; old[1 % VEC] = q.y; old[2 % VEC] = q.z; old[3 % VEC] = q.w; }
+        else if (VEC == 2) { const int2 q = *reinterpret_cast<const int2*>(own); old[0] = q.x; old[1 % VEC] = q.y; }
         else old[0] = own[0];
 #pragma unroll
-        for (int i = 0; i < VEC; ++i) {
-            const float alpha = ulm::atan2_acc(Sy[i], Sx[i]);
-            out[i] = ulm::to_units(ulm::wrap(fmaf(2.0f, alpha, -ulm::to_rad(old[i]))));   // overrelaxation (O2)
-        }
+        for (int i = 0; i < VEC; ++i)                 // overrelaxation (O2): theta' = 2 alpha - theta, exact mod 2 pi
+            out[i] = (int)(2u * (unsigned)ulm::atan2_bt(Sy[i], Sx[i]) - (unsigned)old[i]);
     } else {
+        // Heatbath (O3).  Attempt n of a link is a pure function of (site, sweep, n), so the order in
+        // which a thread works through its rejections is free: every link gets attempt 0 with the warp
+        // converged; a lane then retries its own rejected links one at a time (lane-local queue), which
+        // bounds the warp's extra rounds by the worst lane's total instead of the sum of per-link maxima.
         const uint32_t site0 = (uint32_t)((st.e0 - h0) * 2 + 2 * h0 + st.off);            // canonical site index
         const uint32_t c3 = ((uint32_t)p << 2) | (uint32_t)MU;                            // tag 0 = heatbath
+        float pa[VEC], pq[VEC], pc[VEC], sn[VEC], cs[VEC];
+        uint32_t pend = 0u, neg = 0u, tries = 0u;                                         // tries: 8 bits per link
 #pragma unroll
         for (int i = 0; i < VEC; ++i) {
-            const float k = sqrtf(fmaf(Sx[i], Sx[i], Sy[i] * Sy[i]));
-            const ulm::HbParams hp = ulm::hb_setup(P.beta * k);
-            float sn = 0.0f, cs = 1.0f;
+            const float k2 = fmaf(Sx[i], Sx[i], Sy[i] * Sy[i]);
+            if (k2 == 0.0f) Sx[i] = 1.0f;                                                 // k = 0: alpha = 0 (O1)
+            const ulm::HbParams hp = ulm::hb_setup(P.beta * ulm::mufu_sqrt(k2));
+            pa[i] = hp.a; pq[i] = hp.q; pc[i] = hp.c0;
             uint32_t w[4];
-            for (uint32_t n = 0; n < 64u; ++n) {                                          // cap 64 (O3)
-                ulm::philox4x32_10(site0 + 2u * i, P.sweep_lo, P.sweep_hi, (n << 8) | c3, P.key0, P.key1, w);
-                if (ulm::hb_attempt(hp, w[0], w[1], sn, cs)) break;
-            }
-            out[i] = ulm::to_units(ulm::hb_finish(Sx[i], Sy[i], sn, cs, (w[2] >> 31) != 0));   // heatbath (O3)
+            ulm::philox4x32_10(site0 + 2u * i, P.sweep_lo, P.sweep_hi, c3, P.key0, P.key1, w);
+            const bool ok = ulm::hb_attempt(hp, w[0], w[1], sn[i], cs[i]);
+            neg |= (w[2] >> 31) << i;
+            pend |= (ok ? 0u : 1u) << i;
+            tries |= 1u << (8 * i);
         }
+        while (pend) {
+            const int j = __ffs(pend) - 1;
+            ulm::HbParams hp;
+            hp.a = pick<float, VEC>(pa, j); hp.q = pick<float, VEC>(pq, j); hp.c0 = pick<float, VEC>(pc, j);
+            const uint32_t n = (tries >> (8 * j)) & 0xffu;
+            uint32_t w[4];
+            ulm::philox4x32_10(site0 + 2u * (uint32_t)j, P.sweep_lo, P.sweep_hi, (n << 8) | c3, P.key0, P.key1, w);
+            float s1, c1;
+            const bool ok = ulm::hb_attempt(hp, w[0], w[1], s1, c1);
+#pragma unroll
+            for (int i = 0; i < VEC; ++i) { sn[i] = (j == i) ? s1 : sn[i]; cs[i] = (j == i) ? c1 : cs[i]; }
+            neg = (neg & ~(1u << j)) | ((w[2] >> 31) << j);
+            tries += 1u << (8 * j);
+            if (ok || n == 63u) pend &= ~(1u << j);                                       // cap 64: keep the last proposal (O3)
+        }
+#pragma unroll
+        for (int i = 0; i < VEC; ++i) out[i] = ulm::hb_finish(Sx[i], Sy[i], sn[i], cs[i], ((neg >> i) & 1u) != 0);
     }
-    if (VEC == 4) *reinterpret_cast<float4*>(own) = make_float4(out[0], out[1 % VEC], out[2 % VEC], out[3 % VEC]);
-    else if (VEC == 2) *reinterpret_cast<float2*>(own) = make_float2(out[0], out[1 % VEC]);
+    if (VEC == 4) *reinterpret_cast<int4*>(own) = make_int4(out[0], out[1 % VEC], out[2 % VEC], out[3 % VEC]);
+    else if (VEC == 2) *reinterpret_cast<int2*>(own) = make_int2(out[0], out[1 % VEC]);
     else own[0] = out[0];
 }
 

@@ -17,7 +17,7 @@ UL_OK, UL_EINVAL, UL_ENOMEM, UL_ECUDA, UL_ESTATE = 0, -1, -2, -3, -4
 # every symbol include/ul.h declares (tests check that the library exports exactly these)
 SYMBOLS = [
     "ul_create", "ul_create_ext", "ul_workspace_bytes", "ul_destroy", "ul_init", "ul_set_beta",
-    "ul_set_links", "ul_get_links", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep",
+    "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep",
     "ul_set_subupdate", "ul_multilevel", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
     "ul_measure_end", "ul_plaquette", "ul_read_correlators", "ul_read_slab_averages",
     "ul_get_launch_count", "ul_philox_selftest", "ul_sync", "ul_last_error",
@@ -51,6 +51,8 @@ def lib():
         L.ul_set_beta.argtypes = [P, C.c_double]
         L.ul_set_links.argtypes = [P, P]
         L.ul_get_links.argtypes = [P, P]
+        L.ul_set_links_raw.argtypes = [P, P]
+        L.ul_get_links_raw.argtypes = [P, P]
         L.ul_get_counter.argtypes = [P, C.POINTER(C.c_uint64)]
         L.ul_set_counter.argtypes = [P, C.c_uint64]
         L.ul_sweep.argtypes = [P, C.c_int, C.c_int]
@@ -162,6 +164,17 @@ class Lattice:
             return out
         a = np.empty((4, self.Nt, self.Ns, self.Ns, self.Ns), dtype=np.float32) if out is None else out
         self._ck(lib().ul_get_links(self._h, _ptr(a)))
+        return a
+
+    def set_links_raw(self, raw):
+        """raw: canonical host array int32[4][Nt][Ns][Ns][Ns] of binary angles (exact state)."""
+        a = np.ascontiguousarray(raw, dtype=np.int32).reshape(-1)
+        assert a.size == 4 * self.V
+        self._ck(lib().ul_set_links_raw(self._h, _ptr(a)))
+
+    def get_links_raw(self):
+        a = np.empty((4, self.Nt, self.Ns, self.Ns, self.Ns), dtype=np.int32)
+        self._ck(lib().ul_get_links_raw(self._h, _ptr(a)))
         return a
 
     def get_counter(self):

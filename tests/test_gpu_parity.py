@@ -30,6 +30,16 @@ def wrapdiff(a, b):
     return np.abs(d - 2 * np.pi * np.round(d / (2 * np.pi)))
 
 
+def same_links(got, want):
+    """Boundary round trip: the library keeps 32-bit binary angles (2 pi / 2^32 per
+    unit).  fp32 radians come back bit for bit when 2^-6 <= |theta| < pi, to 1.2e-9 rad below that, and
+    mod 2 pi at the fp32 neighbours of +-pi (fp32(pi) > pi wraps to the other end)."""
+    a = np.abs(want)
+    mid = (a >= 2.0 ** -6) & (a < 3.14159)
+    d = wrapdiff(got, want)
+    return np.array_equal(got[mid], want[mid]) and d[a < 3.14159].max(initial=0.0) <= 1.3e-9 and d.max(initial=0.0) <= 1e-7
+
+
 def staple_k(o, mu, flat_sites):
     return np.array([o.staple(mu, int(s))[0] for s in flat_sites])
 
@@ -38,7 +48,7 @@ def check_links(got, want, before, o_before, label, allow_frac=1e-5):
     """P1 criterion.  o_before: oracle holding the configuration BEFORE the update (for k)."""
     diff = wrapdiff(got, want)
     untouched = (want == before)
-    assert np.array_equal(got[untouched & (diff == 0)], want[untouched & (diff == 0)])
+    assert diff[untouched].max(initial=0.0) <= 1.3e-9            # frozen / other-parity links: boundary round trip only
     bad = np.argwhere(diff > TOL)
     n_links = got.size
     n_ill = 0
@@ -80,14 +90,17 @@ def test_hot_start_and_layout_roundtrip(ul, ulo, Ns, Nt):
     seed = (0x51 << 32) | 0xC0FFEE
     g = ul.Lattice(Ns, Nt, 1.0, seed)
     o = ulo.Oracle(Ns, Nt, 1.0, seed)
-    assert np.array_equal(g.get_links(), o.get_links())          # same Philox stream, bit for bit
+    assert same_links(g.get_links(), o.get_links())              # same Philox stream
     links = inputs.hot_links(Ns, Nt, 3)
     g.set_links(links)
-    assert np.array_equal(g.get_links(), links)
+    assert same_links(g.get_links(), links)
+    again = g.get_links()
+    g.set_links(again)
+    assert np.array_equal(g.get_links(), again)                  # idempotent after the first conversion
     g.init(0)
     assert not g.get_links().any()
     g.init(1)
-    assert np.array_equal(g.get_links(), o.get_links())
+    assert same_links(g.get_links(), o.get_links())
 
 
 def test_set_links_rejects_unwrapped_angles(ul):
@@ -203,10 +216,10 @@ def test_runs_are_bitwise_reproducible(ul):
 def test_counter_resume_is_exact(ul):
     a = ul.Lattice(8, 4, 1.0, 11)
     a.sweep(2, 1)
-    links, ctr = a.get_links(), a.get_counter()
+    links, ctr = a.get_links_raw(), a.get_counter()
     a.sweep(1, 1)
     b = ul.Lattice(8, 4, 1.0, 11)
-    b.set_links(links)
+    b.set_links_raw(links)
     b.set_counter(ctr)
     b.sweep(1, 1)
     assert np.array_equal(a.get_links(), b.get_links())
@@ -430,7 +443,7 @@ def test_full_size_64_sampled_against_oracle(ul, ulo):
     g = ul.Lattice(Ns, Nt, beta, seed)
     o = ulo.Oracle(Ns, Nt, beta, seed)
     links = o.get_links()
-    assert np.array_equal(g.get_links(), links)
+    assert same_links(g.get_links(), links)
     ok, worst = rel_ok(g.plaquette(), o.plaquette(), 3 * Ns ** 4, rms_term=0.7)
     assert ok, worst
     for kind, parity, mu, d in ((1, 0, 1, 0), (0, 1, 0, 0), (0, 0, 3, 2)):
