@@ -150,7 +150,7 @@ def run_reference(args, rank, world):
         return
     w = WORKLOAD
     total = args.steps + args.warmup
-    budget = max(0.3, min(20.0, 150.0 / max(1, total)))
+    budget = args.budget_s if args.budget_s else max(0.3, min(20.0, 150.0 / max(1, total)))
     vals, sample, secs = [], "", []
     for i in range(total):
         v, sample, dt = oracle_sample(w, budget)
@@ -292,6 +292,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--budget-s", type=float, default=0.0, help="CPU seconds per oracle sample (reference arm / cpu_baseline)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
