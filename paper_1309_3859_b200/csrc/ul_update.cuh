@@ -83,8 +83,8 @@ __device__ __forceinline__ void staple_pair(const int* __restrict__ th, int Vh, 
     load_row<VEC, -n1>(th, a_nu_q + st.e0 + st.dm[NU], st, F);                     // theta_nu(x-nu)
 #pragma unroll
     for (int i = 0; i < VEC; ++i) {
-        ulm::cis_accumulate((int)((unsigned)A[i] + (unsigned)B[i] - (unsigned)C[i]), Sx[i], Sy[i]);
-        ulm::cis_accumulate((int)((unsigned)D[i] + (unsigned)E[i] - (unsigned)F[i]), Sx[i], Sy[i]);
+        ulm::cis_pair_accumulate((int)((unsigned)A[i] + (unsigned)B[i] - (unsigned)C[i]),
+                                 (int)((unsigned)D[i] + (unsigned)E[i] - (unsigned)F[i]), Sx[i], Sy[i]);
     }
 }
 
