@@ -28,7 +28,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-WORKLOAD = dict(name="cfg5_64^4", Ns=64, Nt=64, beta=0.98, seed=5, n_hb=1, n_or=4, slab_d=2, n_sub=2, r_max=16)
+WORKLOAD = dict(name="cfg5_64^4", Ns=64, Nt=64, beta=0.98, seed=5, n_hb=1, n_or=4, slab_d=2, n_sub=8, r_max=16)
 METRIC = "link_updates_per_s"
 UNIT = "link updates/s"
 BYTES_PER_UPDATE_OR = 36.0     # DESIGN.md / SURVEY 8(d): 3V + V/2 + V/2 reads, V/2 writes per V/2 updates, fp32

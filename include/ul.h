@@ -128,6 +128,14 @@ int ul_measure_begin(ul_ctx* h, int slab_thickness, int r_max, const int* field_
 int ul_accumulate(ul_ctx* h);
 int ul_measure_end(ul_ctx* h);
 
+/* Accumulation batch depth (rows a7, a8).  The library tabulates up to `depth` configurations
+ * (exp(i sum_t theta_0) per slab and site, and the plaquette sums) and adds them to the slab sums
+ * in ONE read-modify-write pass, in sub-update order: the same sequence of fp64 additions as
+ * `depth` single passes, so results do not depend on it (tested bit for bit).  depth = 0 restores
+ * the default (8, less when the tables would outgrow the accumulators); values above the default
+ * are clamped.  Takes effect at the next measurement.  UL_EINVAL: depth < 0. */
+int ul_set_accum_batch(ul_ctx* h, int depth);
+
 /* Mean of cos theta_P (Eq. 6) over all 6V plaquettes, over the 3V time-like and the
  * 3V space-like ones: HOST double[3].  Synchronises. */
 int ul_plaquette(ul_ctx* h, double* mean_cos);

@@ -19,9 +19,13 @@
 namespace {
 
 constexpr int NBLK = 592;   // blocks of the two-stage reductions: 4 per SM on 148 SMs
+constexpr int TBLK = 8 * NBLK;   // blocks of the slab-table kernel (grid-stride; one partial per block and column)
+
+constexpr int KBATCH = 8;   // configurations accumulated per read-modify-write pass over the accumulators
 
 struct Workspace {           // byte offsets into the measurement workspace
-    size_t Th = 0, Ot = 0, fps = 0, A2 = 0, B2 = 0, A4 = 0, B4 = 0, partial = 0, result = 0, total = 0;
+    size_t U = 0, Ot = 0, fps = 0, A2 = 0, B2 = 0, A4 = 0, B4 = 0, partial = 0, result = 0, total = 0;
+    int kb = 1;              // batch depth: slots of U (and of Ot when field points are measured)
 };
 
 size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
@@ -31,9 +35,15 @@ Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_f
     const size_t Vs = (size_t)Ns * Ns * Ns;
     const size_t n_in = (size_t)(Nt / d_in), n_out = d_out > 0 ? (size_t)(Nt / d_out) : 0;
     const size_t F12 = (size_t)n_fp * 12, R = (size_t)r_max;
+    // batch depth: KBATCH, reduced if the per-configuration tables would outgrow the accumulators they feed
+    const size_t table = n_in * Vs * (16 + (n_fp > 0 ? 48 : 0));
+    const size_t accum = 3 * R * n_in * Vs * 16 * (1 + F12);
+    int kb = KBATCH;
+    while (kb > 1 && (size_t)kb * table > accum / 2 + ((size_t)64 << 20)) kb >>= 1;
+    w.kb = kb;
     size_t o = 0;
-    w.Th = o;  o = align_up(o + n_in * Vs * sizeof(int));
-    w.Ot = o;  o = align_up(o + 12 * n_in * Vs * sizeof(float));
+    w.U = o;   o = align_up(o + (size_t)kb * n_in * Vs * 16);
+    w.Ot = o;  o = align_up(o + (n_fp > 0 ? (size_t)kb * 12 * n_in * Vs * sizeof(float) : 0));
     w.fps = o; o = align_up(o + (size_t)(n_fp > 0 ? n_fp : 1) * 3 * sizeof(int));
     w.A2 = o;  o = align_up(o + 3 * R * n_in * Vs * 16);
     w.B2 = o;  o = align_up(o + 3 * R * n_in * F12 * Vs * 16);
@@ -41,7 +51,7 @@ Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_f
     w.B4 = o;  o = align_up(o + 3 * R * n_out * F12 * Vs * 16);
     const size_t n_entries = R * (1 + F12);
     size_t np = 2 * n_entries;
-    if (np < 12) np = 12;
+    if (np < 12 * (TBLK / NBLK)) np = 12 * (TBLK / NBLK);
     w.partial = o; o = align_up(o + np * NBLK * sizeof(double));
     w.result = o;  o = align_up(o + (2 * n_entries + 12 + 12) * sizeof(double));   // corr|field, vacuum, column sums
     w.total = o;
@@ -67,10 +77,12 @@ struct ul_ctx {
     int* d_bad = nullptr;
     int vec = 1, bx = 1, by = 1, bz = 1;
     int sub_hb = 1, sub_or = 3, sub_k = 1;
+    int batch_cap = 0;       // ul_set_accum_batch: 0 = default depth
     // open measurement
     bool open = false;
     int d = 0, r_max = 0, n_fp = 0, n_slab = 0, d_out = 0, n_outer = 0;
     long long n_acc = 0;
+    int n_pending = 0;       // configurations tabulated but not yet added to the accumulators
     Workspace ws;
     // last result
     bool have = false;
@@ -180,9 +192,11 @@ int open_measurement(ul_ctx* c, int d_in, int d_out, int r_max, const int* fps, 
         c->work = (char*)p; c->work_bytes = w.total; c->own_work = true;
     }
     c->ws = w;
+    if (c->batch_cap > 0 && c->batch_cap < c->ws.kb) c->ws.kb = c->batch_cap;
     c->d = d_in; c->d_out = d_out; c->r_max = r_max; c->n_fp = n_fp;
     c->n_slab = c->Nt / d_in; c->n_outer = d_out > 0 ? c->Nt / d_out : 0;
     c->n_acc = 0;
+    c->n_pending = 0;
     c->have = false;
     if (n_fp > 0) UL_CUDA(c, cudaMemcpyAsync(c->work + w.fps, fps, sizeof(int) * 3 * (size_t)n_fp, cudaMemcpyHostToDevice, c->stream));
     UL_CUDA(c, cudaMemsetAsync(c->work + w.A2, 0, w.partial - w.A2, c->stream));           // A2, B2, A4, B4
@@ -195,22 +209,47 @@ int open_measurement(ul_ctx* c, int d_in, int d_out, int r_max, const int* fps, 
 double* res_colsum(ul_ctx* c) { return wsp<double>(c, c->ws.result) + 2 * (size_t)c->r_max * (1 + 12 * (size_t)c->n_fp) + 12; }
 double* res_vacuum(ul_ctx* c) { return wsp<double>(c, c->ws.result) + 2 * (size_t)c->r_max * (1 + 12 * (size_t)c->n_fp); }
 
-// rows a7, a8 on the current configuration
-int accumulate(ul_ctx* c) {
-    const ulk::Geom g = geom(c);
+// adds the tabulated configurations (slots 0..n_pending-1) to the accumulators: rows a7, a8
+int flush(ul_ctx* c) {
+    if (c->n_pending == 0) return UL_OK;
     const long long n = (long long)c->n_slab * c->Vs;
     const int nb = (int)((n + 255) / 256);
-    ulk::k_slab_tables<<<nb, 256, 0, c->stream>>>(g, c->th, c->d, c->n_slab, wsp<int>(c, c->ws.Th), wsp<float>(c, c->ws.Ot));
     ulk::AccumArgs a;
-    a.g = g; a.d = c->d; a.n_slab = c->n_slab; a.r_max = c->r_max; a.n_fp = c->n_fp;
-    a.Th = wsp<int>(c, c->ws.Th); a.Ot = wsp<float>(c, c->ws.Ot); a.fps = wsp<int>(c, c->ws.fps);
+    a.g = geom(c); a.d = c->d; a.n_slab = c->n_slab; a.r_max = c->r_max; a.n_fp = c->n_fp; a.nk = c->n_pending;
+    a.U = wsp<double2>(c, c->ws.U); a.Ot = wsp<float>(c, c->ws.Ot); a.fps = wsp<int>(c, c->ws.fps);
     a.A = wsp<double2>(c, c->ws.A2); a.B = wsp<double2>(c, c->ws.B2);
-    ulk::k_accumulate<<<nb, 256, 0, c->stream>>>(a);
-    ulk::k_ot_colsum<<<dim3(NBLK, 12), 256, 0, c->stream>>>(wsp<float>(c, c->ws.Ot), n, wsp<double>(c, c->ws.partial));
-    ulk::k_sum_partials<<<12, 256, 0, c->stream>>>(wsp<double>(c, c->ws.partial), NBLK, res_colsum(c), 1.0, 1);
+    if (c->n_fp > 0) {
+        if (a.nk == 1) ulk::k_accumulate<1, true><<<nb, 256, 0, c->stream>>>(a);
+        else if (a.nk <= 4) ulk::k_accumulate<4, true><<<nb, 256, 0, c->stream>>>(a);
+        else ulk::k_accumulate<KBATCH, true><<<nb, 256, 0, c->stream>>>(a);
+    } else {
+        if (a.nk == 1) ulk::k_accumulate<1, false><<<nb, 256, 0, c->stream>>>(a);
+        else if (a.nk <= 4) ulk::k_accumulate<4, false><<<nb, 256, 0, c->stream>>>(a);
+        else ulk::k_accumulate<KBATCH, false><<<nb, 256, 0, c->stream>>>(a);
+    }
     UL_CUDA(c, cudaGetLastError());
-    c->launches += 4;
+    c->launches += 1;
+    c->n_pending = 0;
+    return UL_OK;
+}
+
+// tabulates the current configuration (U, Ot, column sums of O) into the next batch slot; the batch is
+// added to the accumulators when it is full, and before anything reads them
+int accumulate(ul_ctx* c) {
+    const long long n = (long long)c->n_slab * c->Vs;
+    ulk::TableArgs t;
+    t.g = geom(c); t.th = c->th; t.d = c->d; t.n_slab = c->n_slab;
+    t.U = wsp<double2>(c, c->ws.U) + (size_t)c->n_pending * n;
+    t.Ot = c->n_fp > 0 ? wsp<float>(c, c->ws.Ot) + (size_t)c->n_pending * 12 * n : nullptr;
+    t.partial = wsp<double>(c, c->ws.partial);
+    const int tb = (int)((n + 255) / 256) < TBLK ? (int)((n + 255) / 256) : TBLK;
+    ulk::k_slab_tables<<<tb, 256, 0, c->stream>>>(t);
+    ulk::k_sum_partials<<<12, 256, 0, c->stream>>>(t.partial, tb, res_colsum(c), 1.0, 1);
+    UL_CUDA(c, cudaGetLastError());
+    c->launches += 2;
     c->n_acc += 1;
+    c->n_pending += 1;
+    if (c->n_pending == c->ws.kb) return flush(c);
     return UL_OK;
 }
 
@@ -221,7 +260,8 @@ int finish(ul_ctx* c, const double2* A, const double2* B, int n_slab, double inv
     ulk::ReduceArgs a;
     a.Vs = c->Vs; a.r_max = R; a.n_fp = F; a.n_slab = n_slab; a.inv = inv; a.A = A; a.B = B;
     a.partial = wsp<double>(c, c->ws.partial);
-    ulk::k_slab_product<<<dim3(NBLK, n_entries), 256, 0, c->stream>>>(a);
+    ulk::k_slab_product<false><<<dim3(NBLK, R), 256, 0, c->stream>>>(a, 0);
+    if (F > 0) { ulk::k_slab_product<true><<<dim3(NBLK, n_entries - R), 256, 0, c->stream>>>(a, R); c->launches += 1; }
     double* res = wsp<double>(c, c->ws.result);
     // C /= 3 Vs ; G /= 3 Vs Nt (DESIGN R9)
     ulk::k_sum_partials<<<2 * R, 256, 0, c->stream>>>(a.partial, NBLK, res, 1.0 / (3.0 * (double)c->Vs), 0);
@@ -402,6 +442,11 @@ int ul_measure_begin(ul_ctx* c, int d, int r_max, const int* fps, int n_fp) {
     if (rc) return rc;
     return open_measurement(c, d, 0, r_max, fps, n_fp);
 }
+int ul_set_accum_batch(ul_ctx* c, int depth) {
+    if (!c || depth < 0) return fail(c, UL_EINVAL, "depth must be >= 0");
+    c->batch_cap = depth;
+    return UL_OK;
+}
 int ul_accumulate(ul_ctx* c) {
     if (!c) return fail(c, UL_EINVAL, "null handle");
     if (!c->open) return fail(c, UL_ESTATE, "no open measurement");
@@ -410,6 +455,8 @@ int ul_accumulate(ul_ctx* c) {
 int ul_measure_end(ul_ctx* c) {
     if (!c) return fail(c, UL_EINVAL, "null handle");
     if (!c->open || c->n_acc == 0) return fail(c, UL_ESTATE, "nothing accumulated");
+    const int rc = flush(c);
+    if (rc) return rc;
     const double inv = 1.0 / (double)c->n_acc;
     return finish(c, wsp<double2>(c, c->ws.A2), wsp<double2>(c, c->ws.B2), c->n_slab, inv, inv);
 }
@@ -448,6 +495,8 @@ int ul_multilevel2(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, int r_ma
             rc = accumulate(c);
             if (rc) return rc;
         }
+        rc = flush(c);
+        if (rc) return rc;
         ulk::k_combine<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>(a);          // Eqs. 32-33
         UL_CUDA(c, cudaGetLastError());
         c->launches += 1;

@@ -127,16 +127,34 @@ __global__ void __launch_bounds__(256) k_sum_partials(const double* __restrict__
 }
 
 // ---------------------------------------------------------------- plaquette angles
-// theta_P(a,b)(y) = theta_a(y) + theta_b(y+a) - theta_a(y+b) - theta_b(y), binary angle (exact mod 2 pi)
-__device__ __forceinline__ int plaq_fx(const Geom& g, const int* __restrict__ th, int a, int b, const int x[4]) {
-    int xa[4] = {x[0], x[1], x[2], x[3]}, xb[4] = {x[0], x[1], x[2], x[3]};
-    xa[a] = (x[a] + 1 == (a == 0 ? g.Nt : g.Ns)) ? 0 : x[a] + 1;
-    xb[b] = (x[b] + 1 == (b == 0 ? g.Nt : g.Ns)) ? 0 : x[b] + 1;
-    const unsigned t0 = (unsigned)__ldg(th + link_index(g, a, x[0], x[3], x[2], x[1]));
-    const unsigned t1 = (unsigned)__ldg(th + link_index(g, b, xa[0], xa[3], xa[2], xa[1]));
-    const unsigned t2 = (unsigned)__ldg(th + link_index(g, a, xb[0], xb[3], xb[2], xb[1]));
-    const unsigned t3 = (unsigned)__ldg(th + link_index(g, b, x[0], x[3], x[2], x[1]));
-    return (int)(t0 + t1 - t2 - t3);
+// theta_P(a,b)(x) = theta_a(x) + theta_b(x+a) - theta_a(x+b) - theta_b(x) as binary angles (wrapping adds:
+// exact mod 2 pi) for the six orientations (0,1)(0,2)(0,3)(1,2)(1,3)(2,3) of site x; th0 = theta_0(x).
+// 16 loads: the four links at x and the three transverse links at each of the four forward neighbours,
+// addressed by 32-bit element offsets (4V < 2^31 is checked by ul_create).
+__device__ __forceinline__ void site_plaquettes(const Geom& g, const int* __restrict__ th, const int x[4], int pl[6], int& th0) {
+    const int Ns = g.Ns, Nh = g.Nh, Vh = (int)g.Vh;
+    const int par = (x[0] + x[1] + x[2] + x[3]) & 1;
+    const int row = (x[0] * Ns + x[3]) * Ns + x[2];
+    const int e = row * Nh + (x[1] >> 1);
+    int en[4];                                                     // element offsets of the sites x + b (parity 1 - par)
+    en[0] = e + ((x[0] + 1 == g.Nt) ? -(g.Nt - 1) : 1) * Ns * Ns * Nh;
+    en[1] = row * Nh + (((x[1] + 1 == Ns) ? 0 : x[1] + 1) >> 1);
+    en[2] = e + ((x[2] + 1 == Ns) ? -(Ns - 1) : 1) * Nh;
+    en[3] = e + ((x[3] + 1 == Ns) ? -(Ns - 1) : 1) * Ns * Nh;
+    unsigned own[4], nb[4][4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a) own[a] = (unsigned)__ldg(th + (2 * a + par) * Vh + e);
+#pragma unroll
+    for (int b = 0; b < 4; ++b)
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+            if (a != b) nb[b][a] = (unsigned)__ldg(th + (2 * a + 1 - par) * Vh + en[b]);   // theta_a(x + b)
+    int o = 0;
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = a + 1; b < 4; ++b) pl[o++] = (int)(own[a] + nb[a][b] - nb[b][a] - own[b]);
+    th0 = (int)own[0];
 }
 
 // row a11: partial[0*nblk + b] = sum of cos over time-like plaquettes, [1*nblk + b] space-like
@@ -150,69 +168,86 @@ __global__ void __launch_bounds__(256) k_plaquette(Geom g, const int* __restrict
         x[2] = (int)(s % g.Ns); s /= g.Ns;
         x[3] = (int)(s % g.Ns); s /= g.Ns;
         x[0] = (int)s;
+        int pl[6], th0;
+        site_plaquettes(g, th, x, pl, th0);
+        float ct = 0.0f, cs = 0.0f;
 #pragma unroll
-        for (int a = 0; a < 4; ++a)
-#pragma unroll
-            for (int b = a + 1; b < 4; ++b) {
-                float c, sn;
-                ulm::sincos_bt(plaq_fx(g, th, a, b, x), c, sn);
-                if (a == 0) v[0] += (double)c; else v[1] += (double)c;
-            }
+        for (int o = 0; o < 6; ++o) {
+            float c, sn;
+            ulm::sincos_bt(pl[o], c, sn);
+            if (o < 3) ct += c; else cs += c;
+        }
+        v[0] += (double)ct;
+        v[1] += (double)cs;
     }
     block_sum<2>(v, sm);
     if (threadIdx.x == 0) { partial[blockIdx.x] = v[0]; partial[gridDim.x + blockIdx.x] = v[1]; }
 }
 
 // ---------------------------------------------------------------- per-configuration slab tables
-// Th[s][xs] = sum_{t in slab s} theta_0(xs,t), binary angle (wrapping sum = exact mod 2 pi)
-// Ot[o][kind][s][xs] = sum_{t in slab s} O(theta_P(o)(xs,t)),  O = 1 - cos (kind 0), sin (kind 1)
-__global__ void __launch_bounds__(256) k_slab_tables(Geom g, const int* __restrict__ th, int d, int n_slab,
-                                                     int* __restrict__ Th, float* __restrict__ Ot) {
-    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= (long long)n_slab * g.Vs) return;
-    const int s = (int)(idx / g.Vs);
-    long long r = idx - (long long)s * g.Vs;
-    int x[4];
-    x[1] = (int)(r % g.Ns); r /= g.Ns;
-    x[2] = (int)(r % g.Ns); r /= g.Ns;
-    x[3] = (int)r;
-    unsigned acc = 0u;
-    float o_c[6], o_s[6];
+// U[s][xs]  = exp(i sum_{t in slab s} theta_0(xs,t)) in fp64: the angle sum is a wrapping integer add
+//             (exact mod 2 pi) and sincospi of I 2^-31 is exact in its argument, so U is good to 1 ulp and
+//             every T^(d)(x,s,r mu) = U(x + r mu) conj(U(x)) (Eqs. 22, 25) is one fp64 complex product.
+// Ot[o][kind][s][xs] = sum_{t in slab s} O(theta_P(o)(xs,t)),  O = 1 - cos (kind 0), sin (kind 1); stored
+//             only when field points are measured (Ot != nullptr).
+// partial[col*gridDim.x + b] = block partial of the column sums of O (vacuum expectation values).
+struct TableArgs {
+    Geom g;
+    const int* th;
+    int d, n_slab;
+    double2* U;
+    float* Ot;
+    double* partial;
+};
+__global__ void __launch_bounds__(256) k_slab_tables(const TableArgs P) {
+    __shared__ double sm[12 * 32];
+    const Geom& g = P.g;
+    const long long n = (long long)P.n_slab * g.Vs;
+    double v[12];
 #pragma unroll
-    for (int o = 0; o < 6; ++o) { o_c[o] = 0.0f; o_s[o] = 0.0f; }
-    for (int t = s * d; t < (s + 1) * d; ++t) {
-        x[0] = t;
-        acc += (unsigned)__ldg(th + link_index(g, 0, t, x[3], x[2], x[1]));
-        int o = 0;
+    for (int o = 0; o < 12; ++o) v[o] = 0.0;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (long long)gridDim.x * blockDim.x) {
+        const int s = (int)(idx / g.Vs);
+        long long r = idx - (long long)s * g.Vs;
+        int x[4];
+        x[1] = (int)(r % g.Ns); r /= g.Ns;
+        x[2] = (int)(r % g.Ns); r /= g.Ns;
+        x[3] = (int)r;
+        unsigned acc = 0u;
+        float o_c[6], o_s[6];
 #pragma unroll
-        for (int a = 0; a < 4; ++a)
+        for (int o = 0; o < 6; ++o) { o_c[o] = 0.0f; o_s[o] = 0.0f; }
+        for (int t = s * P.d; t < (s + 1) * P.d; ++t) {
+            x[0] = t;
+            int pl[6], th0;
+            site_plaquettes(g, P.th, x, pl, th0);
+            acc += (unsigned)th0;
 #pragma unroll
-            for (int b = a + 1; b < 4; ++b) {
+            for (int o = 0; o < 6; ++o) {
                 float c, sn;
-                ulm::sincos_bt(plaq_fx(g, th, a, b, x), c, sn);
+                ulm::sincos_bt(pl[o], c, sn);
                 o_c[o] += 1.0f - c;
                 o_s[o] += sn;
-                ++o;
             }
-    }
-    Th[idx] = (int)acc;
-    const long long stride = (long long)n_slab * g.Vs;
+        }
+        double us, uc;
+        sincospi((double)(int)acc * (1.0 / 2147483648.0), &us, &uc);
+        P.U[idx] = make_double2(uc, us);
 #pragma unroll
-    for (int o = 0; o < 6; ++o) {
-        Ot[(long long)(2 * o) * stride + idx] = o_c[o];
-        Ot[(long long)(2 * o + 1) * stride + idx] = o_s[o];
+        for (int o = 0; o < 6; ++o) {
+            if (P.Ot) {
+                P.Ot[(long long)(2 * o) * n + idx] = o_c[o];
+                P.Ot[(long long)(2 * o + 1) * n + idx] = o_s[o];
+            }
+            v[2 * o] += (double)o_c[o];
+            v[2 * o + 1] += (double)o_s[o];
+        }
     }
-}
-
-// column sums of Ot for the vacuum expectation values: partial[col*nblk + b], col = 2*o + kind
-__global__ void __launch_bounds__(256) k_ot_colsum(const float* __restrict__ Ot, long long n, double* __restrict__ partial) {
-    __shared__ double sm[32];
-    const int col = blockIdx.y;
-    double v[1] = {0.0};
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
-        v[0] += (double)Ot[(long long)col * n + i];
-    block_sum<1>(v, sm);
-    if (threadIdx.x == 0) partial[(long long)col * gridDim.x + blockIdx.x] = v[0];
+    block_sum<12>(v, sm);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int o = 0; o < 12; ++o) P.partial[(long long)o * gridDim.x + blockIdx.x] = v[o];
+    }
 }
 
 // plaquette orientation (a,b) -> table column o and sign of the sin channel (theta_P(b,a) = -theta_P(a,b))
@@ -237,69 +272,101 @@ __device__ __forceinline__ void comp_dirs(int mu, int comp, int& a, int& b) {
 struct AccumArgs {
     Geom g;
     int d, n_slab, r_max, n_fp;
-    const int* Th;
-    const float* Ot;
+    int nk;               // configurations in this batch (1..KB), slots 0..nk-1 in sub-update order
+    const double2* U;     // [nk][n_slab*Vs]
+    const float* Ot;      // [nk][12][n_slab*Vs]   (n_fp > 0 only)
     const int* fps;       // device int[n_fp][3]
     double2* A;
     double2* B;
 };
 
-// rows a7, a8: one thread per (s, xs); loops over the charge axis mu and separation r
+// rows a7, a8 for a BATCH of nk <= KB configurations: one thread per (s, xs) loops over the charge axis mu and
+// the separation r, reads each accumulator entry once, adds the nk terms in sub-update order (the same
+// sequence of fp64 additions as nk single passes, so the result does not depend on the batching) and
+// writes it back once: 32/nk bytes of accumulator traffic per entry and sub-update instead of 32.
+// The accumulators are streamed (ld.cs / st.cs, RB entries in flight per thread); the U tables, which every
+// site re-reads 6 r_max times, stay in L1/L2.
+constexpr int ACC_RB = 4;
+
+template <int KB, bool FIELD>
 __global__ void __launch_bounds__(256) k_accumulate(const AccumArgs P) {
     const Geom& g = P.g;
+    const long long n = (long long)P.n_slab * g.Vs;
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= (long long)P.n_slab * g.Vs) return;
+    if (idx >= n) return;
     const int s = (int)(idx / g.Vs);
-    const long long xs = idx - (long long)s * g.Vs;
-    long long q = xs;
+    const int xs = (int)(idx - (long long)s * g.Vs);
+    const int Ns = g.Ns;
     int x[4];
     x[0] = 0;
-    x[1] = (int)(q % g.Ns); q /= g.Ns;
-    x[2] = (int)(q % g.Ns); q /= g.Ns;
-    x[3] = (int)q;
-    const int Ns = g.Ns;
-    const int* Ths = P.Th + (long long)s * g.Vs;
-    const int th0 = Ths[xs];
-    const long long ot_stride = (long long)P.n_slab * g.Vs;
+    x[1] = xs % Ns;
+    x[2] = (xs / Ns) % Ns;
+    x[3] = xs / (Ns * Ns);
+    const int stride[4] = {0, 1, Ns, Ns * Ns};
+    const double2* __restrict__ Us = P.U + (long long)s * g.Vs;
+    const long long stepA = (long long)P.n_slab * g.Vs;                  // A[mu][r] -> A[mu][r+1]
+    double2 u0[KB];
+#pragma unroll
+    for (int k = 0; k < KB; ++k)
+        if (k < P.nk) u0[k] = Us[k * n + xs];
+#pragma unroll
     for (int mu = 1; mu <= 3; ++mu) {
         const int nu = 1 + (mu % 3), rho = 1 + ((mu + 1) % 3);
-        for (int r = 1; r <= P.r_max; ++r) {
-            int y[4] = {0, x[1], x[2], x[3]};
-            y[mu] = wrapc(x[mu] + r, Ns);                                      // r <= Ns/2
-            const long long ys = y[1] + (long long)Ns * (y[2] + (long long)Ns * y[3]);
-            // T^(d)(x,s,r mu) = exp(i sum_{t in slab} [theta_0(x + r mu, t) - theta_0(x, t)])  (Eq. 22, 25)
-            float c, sn;
-            ulm::sincos_bt((int)((unsigned)Ths[ys] - (unsigned)th0), c, sn);
-            const double Tr = (double)c, Ti = (double)sn;
-            const long long a_idx = (((long long)(mu - 1) * P.r_max + (r - 1)) * P.n_slab + s) * g.Vs + xs;
-            double2 a = P.A[a_idx];
-            a.x += Tr; a.y += Ti;
-            P.A[a_idx] = a;
-            for (int fp = 0; fp < P.n_fp; ++fp) {
-                // anchor y = x + (floor(r/2)+a) mu + b nu + c rho  (DESIGN R10)
-                int z[4] = {0, x[1], x[2], x[3]};
-                z[mu] = modc(z[mu] + r / 2 + P.fps[3 * fp], Ns);
-                z[nu] = modc(z[nu] + P.fps[3 * fp + 1], Ns);
-                z[rho] = modc(z[rho] + P.fps[3 * fp + 2], Ns);
-                const long long zs = z[1] + (long long)Ns * (z[2] + (long long)Ns * z[3]) + (long long)s * g.Vs;
-                const long long b_base = (((long long)(mu - 1) * P.r_max + (r - 1)) * P.n_slab + s) * P.n_fp + fp;
+        double2* Ap = P.A + ((long long)(mu - 1) * P.r_max * P.n_slab + s) * g.Vs + xs;
+        for (int r0 = 1; r0 <= P.r_max; r0 += ACC_RB) {
+            double2 a[ACC_RB];
 #pragma unroll
-                for (int comp = 0; comp < 6; ++comp) {
-                    int pa, pb, o;
-                    float sgn;
-                    comp_dirs(mu, comp, pa, pb);
-                    orient_of(pa, pb, o, sgn);
-                    const double Oc = (double)P.Ot[(long long)(2 * o) * ot_stride + zs];
-                    const double Os = (double)(sgn * P.Ot[(long long)(2 * o + 1) * ot_stride + zs]);
-                    const long long b0 = (b_base * 12 + 2 * comp) * g.Vs + xs;
-                    double2 b = P.B[b0];
-                    b.x += Tr * Oc; b.y += Ti * Oc;
-                    P.B[b0] = b;
-                    b = P.B[b0 + g.Vs];
-                    b.x += Tr * Os; b.y += Ti * Os;
-                    P.B[b0 + g.Vs] = b;
+            for (int i = 0; i < ACC_RB; ++i)
+                if (r0 + i <= P.r_max) a[i] = __ldcs(Ap + i * stepA);
+#pragma unroll
+            for (int i = 0; i < ACC_RB; ++i) {
+                const int r = r0 + i;
+                if (r > P.r_max) break;
+                // T^(d)(x,s,r mu) = U(x + r mu) conj(U(x))  (Eqs. 22, 25)
+                const int ys = xs + (wrapc(x[mu] + r, Ns) - x[mu]) * stride[mu];         // r <= Ns/2
+                double2 T[KB];
+#pragma unroll
+                for (int k = 0; k < KB; ++k)
+                    if (k < P.nk) {
+                        const double2 v = Us[k * n + ys];
+                        T[k].x = fma(v.x, u0[k].x, v.y * u0[k].y);
+                        T[k].y = fma(v.y, u0[k].x, -(v.x * u0[k].y));
+                        a[i].x += T[k].x; a[i].y += T[k].y;
+                    }
+                __stcs(Ap + i * stepA, a[i]);
+                if (FIELD) {
+                    for (int fp = 0; fp < P.n_fp; ++fp) {
+                        // anchor y = x + (floor(r/2)+a) mu + b nu + c rho  (DESIGN R10)
+                        int z[4] = {0, x[1], x[2], x[3]};
+                        z[mu] = modc(z[mu] + r / 2 + P.fps[3 * fp], Ns);
+                        z[nu] = modc(z[nu] + P.fps[3 * fp + 1], Ns);
+                        z[rho] = modc(z[rho] + P.fps[3 * fp + 2], Ns);
+                        const long long zs = z[1] + (long long)Ns * (z[2] + (long long)Ns * z[3]) + (long long)s * g.Vs;
+                        const long long b_base = (((long long)(mu - 1) * P.r_max + (r - 1)) * P.n_slab + s) * P.n_fp + fp;
+#pragma unroll
+                        for (int comp = 0; comp < 6; ++comp) {
+                            int pa, pb, o;
+                            float sgn;
+                            comp_dirs(mu, comp, pa, pb);
+                            orient_of(pa, pb, o, sgn);
+                            const long long b0 = (b_base * 12 + 2 * comp) * g.Vs + xs;
+                            double2 bc = __ldcs(P.B + b0), bs = __ldcs(P.B + b0 + g.Vs);
+#pragma unroll
+                            for (int k = 0; k < KB; ++k)
+                                if (k < P.nk) {
+                                    const float* Otk = P.Ot + (long long)k * 12 * n;
+                                    const double Oc = (double)Otk[(long long)(2 * o) * n + zs];
+                                    const double Os = (double)(sgn * Otk[(long long)(2 * o + 1) * n + zs]);
+                                    bc.x += T[k].x * Oc; bc.y += T[k].y * Oc;
+                                    bs.x += T[k].x * Os; bs.y += T[k].y * Os;
+                                }
+                            __stcs(P.B + b0, bc);
+                            __stcs(P.B + b0 + g.Vs, bs);
+                        }
+                    }
                 }
             }
+            Ap += ACC_RB * stepA;
         }
     }
 }
@@ -366,33 +433,47 @@ struct ReduceArgs {
     const double2* B;
     double* partial;
 };
-__global__ void __launch_bounds__(256) k_slab_product(const ReduceArgs P) {
+template <bool FIELD>
+__global__ void __launch_bounds__(256) k_slab_product(const ReduceArgs P, int o_first) {
     __shared__ double sm[2 * 32];
-    const int o = blockIdx.y;
+    const int o = o_first + blockIdx.y;
     const int F12 = P.n_fp * 12;
-    const bool is_c = o < P.r_max;
-    const int r1 = is_c ? o : (o - P.r_max) / F12;                             // r - 1
-    const int f = is_c ? 0 : (o - P.r_max) - r1 * F12;
+    const int r1 = FIELD ? (o - P.r_max) / F12 : o;                            // r - 1
+    const int f = FIELD ? (o - P.r_max) - r1 * F12 : 0;
     double v[2] = {0.0, 0.0};
     for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < 3 * P.Vs; j += (long long)gridDim.x * blockDim.x) {
         const int mu1 = (int)(j / P.Vs);
         const long long xs = j - (long long)mu1 * P.Vs;
         const long long mr = (long long)mu1 * P.r_max + r1;
+        const double2* Ap = P.A + mr * P.n_slab * P.Vs + xs;
         double2 pp = make_double2(1.0, 0.0), gg = make_double2(0.0, 0.0);
-        for (int s = 0; s < P.n_slab; ++s) {
-            const long long si = mr * P.n_slab + s;
-            double2 a = P.A[si * P.Vs + xs];
-            a.x *= P.inv; a.y *= P.inv;
-            if (!is_c) {
+        if (!FIELD) {
+            int s = 0;
+            for (; s + 4 <= P.n_slab; s += 4) {                                 // four loads in flight per thread
+                double2 a[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) a[i] = __ldcs(Ap + (long long)(s + i) * P.Vs);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) { a[i].x *= P.inv; a[i].y *= P.inv; pp = cmul(pp, a[i]); }
+            }
+            for (; s < P.n_slab; ++s) {
+                double2 a = __ldcs(Ap + (long long)s * P.Vs);
+                a.x *= P.inv; a.y *= P.inv;
+                pp = cmul(pp, a);
+            }
+            v[0] += pp.x; v[1] += pp.y;
+        } else {
+            for (int s = 0; s < P.n_slab; ++s) {
+                const long long si = mr * P.n_slab + s;
+                double2 a = Ap[(long long)s * P.Vs];
                 double2 b = P.B[(si * F12 + f) * P.Vs + xs];
-                b.x *= P.inv; b.y *= P.inv;
+                a.x *= P.inv; a.y *= P.inv; b.x *= P.inv; b.y *= P.inv;
                 const double2 g1 = cmul(gg, a), g2 = cmul(pp, b);
                 gg = make_double2(g1.x + g2.x, g1.y + g2.y);
+                pp = cmul(pp, a);
             }
-            pp = cmul(pp, a);
+            v[0] += gg.x; v[1] += gg.y;
         }
-        v[0] += is_c ? pp.x : gg.x;
-        v[1] += is_c ? pp.y : gg.y;
     }
     block_sum<2>(v, sm);
     if (threadIdx.x == 0) {

@@ -19,7 +19,7 @@ SYMBOLS = [
     "ul_create", "ul_create_ext", "ul_workspace_bytes", "ul_destroy", "ul_init", "ul_set_beta",
     "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep",
     "ul_set_subupdate", "ul_multilevel", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
-    "ul_measure_end", "ul_plaquette", "ul_read_correlators", "ul_read_slab_averages",
+    "ul_measure_end", "ul_set_accum_batch", "ul_plaquette", "ul_read_correlators", "ul_read_slab_averages",
     "ul_get_launch_count", "ul_philox_selftest", "ul_sync", "ul_last_error",
 ]
 
@@ -61,6 +61,7 @@ def lib():
         L.ul_multilevel.argtypes = [P, C.c_int, C.c_int, C.c_int, P, C.c_int]
         L.ul_multilevel2.argtypes = [P, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, P, C.c_int]
         L.ul_measure_begin.argtypes = [P, C.c_int, C.c_int, P, C.c_int]
+        L.ul_set_accum_batch.argtypes = [P, C.c_int]
         L.ul_accumulate.argtypes = [P]
         L.ul_measure_end.argtypes = [P]
         L.ul_plaquette.argtypes = [P, P]
@@ -193,6 +194,9 @@ class Lattice:
 
     def set_subupdate(self, n_hb, n_or, k_sweeps=1):
         self._ck(lib().ul_set_subupdate(self._h, int(n_hb), int(n_or), int(k_sweeps)))
+
+    def set_accum_batch(self, depth):
+        self._ck(lib().ul_set_accum_batch(self._h, int(depth)))
 
     def multilevel(self, slab_thickness, n_sub, r_max, field_points=None):
         fp, n = _fps(field_points)

@@ -49,13 +49,14 @@ def test_argument_validation_without_device(libul):
 
 def test_workspace_sizing_follows_paper_formula(libul):
     # field accumulators = 2 x 8 B x (volume / step) x (points) per (mu, r, channel).
-    # Here: Ns^3 (Nt/d) 3 r_max (1 + 12 n_fp) complex doubles plus O(volume) scratch.
+    # Here: Ns^3 (Nt/d) 3 r_max (1 + 12 n_fp) complex doubles plus O(volume) scratch: up to 8 batched
+    # per-configuration tables of 64 B per (slab, site) (fp64 U, 12 fp32 plaquette sums).
     Ns, Nt, d, R, F = 24, 16, 2, 12, 5
     Vs, S = Ns ** 3, Nt // d
     acc = 16 * Vs * S * 3 * R * (1 + 12 * F)
     got = libul.workspace_bytes(Ns, Nt, d, 0, R, F)
     scratch = got - acc
-    assert 0 < scratch < 64 * Vs * S + 2 * R * (1 + 12 * F) * 2 * 592 * 8 + 65536
+    assert 0 < scratch < 8 * 64 * Vs * S + 2 * R * (1 + 12 * F) * 2 * 592 * 8 + 65536
     two = libul.workspace_bytes(Ns, Nt, 2, 4, R, F)
     assert abs((two - got) - acc // 2) < 4096
     assert libul.workspace_bytes(Ns, Nt, 3, 0, R, F) == 0          # 16 % 3 != 0

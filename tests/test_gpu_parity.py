@@ -213,6 +213,25 @@ def test_runs_are_bitwise_reproducible(ul):
     assert np.array_equal(res[0][2], res[1][2])
 
 
+@pytest.mark.parametrize("n_sub", [5, 11])
+def test_accumulation_batch_depth_does_not_change_results(ul, n_sub):
+    """Rows a7/a8: the batched read-modify-write pass adds the configurations in sub-update order, so
+    slab sums, correlators and field values are bit-identical for every batch depth (ragged tails too)."""
+    res = []
+    for depth in (1, 3, 4, 0):
+        g = ul.Lattice(8, 4, 0.99, 21)
+        g.sweep(2, 2)
+        g.set_accum_batch(depth)
+        g.multilevel(2, n_sub, 4, [(0, 0, 0), (1, 1, 0)])
+        res.append((g.read_slab_averages(),) + tuple(g.read_correlators()))
+        launches = g.launch_count()
+        g.multilevel2(2, 3, 4, 2, 3, [(0, 1, 0)])
+        res[-1] = res[-1] + tuple(g.read_correlators()) + (launches,)
+    for r in res[1:]:
+        assert all(np.array_equal(a, b) for a, b in zip(res[0][:-1], r[:-1]))
+    assert res[0][-1] > res[-1][-1]                                # deeper batches launch fewer passes
+
+
 def test_counter_resume_is_exact(ul):
     a = ul.Lattice(8, 4, 1.0, 11)
     a.sweep(2, 1)
