@@ -151,7 +151,7 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
     a.parity = parity; a.slab_d = slab_d; a.beta = (float)c->beta;
     a.key0 = (uint32_t)(c->seed & 0xffffffffu); a.key1 = (uint32_t)(c->seed >> 32);
     a.sweep_lo = (uint32_t)(c->sweep & 0xffffffffu); a.sweep_hi = (uint32_t)(c->sweep >> 32);
-    const dim3 block(c->bx, c->by, c->bz), grid(c->Ns / c->by, c->Ns / c->bz, n_t);
+    const dim3 block(c->bx, c->by, 2 * c->bz), grid(c->Nh / c->by, c->Ns / c->bz, n_t);   // by = x2 row PAIRS per block
     const cudaError_t e = kind == 0 ? launch_update_mu<0>(c, mu, a, grid, block) : launch_update_mu<1>(c, mu, a, grid, block);
     if (e != cudaSuccess) return fail(c, UL_ECUDA, std::string("k_update launch: ") + cudaGetErrorString(e));
     c->launches += 1;
@@ -293,7 +293,7 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     if (Ns < 2 || Nt < 2 || (Ns & 1) || (Nt & 1) || !(beta >= 0.0)) return fail(nullptr, UL_EINVAL, "need even Ns, Nt >= 2 and beta >= 0");
     const int Nh = Ns / 2;
     const int vec = (Nh % 4 == 0) ? 4 : ((Nh % 2 == 0) ? 2 : 1);
-    if (Nh / vec > 256 || 4.0 * (double)Ns * Ns * Ns * Nt >= 2147483648.0) return fail(nullptr, UL_EINVAL, "lattice too large for this build");
+    if (Nh / vec > 128 || 4.0 * (double)Ns * Ns * Ns * Nt >= 2147483648.0) return fail(nullptr, UL_EINVAL, "lattice too large for this build");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(nullptr, UL_ECUDA, "no CUDA device");
     ul_ctx* c = new (std::nothrow) ul_ctx;
@@ -302,8 +302,8 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     c->Vs = (long long)Ns * Ns * Ns; c->V = c->Vs * Nt; c->Vh = c->V / 2;
     c->beta = beta; c->seed = seed;
     c->vec = vec; c->bx = Nh / vec;
-    c->by = largest_divisor_le(Ns, 256 / c->bx);
-    c->bz = largest_divisor_le(Ns, 256 / (c->bx * c->by));
+    c->by = largest_divisor_le(Nh, 128 / c->bx);                     // x2 row pairs per block
+    c->bz = largest_divisor_le(Ns, 128 / (c->bx * c->by));
     const size_t need = sizeof(float) * 4 * (size_t)c->V;
     if (ext) {
         if (!dev_links || links_bytes < need || ((uintptr_t)dev_links & 255)) { delete c; return fail(nullptr, UL_EINVAL, "dev_links too small or misaligned"); }

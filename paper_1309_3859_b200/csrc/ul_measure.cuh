@@ -329,9 +329,14 @@ __global__ void __launch_bounds__(256) k_accumulate(const AccumArgs P) {
                 for (int k = 0; k < KB; ++k)
                     if (k < P.nk) {
                         const double2 v = Us[k * n + ys];
-                        T[k].x = fma(v.x, u0[k].x, v.y * u0[k].y);
-                        T[k].y = fma(v.y, u0[k].x, -(v.x * u0[k].y));
-                        a[i].x += T[k].x; a[i].y += T[k].y;
+                        if (FIELD) {
+                            T[k].x = fma(v.x, u0[k].x, v.y * u0[k].y);
+                            T[k].y = fma(v.y, u0[k].x, -(v.x * u0[k].y));
+                            a[i].x += T[k].x; a[i].y += T[k].y;
+                        } else {                                   // the same term folded into the sum: 4 DFMA instead of 6 ops
+                            a[i].x = fma(v.y, u0[k].y, fma(v.x, u0[k].x, a[i].x));
+                            a[i].y = fma(-v.x, u0[k].y, fma(v.y, u0[k].x, a[i].y));
+                        }
                     }
                 __stcs(Ap + i * stepA, a[i]);
                 if (FIELD) {

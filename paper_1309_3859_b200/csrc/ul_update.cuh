@@ -37,7 +37,7 @@ struct Site {
 
 // Loads the VEC angles at element offset `idx` shifted by the x1-displacement D1 (-1, 0, +1):
 // x1 + 1 lives at h + off, x1 - 1 at h - 1 + off of the other-parity row.
-template <int VEC, int D1>
+template <int VEC, int D1, int OFF>
 __device__ __forceinline__ void load_row(const int* __restrict__ th, int idx, const Site& st, int v[VEC]) {
     if (VEC == 4) {
         const int4 q = __ldg(reinterpret_cast<const int4*>(th + idx));
@@ -49,14 +49,14 @@ __device__ __forceinline__ void load_row(const int* __restrict__ th, int idx, co
         v[0] = __ldg(th + idx);
     }
     if (D1 > 0) {
-        if (st.off) {                                 // shift by +1: need element h0 + VEC
+        if (OFF) {                                    // shift by +1: need element h0 + VEC
             const int x = __ldg(th + idx + st.dxp);
 #pragma unroll
             for (int i = 0; i < VEC - 1; ++i) v[i] = v[i + 1];
             v[VEC - 1] = x;
         }
     } else if (D1 < 0) {
-        if (!st.off) {                                // shift by -1: need element h0 - 1
+        if (!OFF) {                                   // shift by -1: need element h0 - 1
             const int x = __ldg(th + idx + st.dxm);
 #pragma unroll
             for (int i = VEC - 1; i > 0; --i) v[i] = v[i - 1];
@@ -69,18 +69,18 @@ __device__ __forceinline__ void load_row(const int* __restrict__ th, int idx, co
 //   S += e^{-i sigma+} + e^{-i sigma-},  -sigma+ = th_nu(x) + th_mu(x+nu) - th_nu(x+mu),
 //                                        -sigma- = th_nu(x+mu-nu) + th_mu(x-nu) - th_nu(x-nu).
 // The phase sums are wrapping int32 adds: exact and already reduced mod 2 pi.
-template <int MU, int NU, int VEC>
+template <int MU, int NU, int VEC, int OFF>
 __device__ __forceinline__ void staple_pair(const int* __restrict__ th, int Vh, int p, const Site& st,
                                             float Sx[VEC], float Sy[VEC]) {
     constexpr int m1 = (MU == 1), n1 = (NU == 1);
     const int a_nu_p = (NU * 2 + p) * Vh, a_nu_q = (NU * 2 + 1 - p) * Vh, a_mu_q = (MU * 2 + 1 - p) * Vh;
     int A[VEC], B[VEC], C[VEC], D[VEC], E[VEC], F[VEC];
-    load_row<VEC, 0>(th, a_nu_p + st.e0, st, A);                                   // theta_nu(x)
-    load_row<VEC, n1>(th, a_mu_q + st.e0 + st.dp[NU], st, B);                      // theta_mu(x+nu)
-    load_row<VEC, m1>(th, a_nu_q + st.e0 + st.dp[MU], st, C);                      // theta_nu(x+mu)
-    load_row<VEC, m1 - n1>(th, a_nu_p + st.e0 + st.dp[MU] + st.dm[NU], st, D);     // theta_nu(x+mu-nu)
-    load_row<VEC, -n1>(th, a_mu_q + st.e0 + st.dm[NU], st, E);                     // theta_mu(x-nu)
-    load_row<VEC, -n1>(th, a_nu_q + st.e0 + st.dm[NU], st, F);                     // theta_nu(x-nu)
+    load_row<VEC, 0, OFF>(th, a_nu_p + st.e0, st, A);                                   // theta_nu(x)
+    load_row<VEC, n1, OFF>(th, a_mu_q + st.e0 + st.dp[NU], st, B);                      // theta_mu(x+nu)
+    load_row<VEC, m1, OFF>(th, a_nu_q + st.e0 + st.dp[MU], st, C);                      // theta_nu(x+mu)
+    load_row<VEC, m1 - n1, OFF>(th, a_nu_p + st.e0 + st.dp[MU] + st.dm[NU], st, D);     // theta_nu(x+mu-nu)
+    load_row<VEC, -n1, OFF>(th, a_mu_q + st.e0 + st.dm[NU], st, E);                     // theta_mu(x-nu)
+    load_row<VEC, -n1, OFF>(th, a_nu_q + st.e0 + st.dm[NU], st, F);                     // theta_nu(x-nu)
 #pragma unroll
     for (int i = 0; i < VEC; ++i) {
         ulm::cis_pair_accumulate((int)((unsigned)A[i] + (unsigned)B[i] - (unsigned)C[i]),
@@ -96,38 +96,18 @@ __device__ __forceinline__ T pick(const T v[VEC], int j) {        // v[j] withou
     return r;
 }
 
-// KIND 0 = heatbath, 1 = overrelaxation.  Block (Nh/VEC, BY, BZ); grid (Ns/BY, Ns/BZ, n_t)
-// with n_t = Nt, or Nt*(d-1)/d active time layers for a masked spatial direction.
-template <int KIND, int MU, int VEC>
-__global__ void __launch_bounds__(256) k_update(const UpdateArgs P) {
-    const int Ns = P.Ns, Nh = P.Nh, Nt = P.Nt;
-    const int h0 = threadIdx.x * VEC;
-    const int x2 = blockIdx.x * blockDim.y + threadIdx.y;
-    const int x3 = blockIdx.y * blockDim.z + threadIdx.z;
-    int t = blockIdx.z;
-    if (MU != 0 && P.slab_d > 0) {                    // enumerate only the non-frozen layers
-        const int dm = P.slab_d - 1;
-        const int s = t / dm;
-        t = s * P.slab_d + 1 + (t - s * dm);
-    }
+// The update of the VEC links of one thread, compiled separately for the two values of the row's offset
+// bit OFF (x1 = 2h + OFF) so that the x1-shifted neighbour rows are selected by register naming at compile
+// time instead of predicated moves.  KIND 0 = heatbath, 1 = overrelaxation.
+template <int KIND, int MU, int VEC, int OFF>
+__device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st, const int h0) {
     const int p = P.parity;
-    const int sy = Nh, sz = Ns * Nh, stt = Ns * Ns * Nh;     // element strides of x2, x3, t
-    Site st;
-    st.off = (p + x2 + x3 + t) & 1;                   // x1 = 2h + off for the links of this thread
-    st.e0 = ((t * Ns + x3) * Ns + x2) * Nh + h0;
-    st.dp[0] = (t == Nt - 1) ? -(Nt - 1) * stt : stt;   st.dm[0] = (t == 0) ? (Nt - 1) * stt : -stt;
-    st.dp[1] = 0;                                       st.dm[1] = 0;
-    st.dp[2] = (x2 == Ns - 1) ? -(Ns - 1) * sy : sy;    st.dm[2] = (x2 == 0) ? (Ns - 1) * sy : -sy;
-    st.dp[3] = (x3 == Ns - 1) ? -(Ns - 1) * sz : sz;    st.dm[3] = (x3 == 0) ? (Ns - 1) * sz : -sz;
-    st.dxp = (h0 + VEC >= Nh) ? VEC - Nh : VEC;
-    st.dxm = (h0 == 0) ? Nh - 1 : -1;
-
     float Sx[VEC], Sy[VEC];
 #pragma unroll
     for (int i = 0; i < VEC; ++i) { Sx[i] = 0.0f; Sy[i] = 0.0f; }
-    staple_pair<MU, (MU + 1) & 3, VEC>(P.th, P.Vh, p, st, Sx, Sy);
-    staple_pair<MU, (MU + 2) & 3, VEC>(P.th, P.Vh, p, st, Sx, Sy);
-    staple_pair<MU, (MU + 3) & 3, VEC>(P.th, P.Vh, p, st, Sx, Sy);
+    staple_pair<MU, (MU + 1) & 3, VEC, OFF>(P.th, P.Vh, p, st, Sx, Sy);
+    staple_pair<MU, (MU + 2) & 3, VEC, OFF>(P.th, P.Vh, p, st, Sx, Sy);
+    staple_pair<MU, (MU + 3) & 3, VEC, OFF>(P.th, P.Vh, p, st, Sx, Sy);
 
     int* own = P.th + ((MU * 2 + p) * P.Vh + st.e0);
     int out[VEC];
@@ -182,6 +162,41 @@ __global__ void __launch_bounds__(256) k_update(const UpdateArgs P) {
     if (VEC == 4) *reinterpret_cast<int4*>(own) = make_int4(out[0], out[1 % VEC], out[2 % VEC], out[3 % VEC]);
     else if (VEC == 2) *reinterpret_cast<int2*>(own) = make_int2(out[0], out[1 % VEC]);
     else own[0] = out[0];
+}
+
+
+// Block (Nh/VEC, BYH, 2 BZ); grid (Ns/2/BYH, Ns/BZ, n_t) with n_t = Nt, or Nt*(d-1)/d active time layers for
+// a masked spatial direction.  The x2 rows are taken in pairs (2j, 2j+1): threads with threadIdx.z < BZ
+// take the row of the pair whose offset bit is 0, the others the row whose offset bit is 1, so the offset
+// bit is uniform over a warp whenever (Nh/VEC) BYH BZ is a multiple of 32 (any Ns that is a multiple of
+// 16; smaller lattices still compute the same thing, with both branches issued).
+template <int KIND, int MU, int VEC>
+__global__ void __launch_bounds__(256) k_update(const UpdateArgs P) {
+    const int Ns = P.Ns, Nh = P.Nh, Nt = P.Nt;
+    const int h0 = threadIdx.x * VEC;
+    const int bz = blockDim.z >> 1;
+    const int sel = threadIdx.z >= bz ? 1 : 0;
+    const int x3 = blockIdx.y * bz + (threadIdx.z - sel * bz);
+    int t = blockIdx.z;
+    if (MU != 0 && P.slab_d > 0) {                    // enumerate only the non-frozen layers
+        const int dm = P.slab_d - 1;
+        const int s = t / dm;
+        t = s * P.slab_d + 1 + (t - s * dm);
+    }
+    const int p = P.parity;
+    const int x2 = 2 * (blockIdx.x * blockDim.y + threadIdx.y) + ((sel + p + x3 + t) & 1);
+    const int sy = Nh, sz = Ns * Nh, stt = Ns * Ns * Nh;     // element strides of x2, x3, t
+    Site st;
+    st.off = sel;                                     // = (p + x2 + x3 + t) & 1: x1 = 2h + off for the links of this thread
+    st.e0 = ((t * Ns + x3) * Ns + x2) * Nh + h0;
+    st.dp[0] = (t == Nt - 1) ? -(Nt - 1) * stt : stt;   st.dm[0] = (t == 0) ? (Nt - 1) * stt : -stt;
+    st.dp[1] = 0;                                       st.dm[1] = 0;
+    st.dp[2] = (x2 == Ns - 1) ? -(Ns - 1) * sy : sy;    st.dm[2] = (x2 == 0) ? (Ns - 1) * sy : -sy;
+    st.dp[3] = (x3 == Ns - 1) ? -(Ns - 1) * sz : sz;    st.dm[3] = (x3 == 0) ? (Ns - 1) * sz : -sz;
+    st.dxp = (h0 + VEC >= Nh) ? VEC - Nh : VEC;
+    st.dxm = (h0 == 0) ? Nh - 1 : -1;
+    if (sel) update_links<KIND, MU, VEC, 1>(P, st, h0);
+    else update_links<KIND, MU, VEC, 0>(P, st, h0);
 }
 
 }  // namespace ulk
