@@ -218,15 +218,21 @@ int flush(ul_ctx* c) {
     a.g = geom(c); a.d = c->d; a.n_slab = c->n_slab; a.r_max = c->r_max; a.n_fp = c->n_fp; a.nk = c->n_pending;
     a.U = wsp<double2>(c, c->ws.U); a.Ot = wsp<float>(c, c->ws.Ot); a.fps = wsp<int>(c, c->ws.fps);
     a.A = wsp<double2>(c, c->ws.A2); a.B = wsp<double2>(c, c->ws.B2);
+#define UL_ACC_LAUNCH(KB, FIELD)                                                                     \
+    do {                                                                                            \
+        if (a.nk == KB) ulk::k_accumulate<KB, FIELD, true><<<nb, 256, 0, c->stream>>>(a);           \
+        else ulk::k_accumulate<KB, FIELD, false><<<nb, 256, 0, c->stream>>>(a);                     \
+    } while (0)
     if (c->n_fp > 0) {
-        if (a.nk == 1) ulk::k_accumulate<1, true><<<nb, 256, 0, c->stream>>>(a);
-        else if (a.nk <= 4) ulk::k_accumulate<4, true><<<nb, 256, 0, c->stream>>>(a);
-        else ulk::k_accumulate<KBATCH, true><<<nb, 256, 0, c->stream>>>(a);
+        if (a.nk == 1) UL_ACC_LAUNCH(1, true);
+        else if (a.nk <= 4) UL_ACC_LAUNCH(4, true);
+        else UL_ACC_LAUNCH(KBATCH, true);
     } else {
-        if (a.nk == 1) ulk::k_accumulate<1, false><<<nb, 256, 0, c->stream>>>(a);
-        else if (a.nk <= 4) ulk::k_accumulate<4, false><<<nb, 256, 0, c->stream>>>(a);
-        else ulk::k_accumulate<KBATCH, false><<<nb, 256, 0, c->stream>>>(a);
+        if (a.nk == 1) UL_ACC_LAUNCH(1, false);
+        else if (a.nk <= 4) UL_ACC_LAUNCH(4, false);
+        else UL_ACC_LAUNCH(KBATCH, false);
     }
+#undef UL_ACC_LAUNCH
     UL_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->n_pending = 0;
@@ -292,7 +298,10 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     *h = nullptr;
     if (Ns < 2 || Nt < 2 || (Ns & 1) || (Nt & 1) || !(beta >= 0.0)) return fail(nullptr, UL_EINVAL, "need even Ns, Nt >= 2 and beta >= 0");
     const int Nh = Ns / 2;
-    const int vec = (Nh % 4 == 0) ? 4 : ((Nh % 2 == 0) ? 2 : 1);
+    int vec = (Nh % 4 == 0) ? 4 : ((Nh % 2 == 0) ? 2 : 1);
+#ifdef UL_DBG_VEC
+    if (vec > UL_DBG_VEC) vec = UL_DBG_VEC;
+#endif
     if (Nh / vec > 128 || 4.0 * (double)Ns * Ns * Ns * Nt >= 2147483648.0) return fail(nullptr, UL_EINVAL, "lattice too large for this build");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(nullptr, UL_ECUDA, "no CUDA device");

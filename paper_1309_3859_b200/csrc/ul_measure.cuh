@@ -286,10 +286,16 @@ struct AccumArgs {
 // writes it back once: 32/nk bytes of accumulator traffic per entry and sub-update instead of 32.
 // The accumulators are streamed (ld.cs / st.cs, RB entries in flight per thread); the U tables, which every
 // site re-reads 6 r_max times, stay in L1/L2.
-constexpr int ACC_RB = 4;
+#ifndef UL_ACC_RB
+#define UL_ACC_RB 4
+#endif
+#ifndef UL_ACC_MINB
+#define UL_ACC_MINB 1
+#endif
+constexpr int ACC_RB = UL_ACC_RB;
 
-template <int KB, bool FIELD>
-__global__ void __launch_bounds__(256) k_accumulate(const AccumArgs P) {
+template <int KB, bool FIELD, bool FULL>
+__global__ void __launch_bounds__(256, UL_ACC_MINB) k_accumulate(const AccumArgs P) {
     const Geom& g = P.g;
     const long long n = (long long)P.n_slab * g.Vs;
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -308,7 +314,7 @@ __global__ void __launch_bounds__(256) k_accumulate(const AccumArgs P) {
     double2 u0[KB];
 #pragma unroll
     for (int k = 0; k < KB; ++k)
-        if (k < P.nk) u0[k] = Us[k * n + xs];
+        if (FULL || k < P.nk) u0[k] = Us[k * n + xs];
 #pragma unroll
     for (int mu = 1; mu <= 3; ++mu) {
         const int nu = 1 + (mu % 3), rho = 1 + ((mu + 1) % 3);
@@ -324,18 +330,20 @@ __global__ void __launch_bounds__(256) k_accumulate(const AccumArgs P) {
                 if (r > P.r_max) break;
                 // T^(d)(x,s,r mu) = U(x + r mu) conj(U(x))  (Eqs. 22, 25)
                 const int ys = xs + (wrapc(x[mu] + r, Ns) - x[mu]) * stride[mu];         // r <= Ns/2
-                double2 T[KB];
+                double2 T[KB], v[KB];
+#pragma unroll
+                for (int k = 0; k < KB; ++k)                       // all loads of this entry in flight before the first use
+                    if (FULL || k < P.nk) v[k] = Us[k * n + ys];
 #pragma unroll
                 for (int k = 0; k < KB; ++k)
-                    if (k < P.nk) {
-                        const double2 v = Us[k * n + ys];
+                    if (FULL || k < P.nk) {
                         if (FIELD) {
-                            T[k].x = fma(v.x, u0[k].x, v.y * u0[k].y);
-                            T[k].y = fma(v.y, u0[k].x, -(v.x * u0[k].y));
+                            T[k].x = fma(v[k].x, u0[k].x, v[k].y * u0[k].y);
+                            T[k].y = fma(v[k].y, u0[k].x, -(v[k].x * u0[k].y));
                             a[i].x += T[k].x; a[i].y += T[k].y;
                         } else {                                   // the same term folded into the sum: 4 DFMA instead of 6 ops
-                            a[i].x = fma(v.y, u0[k].y, fma(v.x, u0[k].x, a[i].x));
-                            a[i].y = fma(-v.x, u0[k].y, fma(v.y, u0[k].x, a[i].y));
+                            a[i].x = fma(v[k].y, u0[k].y, fma(v[k].x, u0[k].x, a[i].x));
+                            a[i].y = fma(-v[k].x, u0[k].y, fma(v[k].y, u0[k].x, a[i].y));
                         }
                     }
                 __stcs(Ap + i * stepA, a[i]);
@@ -358,7 +366,7 @@ __global__ void __launch_bounds__(256) k_accumulate(const AccumArgs P) {
                             double2 bc = __ldcs(P.B + b0), bs = __ldcs(P.B + b0 + g.Vs);
 #pragma unroll
                             for (int k = 0; k < KB; ++k)
-                                if (k < P.nk) {
+                                if (FULL || k < P.nk) {
                                     const float* Otk = P.Ot + (long long)k * 12 * n;
                                     const double Oc = (double)Otk[(long long)(2 * o) * n + zs];
                                     const double Os = (double)(sgn * Otk[(long long)(2 * o + 1) * n + zs]);

@@ -96,19 +96,22 @@ __device__ __forceinline__ T pick(const T v[VEC], int j) {        // v[j] withou
     return r;
 }
 
-// The update of the VEC links of one thread, compiled separately for the two values of the row's offset
-// bit OFF (x1 = 2h + OFF) so that the x1-shifted neighbour rows are selected by register naming at compile
-// time instead of predicated moves.  KIND 0 = heatbath, 1 = overrelaxation.
-template <int KIND, int MU, int VEC, int OFF>
-__device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st, const int h0) {
-    const int p = P.parity;
-    float Sx[VEC], Sy[VEC];
+// The staple sums of the VEC links of one thread, compiled separately for the two values of the row's
+// offset bit OFF (x1 = 2h + OFF) so that the x1-shifted neighbour rows are selected by register naming at
+// compile time instead of predicated moves.
+template <int MU, int VEC, int OFF>
+__device__ __forceinline__ void gather_staples(const UpdateArgs& P, const Site& st, float Sx[VEC], float Sy[VEC]) {
 #pragma unroll
     for (int i = 0; i < VEC; ++i) { Sx[i] = 0.0f; Sy[i] = 0.0f; }
-    staple_pair<MU, (MU + 1) & 3, VEC, OFF>(P.th, P.Vh, p, st, Sx, Sy);
-    staple_pair<MU, (MU + 2) & 3, VEC, OFF>(P.th, P.Vh, p, st, Sx, Sy);
-    staple_pair<MU, (MU + 3) & 3, VEC, OFF>(P.th, P.Vh, p, st, Sx, Sy);
+    staple_pair<MU, (MU + 1) & 3, VEC, OFF>(P.th, P.Vh, P.parity, st, Sx, Sy);
+    staple_pair<MU, (MU + 2) & 3, VEC, OFF>(P.th, P.Vh, P.parity, st, Sx, Sy);
+    staple_pair<MU, (MU + 3) & 3, VEC, OFF>(P.th, P.Vh, P.parity, st, Sx, Sy);
+}
 
+// The update proper from the staple sums.  KIND 0 = heatbath, 1 = overrelaxation.
+template <int KIND, int MU, int VEC>
+__device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st, const int h0, float Sx[VEC], float Sy[VEC]) {
+    const int p = P.parity;
     int* own = P.th + ((MU * 2 + p) * P.Vh + st.e0);
     int out[VEC];
     if (KIND == 1) {
@@ -170,8 +173,14 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
 // take the row of the pair whose offset bit is 0, the others the row whose offset bit is 1, so the offset
 // bit is uniform over a warp whenever (Nh/VEC) BYH BZ is a multiple of 32 (any Ns that is a multiple of
 // 16; smaller lattices still compute the same thing, with both branches issued).
+#ifndef UL_HB_MINB
+#define UL_HB_MINB 4
+#endif
+#ifndef UL_OR_MINB
+#define UL_OR_MINB 0   // 0 = unspecified
+#endif
 template <int KIND, int MU, int VEC>
-__global__ void __launch_bounds__(256) k_update(const UpdateArgs P) {
+__global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_update(const UpdateArgs P) {
     const int Ns = P.Ns, Nh = P.Nh, Nt = P.Nt;
     const int h0 = threadIdx.x * VEC;
     const int bz = blockDim.z >> 1;
@@ -195,8 +204,17 @@ __global__ void __launch_bounds__(256) k_update(const UpdateArgs P) {
     st.dp[3] = (x3 == Ns - 1) ? -(Ns - 1) * sz : sz;    st.dm[3] = (x3 == 0) ? (Ns - 1) * sz : -sz;
     st.dxp = (h0 + VEC >= Nh) ? VEC - Nh : VEC;
     st.dxm = (h0 == 0) ? Nh - 1 : -1;
-    if (sel) update_links<KIND, MU, VEC, 1>(P, st, h0);
-    else update_links<KIND, MU, VEC, 0>(P, st, h0);
+    float Sx[VEC], Sy[VEC];
+    if (KIND == 1) {
+        // overrelaxation: the short tail is compiled into both branches (56 registers, 4 blocks per SM)
+        if (sel) { gather_staples<MU, VEC, 1>(P, st, Sx, Sy); update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy); }
+        else { gather_staples<MU, VEC, 0>(P, st, Sx, Sy); update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy); }
+    } else {
+        // heatbath: one copy of the sampler after the branch keeps it at 64 registers (4 blocks per SM)
+        if (sel) gather_staples<MU, VEC, 1>(P, st, Sx, Sy);
+        else gather_staples<MU, VEC, 0>(P, st, Sx, Sy);
+        update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy);
+    }
 }
 
 }  // namespace ulk
