@@ -83,6 +83,7 @@ struct ul_ctx {
     int d = 0, r_max = 0, n_fp = 0, n_slab = 0, d_out = 0, n_outer = 0;
     long long n_acc = 0;
     int n_pending = 0;       // configurations tabulated but not yet added to the accumulators
+    bool acc_fresh = true;   // the inner sums A2, B2 hold nothing yet: the next pass writes instead of adding
     Workspace ws;
     // last result
     bool have = false;
@@ -197,9 +198,10 @@ int open_measurement(ul_ctx* c, int d_in, int d_out, int r_max, const int* fps, 
     c->n_slab = c->Nt / d_in; c->n_outer = d_out > 0 ? c->Nt / d_out : 0;
     c->n_acc = 0;
     c->n_pending = 0;
+    c->acc_fresh = true;
     c->have = false;
     if (n_fp > 0) UL_CUDA(c, cudaMemcpyAsync(c->work + w.fps, fps, sizeof(int) * 3 * (size_t)n_fp, cudaMemcpyHostToDevice, c->stream));
-    UL_CUDA(c, cudaMemsetAsync(c->work + w.A2, 0, w.partial - w.A2, c->stream));           // A2, B2, A4, B4
+    if (w.partial > w.A4) UL_CUDA(c, cudaMemsetAsync(c->work + w.A4, 0, w.partial - w.A4, c->stream));   // A4, B4 (A2, B2: first pass writes)
     UL_CUDA(c, cudaMemsetAsync(c->work + w.result, 0, w.total - w.result, c->stream));
     if (n_fp > 0) UL_CUDA(c, cudaStreamSynchronize(c->stream));                            // fps is a caller-owned host buffer
     c->open = true;
@@ -215,7 +217,7 @@ int flush(ul_ctx* c) {
     const long long n = (long long)c->n_slab * c->Vs;
     const int nb = (int)((n + 255) / 256);
     ulk::AccumArgs a;
-    a.g = geom(c); a.d = c->d; a.n_slab = c->n_slab; a.r_max = c->r_max; a.n_fp = c->n_fp; a.nk = c->n_pending;
+    a.g = geom(c); a.d = c->d; a.n_slab = c->n_slab; a.r_max = c->r_max; a.n_fp = c->n_fp; a.nk = c->n_pending; a.first = c->acc_fresh ? 1 : 0;
     a.U = wsp<double2>(c, c->ws.U); a.Ot = wsp<float>(c, c->ws.Ot); a.fps = wsp<int>(c, c->ws.fps);
     a.A = wsp<double2>(c, c->ws.A2); a.B = wsp<double2>(c, c->ws.B2);
 #define UL_ACC_LAUNCH(KB, FIELD)                                                                     \
@@ -236,6 +238,7 @@ int flush(ul_ctx* c) {
     UL_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->n_pending = 0;
+    c->acc_fresh = false;
     return UL_OK;
 }
 
@@ -248,9 +251,10 @@ int accumulate(ul_ctx* c) {
     t.U = wsp<double2>(c, c->ws.U) + (size_t)c->n_pending * n;
     t.Ot = c->n_fp > 0 ? wsp<float>(c, c->ws.Ot) + (size_t)c->n_pending * 12 * n : nullptr;
     t.partial = wsp<double>(c, c->ws.partial);
-    const int tb = (int)((n + 255) / 256) < TBLK ? (int)((n + 255) / 256) : TBLK;
-    ulk::k_slab_tables<<<tb, 256, 0, c->stream>>>(t);
-    ulk::k_sum_partials<<<12, 256, 0, c->stream>>>(t.partial, tb, res_colsum(c), 1.0, 1);
+    const int gx = (c->Ns * c->Ns + 255) / 256, rows = c->n_slab * c->Ns;
+    const int gy = rows < TBLK / gx ? rows : (TBLK / gx > 0 ? TBLK / gx : 1);
+    ulk::k_slab_tables<<<dim3(gx, gy), 256, 0, c->stream>>>(t);
+    ulk::k_sum_partials<<<12, 256, 0, c->stream>>>(t.partial, gx * gy, res_colsum(c), 1.0, 1);
     UL_CUDA(c, cudaGetLastError());
     c->launches += 2;
     c->n_acc += 1;
@@ -498,7 +502,7 @@ int ul_multilevel2(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, int r_ma
     const long long total = 3LL * r_max * c->n_outer * c->Vs;
     for (int J = 0; J < n_out; ++J) {
         for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d_out); if (rc) return rc; }
-        if (J > 0) UL_CUDA(c, cudaMemsetAsync(c->work + w.A2, 0, w.A4 - w.A2, c->stream));   // A2, B2 <- 0
+        c->acc_fresh = true;                                                                 // A2, B2 <- 0
         for (int j = 0; j < n_in; ++j) {
             for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d_in); if (rc) return rc; }
             rc = accumulate(c);
@@ -515,8 +519,11 @@ int ul_multilevel2(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, int r_ma
 
 int ul_plaquette(ul_ctx* c, double* out) {
     if (!c || !out) return fail(c, UL_EINVAL, "null pointer");
-    ulk::k_plaquette<<<NBLK, 256, 0, c->stream>>>(geom(c), c->th, c->scratch);
-    ulk::k_sum_partials<<<2, 256, 0, c->stream>>>(c->scratch, NBLK, c->scratch + 2 * NBLK, 1.0 / (3.0 * (double)c->V), 0);
+    const int gx = (c->Ns * c->Ns + 255) / 256, rows = c->Nt * c->Ns;
+    const int gy = rows < NBLK / gx ? rows : (NBLK / gx > 0 ? NBLK / gx : 1);
+    if (gx * gy > NBLK) return fail(c, UL_EINVAL, "lattice too large for this build");
+    ulk::k_plaquette<<<dim3(gx, gy), 256, 0, c->stream>>>(geom(c), c->th, c->scratch);
+    ulk::k_sum_partials<<<2, 256, 0, c->stream>>>(c->scratch, gx * gy, c->scratch + 2 * NBLK, 1.0 / (3.0 * (double)c->V), 0);
     UL_CUDA(c, cudaGetLastError());
     c->launches += 2;
     double v[2];

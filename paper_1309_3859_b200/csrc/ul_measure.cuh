@@ -158,16 +158,21 @@ __device__ __forceinline__ void site_plaquettes(const Geom& g, const int* __rest
 }
 
 // row a11: partial[0*nblk + b] = sum of cos over time-like plaquettes, [1*nblk + b] space-like
+// Grid (ceil(Ns^2/256), rows): a thread keeps its (x1, x2) and walks over the (t, x3) rows, so the only
+// divisions are one per thread and one per row (all 32-bit).
 __global__ void __launch_bounds__(256) k_plaquette(Geom g, const int* __restrict__ th, double* __restrict__ partial) {
     __shared__ double sm[2 * 32];
+    const unsigned Ns = (unsigned)g.Ns;
+    const unsigned i2 = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool in = i2 < Ns * Ns;
+    int x[4];
+    x[2] = (int)(i2 / Ns);
+    x[1] = (int)(i2 - (unsigned)x[2] * Ns);
     double v[2] = {0.0, 0.0};
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.V; i += (long long)gridDim.x * blockDim.x) {
-        long long s = i;
-        int x[4];
-        x[1] = (int)(s % g.Ns); s /= g.Ns;
-        x[2] = (int)(s % g.Ns); s /= g.Ns;
-        x[3] = (int)(s % g.Ns); s /= g.Ns;
-        x[0] = (int)s;
+    for (unsigned row = blockIdx.y; row < (unsigned)g.Nt * Ns; row += gridDim.y) {
+        x[0] = (int)(row / Ns);
+        x[3] = (int)(row - (unsigned)x[0] * Ns);
+        if (!in) continue;
         int pl[6], th0;
         site_plaquettes(g, th, x, pl, th0);
         float ct = 0.0f, cs = 0.0f;
@@ -181,16 +186,18 @@ __global__ void __launch_bounds__(256) k_plaquette(Geom g, const int* __restrict
         v[1] += (double)cs;
     }
     block_sum<2>(v, sm);
-    if (threadIdx.x == 0) { partial[blockIdx.x] = v[0]; partial[gridDim.x + blockIdx.x] = v[1]; }
+    const unsigned nblk = gridDim.x * gridDim.y, blk = blockIdx.y * gridDim.x + blockIdx.x;
+    if (threadIdx.x == 0) { partial[blk] = v[0]; partial[nblk + blk] = v[1]; }
 }
 
 // ---------------------------------------------------------------- per-configuration slab tables
 // U[s][xs]  = exp(i sum_{t in slab s} theta_0(xs,t)) in fp64: the angle sum is a wrapping integer add
-//             (exact mod 2 pi) and sincospi of I 2^-31 is exact in its argument, so U is good to 1 ulp and
+//             (exact mod 2 pi), reduced in integers and expanded in fp64 (sincos_bt_f64), so U is good to 1 ulp and
 //             every T^(d)(x,s,r mu) = U(x + r mu) conj(U(x)) (Eqs. 22, 25) is one fp64 complex product.
 // Ot[o][kind][s][xs] = sum_{t in slab s} O(theta_P(o)(xs,t)),  O = 1 - cos (kind 0), sin (kind 1); stored
 //             only when field points are measured (Ot != nullptr).
-// partial[col*gridDim.x + b] = block partial of the column sums of O (vacuum expectation values).
+// partial[col*nblk + b] = block partial of the column sums of O (vacuum expectation values).
+// Grid (ceil(Ns^2/256), rows): a thread keeps its (x1, x2) and walks over the (s, x3) rows.
 struct TableArgs {
     Geom g;
     const int* th;
@@ -203,16 +210,20 @@ __global__ void __launch_bounds__(256) k_slab_tables(const TableArgs P) {
     __shared__ double sm[12 * 32];
     const Geom& g = P.g;
     const long long n = (long long)P.n_slab * g.Vs;
-    double v[12];
+    const unsigned Ns = (unsigned)g.Ns;
+    const unsigned i2 = blockIdx.x * blockDim.x + threadIdx.x;                 // (x1, x2) of this thread
+    const bool in = i2 < Ns * Ns;
+    int x[4];
+    x[2] = (int)(i2 / Ns);
+    x[1] = (int)(i2 - (unsigned)x[2] * Ns);
+    float vf[12];                                   // per-thread column sums: a few terms of magnitude <= 2 each, then fp64
 #pragma unroll
-    for (int o = 0; o < 12; ++o) v[o] = 0.0;
-    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (long long)gridDim.x * blockDim.x) {
-        const int s = (int)(idx / g.Vs);
-        long long r = idx - (long long)s * g.Vs;
-        int x[4];
-        x[1] = (int)(r % g.Ns); r /= g.Ns;
-        x[2] = (int)(r % g.Ns); r /= g.Ns;
-        x[3] = (int)r;
+    for (int o = 0; o < 12; ++o) vf[o] = 0.0f;
+    for (unsigned row = blockIdx.y; row < (unsigned)P.n_slab * Ns; row += gridDim.y) {   // rows (s, x3): 32-bit divisions only
+        const int s = (int)(row / Ns);
+        x[3] = (int)(row - (unsigned)s * Ns);
+        if (!in) continue;
+        const long long idx = (long long)row * (Ns * Ns) + i2;
         unsigned acc = 0u;
         float o_c[6], o_s[6];
 #pragma unroll
@@ -231,7 +242,7 @@ __global__ void __launch_bounds__(256) k_slab_tables(const TableArgs P) {
             }
         }
         double us, uc;
-        sincospi((double)(int)acc * (1.0 / 2147483648.0), &us, &uc);
+        ulm::sincos_bt_f64((int)acc, uc, us);
         P.U[idx] = make_double2(uc, us);
 #pragma unroll
         for (int o = 0; o < 6; ++o) {
@@ -239,14 +250,18 @@ __global__ void __launch_bounds__(256) k_slab_tables(const TableArgs P) {
                 P.Ot[(long long)(2 * o) * n + idx] = o_c[o];
                 P.Ot[(long long)(2 * o + 1) * n + idx] = o_s[o];
             }
-            v[2 * o] += (double)o_c[o];
-            v[2 * o + 1] += (double)o_s[o];
+            vf[2 * o] += o_c[o];
+            vf[2 * o + 1] += o_s[o];
         }
     }
+    double v[12];
+#pragma unroll
+    for (int o = 0; o < 12; ++o) v[o] = (double)vf[o];
     block_sum<12>(v, sm);
     if (threadIdx.x == 0) {
+        const unsigned nblk = gridDim.x * gridDim.y, blk = blockIdx.y * gridDim.x + blockIdx.x;
 #pragma unroll
-        for (int o = 0; o < 12; ++o) P.partial[(long long)o * gridDim.x + blockIdx.x] = v[o];
+        for (int o = 0; o < 12; ++o) P.partial[(long long)o * nblk + blk] = v[o];
     }
 }
 
@@ -273,6 +288,7 @@ struct AccumArgs {
     Geom g;
     int d, n_slab, r_max, n_fp;
     int nk;               // configurations in this batch (1..KB), slots 0..nk-1 in sub-update order
+    int first;            // 1: first pass of a measurement: the sums start from zero (no read, no memset)
     const double2* U;     // [nk][n_slab*Vs]
     const float* Ot;      // [nk][12][n_slab*Vs]   (n_fp > 0 only)
     const int* fps;       // device int[n_fp][3]
@@ -323,7 +339,7 @@ __global__ void __launch_bounds__(256, UL_ACC_MINB) k_accumulate(const AccumArgs
             double2 a[ACC_RB];
 #pragma unroll
             for (int i = 0; i < ACC_RB; ++i)
-                if (r0 + i <= P.r_max) a[i] = __ldcs(Ap + i * stepA);
+                if (r0 + i <= P.r_max) a[i] = P.first ? make_double2(0.0, 0.0) : __ldcs(Ap + i * stepA);
 #pragma unroll
             for (int i = 0; i < ACC_RB; ++i) {
                 const int r = r0 + i;
@@ -363,7 +379,8 @@ __global__ void __launch_bounds__(256, UL_ACC_MINB) k_accumulate(const AccumArgs
                             comp_dirs(mu, comp, pa, pb);
                             orient_of(pa, pb, o, sgn);
                             const long long b0 = (b_base * 12 + 2 * comp) * g.Vs + xs;
-                            double2 bc = __ldcs(P.B + b0), bs = __ldcs(P.B + b0 + g.Vs);
+                            double2 bc = make_double2(0.0, 0.0), bs = make_double2(0.0, 0.0);
+                            if (!P.first) { bc = __ldcs(P.B + b0); bs = __ldcs(P.B + b0 + g.Vs); }
 #pragma unroll
                             for (int k = 0; k < KB; ++k)
                                 if (FULL || k < P.nk) {
