@@ -476,3 +476,133 @@ def test_full_size_64_sampled_against_oracle(ul, ulo):
         # hot start: links with tiny staples (k < 0.05, P ~ 3e-4) amplify rounding; flips are rare
         assert frac < 1e-4, (kind, parity, mu, d, frac, diff.max())
         assert (diff > 1e-3).sum() / (diff.size / 8) < 1e-5
+
+
+def test_full_size_64_measurement_against_oracle(ul, ulo):
+    """64^4, d = 2, r_max = 16 (the bench's measurement launch configuration): the frozen-configuration
+    estimator equals the naive Polyakov-loop correlator (Eq. 23) that the oracle computes
+    straight from Eq. 15; the batched pass over 8 configurations (here 8 copies of the same one, fed
+    through ul_accumulate) gives the same slab products; vacuum values against the oracle's plaquette."""
+    Ns = Nt = 64
+    R = 16
+    g = ul.Lattice(Ns, Nt, 0.98, 5, workspace_bytes=ul.workspace_bytes(Ns, Nt, 2, 0, R, 0))
+    g.sweep(1, 2)                                                   # a configuration with some structure
+    o = ulo.Oracle(Ns, Nt, 0.98, 5)
+    o.set_links(g.get_links())
+    want, _ = o.polyakov_naive(R)
+    g.multilevel(2, 0, R)                                           # accumulate<1>, first pass
+    c1, _, v1 = g.read_correlators()
+    N = 3 * Ns ** 3
+    for got, ref in ((c1.real, want.real), (c1.imag, want.imag)):
+        ok, worst = rel_ok(got, ref, N)
+        assert ok, worst
+    plaq = o.plaquette()
+    # vacuum channels 0, 2, 4 are 1 - cos of the time-like plaquettes (0,mu),(0,nu),(0,rho) averaged over the frames
+    assert abs((1.0 - v1[[0, 2, 4]]).mean() - plaq[1]) < 1e-6 and abs((1.0 - v1[[6, 8, 10]]).mean() - plaq[2]) < 1e-6
+    g.measure_begin(2, R)
+    for _ in range(8):
+        g.accumulate()                                              # one full batch: accumulate<8>
+    g.accumulate()                                                  # and a ragged second pass (read-modify-write)
+    g.measure_end()
+    c9, _, v9 = g.read_correlators()
+    assert np.abs(c9 - c1).max() < 1e-12 and np.abs(v9 - v1).max() < 1e-12
+
+
+# ----------------------------------------------------------------------------- BJ configs 3 and 4
+def _gpu_thermalised(ul, ulo, Ns, Nt, beta, seed, cold, n_sweeps, n_or):
+    """Configurations too long for the oracle to thermalise: the GPU does the sweeps, the oracle takes
+    the result over; every comparison after that starts from identical links."""
+    g = ul.Lattice(Ns, Nt, beta, seed)
+    if cold:
+        g.init(0)
+    for _ in range(n_sweeps):
+        g.sweep(1, n_or)
+    o = ulo.Oracle(Ns, Nt, beta, seed)
+    o.set_links(g.get_links())
+    o.set_counter(g.get_counter())
+    g.set_links(o.get_links())                                      # both sides hold the fp32-rounded angles
+    return g, o
+
+
+def _whole_hb_sweep(g, o, ulo, beta):
+    """One whole heatbath sweep on both sides (GPU: ul_sweep; oracle: its 8 sub-steps, pinned equal to
+    ulo_sweep, with a snapshot before each so that a miss can be classified by the staple magnitude k its
+    link had WHEN it was updated).  BJ's criterion: every link within 2e-5 rad except accept/reject flips
+    (and what they drag along later in the sweep), < 1e-5 of links; links updated at k < 0.05
+    (d alpha = dS / k) are the ill-conditioned class of P1, counted apart."""
+    Ns, Nt = g.Ns, g.Nt
+    snaps = []
+    for parity in range(2):
+        for mu in range(4):
+            snaps.append(o.get_links())
+            o.substep(0, parity, mu, 0)
+    o.set_counter(o.get_counter() + 1)
+    g.sweep(1, 0)
+    assert g.get_counter() == o.get_counter()
+    diff = wrapdiff(g.get_links(), o.get_links())
+    bad = np.argwhere(diff > TOL)
+    ob = ulo.Oracle(Ns, Nt, beta, 1)
+    n_ill = n_other = 0
+    for idx in bad:
+        mu, parity = int(idx[0]), int(idx[1:].sum()) & 1
+        ob.set_links(snaps[parity * 4 + mu])
+        k, _ = ob.staple(mu, int(np.ravel_multi_index(tuple(idx[1:]), diff.shape[1:])))
+        if k < 0.05:
+            n_ill += 1
+        else:
+            n_other += 1
+    assert n_other <= max(1, 1e-5 * diff.size), (n_other, n_ill, diff.max())
+    assert n_ill <= 1e-4 * diff.size, (n_other, n_ill, diff.max())
+    assert (diff > 5e-6).mean() < 2e-4                               # and the bulk sits far below the tolerance
+
+
+def test_config3_24x8_thermalised_sweep_and_fields(ul, ulo):
+    """BJ config 3: 24^3 x 8, beta = 1.00, cold start, 500 x (1 HB + 3 OR); then one HB sweep link by link
+    (P1) and the frozen-configuration estimator with r = 1..12, mid-plane and on-axis field points (P2)."""
+    Ns, Nt, R = 24, 8, 12
+    g, o = _gpu_thermalised(ul, ulo, Ns, Nt, 1.00, 3, True, 500, 3)
+    pg, po = g.plaquette(), o.plaquette()
+    assert 0.55 < pg[0] < 0.75                                       # thermalised around the beta = 1 transition region
+    ok, worst = rel_ok(pg, po, 3 * Ns ** 3 * Nt, rms_term=0.5)
+    assert ok, worst
+    fps = [(0, 0, 0), (0, 5, 0), (0, 10, 0), (3, 0, 0)]
+    o.multilevel(2, 0, R, fps)
+    g.multilevel(2, 0, R, fps)
+    co, fo, vo = o.read_correlators()
+    cg, fg, vg = g.read_correlators()
+    assert np.abs(g.read_slab_averages() - o.read_slab_averages()).max() < 1e-5
+    Vs = Ns ** 3
+    for got, want, n in ((cg, co, 3 * Vs), (fg, fo, 3 * Vs * Nt), (vg, vo, 3 * Vs * Nt)):
+        ok, worst = rel_ok(got, want, n)
+        assert ok, worst
+    _whole_hb_sweep(g, o, ulo, 1.00)
+
+
+def test_config4_32x32_two_level_and_sweep(ul, ulo):
+    """BJ config 4: 32^4, beta = 1.00, hot start seed 4, two-level scheme with slab thicknesses 2 and 4,
+    r = 1..16: the combine path on a frozen configuration (sub-update recipe of zero sweeps) against the
+    oracle, the factorisation Eq. 24, and one whole heatbath sweep link by link."""
+    Ns, Nt, R = 32, 32, 16
+    g, o = _gpu_thermalised(ul, ulo, Ns, Nt, 1.00, 4, False, 40, 4)
+    o.set_subupdate(0, 0, 1)
+    g.set_subupdate(0, 0, 1)
+    o.multilevel2(2, 1, 4, 1, R)
+    g.multilevel2(2, 1, 4, 1, R)
+    co, _, vo = o.read_correlators()
+    cg, _, vg = g.read_correlators()
+    assert np.abs(g.read_slab_averages() - o.read_slab_averages()).max() < 1e-5
+    Vs = Ns ** 3
+    for got, want, n in ((cg, co, 3 * Vs), (vg, vo, 3 * Vs * Nt)):
+        ok, worst = rel_ok(got, want, n)
+        assert ok, worst
+    want, _ = o.polyakov_naive(R)                                    # Eq. 23: frozen configuration = naive correlator
+    assert np.abs(cg - want).max() < 1e-9
+    fps = [(0, 0, 0), (0, 3, 0)]
+    o.multilevel2(2, 1, 4, 1, 2, fps)
+    g.multilevel2(2, 1, 4, 1, 2, fps)
+    fo, fg = o.read_correlators()[1], g.read_correlators()[1]
+    ok, worst = rel_ok(fg, fo, 3 * Vs * Nt)
+    assert ok, worst
+    g.set_subupdate(1, 3, 1)
+    o.set_subupdate(1, 3, 1)
+    _whole_hb_sweep(g, o, ulo, 1.00)
