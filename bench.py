@@ -5,7 +5,7 @@
 
 One STEP = one pass of the whole hot path over a 64^4 lattice (beta = 0.98, hot start seed 5):
     ul_sweep(1 HB, 4 OR)                      full compound sweep          (rows a2-a5)
-    ul_multilevel(d=2, n_sub, r_max=16)       n_sub x {slab-masked compound sub-update (1 HB + 4 OR)
+    ul_multilevel(d=2, n_sub=8, r_max=16)     n_sub x {slab-masked compound sub-update (1 HB + 4 OR)
                                               + T^(2) accumulation}, slab product, reduction (a6, a7, a10, a13)
     ul_plaquette()                                                          (row a11)
 metric = link updates per second (full + masked updates) over the whole step, inputs resident in HBM.
@@ -117,12 +117,17 @@ def measured_peak_hbm():
 
 
 def ncu_traffic():
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary, or None."""
-    p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    """DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum of its
+    `ncu --set full` capture), from the committed summary profiles/roofline_traffic.txt, or None."""
+    p = os.path.join(ROOT, "profiles", "roofline_traffic.txt")
     try:
-        return float(json.load(open(p))["k_update_or_dram_bytes_per_launch"])
+        for line in open(p):
+            f = line.split()
+            if len(f) >= 2 and f[0] == "k_update_or_dram_bytes_per_launch":
+                return float(f[1])
     except Exception:
-        return None
+        pass
+    return None
 
 
 # ------------------------------------------------------------------------------------------- oracle arm
