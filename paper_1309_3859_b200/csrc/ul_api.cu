@@ -8,6 +8,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -75,6 +76,10 @@ struct ul_ctx {
     float* staging = nullptr;  // canonical device copy for set/get links
     double* scratch = nullptr; // [2*NBLK + 4] plaquette partials and sums
     int* d_bad = nullptr;
+    int4* hb_queue = nullptr; // heatbath straggler queue (library-owned)
+    int* hb_qcount = nullptr;
+    int hb_qblocks = 0;
+    int hb_local_rounds = 2;
     int vec = 1, bx = 1, by = 1, bz = 1;
     int sub_hb = 1, sub_or = 3, sub_k = 1;
     int batch_cap = 0;       // ul_set_accum_batch: 0 = default depth
@@ -153,9 +158,16 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
     a.key0 = (uint32_t)(c->seed & 0xffffffffu); a.key1 = (uint32_t)(c->seed >> 32);
     a.sweep_lo = (uint32_t)(c->sweep & 0xffffffffu); a.sweep_hi = (uint32_t)(c->sweep >> 32);
     const dim3 block(c->bx, c->by, 2 * c->bz), grid(c->Nh / c->by, c->Ns / c->bz, n_t);   // by = x2 row PAIRS per block
+    a.queue = c->hb_queue; a.qcount = c->hb_qcount; a.qblocks = (int)(grid.x * grid.y * grid.z); a.local_rounds = c->hb_local_rounds;
+    if (kind == 0 && cudaMemsetAsync(c->hb_qcount, 0, sizeof(int) * (size_t)a.qblocks, c->stream) != cudaSuccess) return fail(c, UL_ECUDA, "memset straggler counters");
     const cudaError_t e = kind == 0 ? launch_update_mu<0>(c, mu, a, grid, block) : launch_update_mu<1>(c, mu, a, grid, block);
     if (e != cudaSuccess) return fail(c, UL_ECUDA, std::string("k_update launch: ") + cudaGetErrorString(e));
     c->launches += 1;
+    if (kind == 0) {                                  // finish the links the heatbath kernel queued
+        ulk::k_hb_stragglers<<<(a.qblocks * ulk::HB_QSEG + 255) / 256, 256, 0, c->stream>>>(a, mu);
+        if (cudaGetLastError() != cudaSuccess) return fail(c, UL_ECUDA, "k_hb_stragglers launch");
+        c->launches += 1;
+    }
     return UL_OK;
 }
 int one_sweep(ul_ctx* c, int kind, int slab_d) {      // O5: parity outer, direction inner
@@ -337,6 +349,14 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     if (cudaMalloc(&s, sizeof(double) * (2 * NBLK + 4) + 256) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ENOMEM, "cudaMalloc scratch"); }
     c->scratch = (double*)s;
     c->d_bad = (int*)((char*)s + sizeof(double) * (2 * NBLK + 4));
+    c->hb_qblocks = (c->Nh / c->by) * (c->Ns / c->bz) * c->Nt;    // blocks of an unmasked sub-step
+    void* q = nullptr;
+    if (cudaMalloc(&q, (sizeof(int4) * ulk::HB_QSEG + sizeof(int)) * (size_t)c->hb_qblocks) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ENOMEM, "cudaMalloc straggler queue"); }
+    c->hb_queue = (int4*)q;
+    c->hb_qcount = (int*)(c->hb_queue + (size_t)ulk::HB_QSEG * c->hb_qblocks);
+#ifdef UL_DBG_TUNE
+    if (const char* ev = getenv("UL_HB_LOCAL_ROUNDS")) c->hb_local_rounds = atoi(ev);
+#endif
     *h = c;
     const int rc = ul_init(c, 1);
     if (rc) { g_err = c->err; ul_destroy(c); *h = nullptr; }
@@ -367,6 +387,7 @@ int ul_destroy(ul_ctx* c) {
     if (c->own_work && c->work) cudaFree(c->work);
     if (c->staging) cudaFree(c->staging);
     if (c->scratch) cudaFree(c->scratch);
+    if (c->hb_queue) cudaFree(c->hb_queue);
     if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
     delete c;
     return UL_OK;

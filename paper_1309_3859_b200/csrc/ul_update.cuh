@@ -25,7 +25,13 @@ struct UpdateArgs {
     float beta;
     uint32_t key0, key1;  // Philox key = seed
     uint32_t sweep_lo, sweep_hi;
+    int4* queue;          // heatbath stragglers: (element offset, site | tries << 29, Sx, Sy), see k_hb_stragglers
+    int* qcount;          // entries queued per block (zeroed before the launch); segment b = queue[b*HB_QSEG ...]
+    int qblocks;          // number of segments
+    int local_rounds;     // lane-local retry rounds before a link is queued
 };
+
+constexpr int HB_QSEG = 128;   // straggler-queue entries per thread block (expected use ~25 of 1024 links)
 
 // per-thread addressing state
 struct Site {
@@ -159,11 +165,11 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
         const uint32_t site0 = (uint32_t)((st.e0 - h0) * 2 + 2 * h0 + st.off);            // canonical site index
         const uint32_t c3 = ((uint32_t)p << 2) | (uint32_t)MU;                            // tag 0 = heatbath
         float pa[VEC], pq[VEC], pc[VEC], sn[VEC], cs[VEC];
-        uint32_t pend = 0u, neg = 0u, tries = 0u;                                         // tries: 8 bits per link
+        uint32_t pend = 0u, neg = 0u, tries = 0u, zero = 0u;                              // tries: 8 bits per link
 #pragma unroll
         for (int i = 0; i < VEC; ++i) {
             const float k2 = fmaf(Sx[i], Sx[i], Sy[i] * Sy[i]);
-            if (k2 == 0.0f) Sx[i] = 1.0f;                                                 // k = 0: alpha = 0 (O1)
+            if (k2 == 0.0f) { Sx[i] = 1.0f; Sy[i] = 0.0f; zero |= 1u << i; }                // k = 0: alpha = 0 (O1)
             const ulm::HbParams hp = ulm::hb_setup(P.beta * ulm::mufu_sqrt(k2));
             pa[i] = hp.a; pq[i] = hp.q; pc[i] = hp.c0;
             uint32_t w[4];
@@ -173,7 +179,7 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
             pend |= (ok ? 0u : 1u) << i;
             tries |= 1u << (8 * i);
         }
-        while (pend) {
+        auto retry_one = [&]() {                                                          // one more attempt of this lane's first pending link
             const int j = __ffs(pend) - 1;
             ulm::HbParams hp;
             hp.a = pick<float, VEC>(pa, j); hp.q = pick<float, VEC>(pq, j); hp.c0 = pick<float, VEC>(pc, j);
@@ -187,6 +193,41 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
             neg = (neg & ~(1u << j)) | ((w[2] >> 31) << j);
             tries += 1u << (8 * j);
             if (ok || n == 63u) pend &= ~(1u << j);                                       // cap 64: keep the last proposal (O3)
+        };
+        for (int round = 0; round < P.local_rounds && pend; ++round) retry_one();
+        // Links still rejected after the lane-local rounds (a few %) go to this block's segment of the straggler
+        // queue instead of keeping the whole warp looping for its unluckiest lane; k_hb_stragglers finishes
+        // them (same attempt counters, same arithmetic) right after this kernel.  One atomic per warp on the
+        // block's own counter; links that do not fit in the segment are simply finished here.
+        const unsigned wmask = __activemask();
+        const unsigned lanes = __ballot_sync(wmask, pend != 0u);
+        if (lanes) {
+            const int lane = (threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z)) & 31;
+            const int blk = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+            int mine = __popc(pend), incl = mine;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {                                            // inclusive warp prefix sum
+                const int v = __shfl_up_sync(wmask, incl, o);
+                if (lane >= o) incl += v;
+            }
+            const int last = 31 - __clz(wmask);
+            const int total = __shfl_sync(wmask, incl, last);
+            int base = 0;
+            if (lane == last) base = atomicAdd(P.qcount + blk, total);
+            base = __shfl_sync(wmask, base, last);
+            int pos = base + incl - mine;                                                 // slots are handed out contiguously, so every
+#pragma unroll                                                                            // slot below min(count, HB_QSEG) gets written
+            for (int i = 0; i < VEC; ++i)
+                if (((pend >> i) & 1u) && pos < HB_QSEG) {
+                    const uint32_t n = (tries >> (8 * i)) & 0xffu;                        // <= 1 + local_rounds <= 7
+                    P.queue[blk * HB_QSEG + pos] = make_int4((MU * 2 + p) * P.Vh + st.e0 + i, (int)((site0 + 2u * i) | (n << 29)),
+                                                             __float_as_int(((zero >> i) & 1u) ? 0.0f : Sx[i]), __float_as_int(Sy[i]));
+                    ++pos;
+                    pend &= ~(1u << i);
+                } else if ((pend >> i) & 1u) {
+                    ++pos;
+                }
+            while (pend) retry_one();
         }
 #pragma unroll
         for (int i = 0; i < VEC; ++i) out[i] = ulm::hb_finish(Sx[i], Sy[i], sn[i], cs[i], ((neg >> i) & 1u) != 0);
@@ -243,6 +284,34 @@ __global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_up
         if (sel) gather_staples<MU, VEC, 1>(P, st, Sx, Sy);
         else gather_staples<MU, VEC, 0>(P, st, Sx, Sy);
         update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy);
+    }
+}
+
+// Finishes the heatbath links that k_update<0,...> queued: one thread per entry, attempts n = tries, tries+1, ...
+// with the same Philox counters and the same device functions as the main kernel (so the result does not
+// depend on where a link is finished), until accept or the cap of 64 attempts (O3).
+__global__ void __launch_bounds__(256) k_hb_stragglers(const UpdateArgs P, int mu) {
+    const uint32_t c3 = ((uint32_t)P.parity << 2) | (uint32_t)mu;
+    {   // one thread per queue slot: grid = qblocks * HB_QSEG / 256 blocks, most of which leave at once
+        const int e = blockIdx.x * blockDim.x + threadIdx.x;
+        if (e >= P.qblocks * HB_QSEG || (e % HB_QSEG) >= P.qcount[e / HB_QSEG]) return;   // a count above HB_QSEG: the rest was finished in place
+        const int4 q = P.queue[e];
+        const uint32_t site = (uint32_t)q.y & 0x1fffffffu;
+        uint32_t n = (uint32_t)q.y >> 29;
+        float Sx = __int_as_float(q.z);
+        const float Sy = __int_as_float(q.w);
+        const float k2 = fmaf(Sx, Sx, Sy * Sy);
+        if (k2 == 0.0f) Sx = 1.0f;                                                        // k = 0: alpha = 0 (O1); Sy is 0 then
+        const ulm::HbParams hp = ulm::hb_setup(P.beta * ulm::mufu_sqrt(k2));
+        float sn, cs;
+        uint32_t w[4];
+        for (;;) {
+            ulm::philox4x32_10(site, P.sweep_lo, P.sweep_hi, (n << 8) | c3, P.key0, P.key1, w);
+            const bool ok = ulm::hb_attempt(hp, w[0], w[1], sn, cs);
+            if (ok || n == 63u) break;
+            ++n;
+        }
+        P.th[q.x] = ulm::hb_finish(Sx, Sy, sn, cs, (w[2] >> 31) != 0);
     }
 }
 
