@@ -27,6 +27,8 @@ struct ulo_ctx {
     uint64_t seed = 0, sweep = 0;  // sweep = count of HB sweeps issued (S8(c)-O4)
     std::vector<float> th;         // [4][V] canonical, fp32 radians
     int sub_hb = 1, sub_or = 3, sub_k = 1;  // sub-update recipe (DESIGN R5)
+    int alg = 0;                   // 0 = heatbath (north star), 1 = Metropolis (DESIGN R21) for the "n_hb" sweeps
+    double met_delta = PI;         // Metropolis proposal half-width (radians)
     // open single-level measurement
     bool open = false;
     int d = 0, r_max = 0, n_fp = 0, n_slab = 0;
@@ -169,6 +171,20 @@ static void substep(ulo_ctx* c, int kind, int parity, int mu, int slab_d) {
         double theta_new;
         if (kind == 1) {
             theta_new = wrap(2.0 * alpha - TH(c, mu, x));                   // overrelaxation, O2
+        } else if (kind == 2) {
+            // Metropolis ("standard Metropolis algorithm"; DESIGN R21: the paper gives no proposal, so:
+            // one hit, symmetric uniform proposal theta' = theta + delta (2 u1 - 1), accepted with probability
+            // min(1, exp(-dS)) where -dS = beta k [cos(theta' - alpha) - cos(theta - alpha)] (Eq. 6).
+            // Philox tag 3, attempt 0.  A rejected link keeps its stored value bit for bit.
+            const uint32_t ctr[4] = {(uint32_t)x, (uint32_t)(c->sweep & 0xffffffffu), (uint32_t)(c->sweep >> 32), c3_low(3, parity, mu)};
+            uint32_t w[4];
+            ulo_philox4x32_10(ctr, key, w);
+            const double u1 = U_of(w[0]), u2 = U_of(w[1]);
+            const double theta = TH(c, mu, x);
+            const double prop = theta + c->met_delta * (2.0 * u1 - 1.0);
+            const double gain = c->beta * k * (std::cos(prop - alpha) - std::cos(theta - alpha));
+            if (!(u2 <= std::exp(gain))) continue;
+            theta_new = wrap(prop);
         } else {
             const double phi = heatbath_phi(c->beta * k, key, (uint32_t)x, (uint32_t)(c->sweep & 0xffffffffu),
                                             (uint32_t)(c->sweep >> 32), c3_low(0, parity, mu), nullptr);
@@ -180,10 +196,10 @@ static void substep(ulo_ctx* c, int kind, int parity, int mu, int slab_d) {
 static void one_sweep(ulo_ctx* c, int kind, int slab_d) {  // O5: parity outer, direction inner
     for (int parity = 0; parity < 2; ++parity)
         for (int mu = 0; mu < 4; ++mu) substep(c, kind, parity, mu, slab_d);
-    if (kind == 0) c->sweep += 1;
+    if (kind != 1) c->sweep += 1;                                            // heatbath and Metropolis sweeps consume the counter
 }
 static void compound(ulo_ctx* c, int n_hb, int n_or, int slab_d) {
-    for (int i = 0; i < n_hb; ++i) one_sweep(c, 0, slab_d);
+    for (int i = 0; i < n_hb; ++i) one_sweep(c, c->alg == 1 ? 2 : 0, slab_d);   // the stochastic sweeps: heatbath or Metropolis
     for (int i = 0; i < n_or; ++i) one_sweep(c, 1, slab_d);
 }
 
@@ -390,9 +406,15 @@ int ulo_sweep(ulo_ctx* c, int n_hb, int n_or) {
     return ULO_OK;
 }
 int ulo_substep(ulo_ctx* c, int kind, int parity, int mu, int slab_d) {
-    if (!c || (kind != 0 && kind != 1) || (parity != 0 && parity != 1) || mu < 0 || mu > 3 || slab_d < 0) return ULO_EINVAL;
+    if (!c || kind < 0 || kind > 2 || (parity != 0 && parity != 1) || mu < 0 || mu > 3 || slab_d < 0) return ULO_EINVAL;
     if (slab_d > 0 && c->Nt % slab_d != 0) return ULO_EINVAL;
     substep(c, kind, parity, mu, slab_d);   // HB draws with the current counter and does not advance it
+    return ULO_OK;
+}
+int ulo_set_update_algorithm(ulo_ctx* c, int alg, double delta) {
+    if (!c || (alg != 0 && alg != 1) || (alg == 1 && !(delta > 0.0 && delta <= PI))) return ULO_EINVAL;
+    c->alg = alg;
+    if (alg == 1) c->met_delta = delta;
     return ULO_OK;
 }
 int ulo_set_subupdate(ulo_ctx* c, int n_hb, int n_or, int k_sweeps) {

@@ -42,7 +42,10 @@ int ulo_set_counter(ulo_ctx* h, uint64_t sweep_counter);
 
 /* updates: S8(c)-O1..O5 */
 int ulo_sweep(ulo_ctx* h, int n_hb, int n_or);
-int ulo_substep(ulo_ctx* h, int kind /*0 HB, 1 OR*/, int parity, int mu, int slab_d /*0 = unmasked*/);
+int ulo_substep(ulo_ctx* h, int kind /*0 HB, 1 OR, 2 Metropolis*/, int parity, int mu, int slab_d /*0 = unmasked*/);
+/* which algorithm the "n_hb" sweeps of ulo_sweep and of the sub-updates use: 0 = heatbath (default), 1 = one-hit
+ * Metropolis with a uniform proposal of half-width delta in (0, pi] (DESIGN R21) */
+int ulo_set_update_algorithm(ulo_ctx* h, int alg, double delta);
 int ulo_set_subupdate(ulo_ctx* h, int n_hb, int n_or, int k_sweeps);
 
 /* multilevel measurement: S8(c)-O6, O7; Alg. 1 */

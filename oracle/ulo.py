@@ -45,6 +45,7 @@ def lib():
         L.ulo_sweep.argtypes = [P, C.c_int, C.c_int]
         L.ulo_substep.argtypes = [P, C.c_int, C.c_int, C.c_int, C.c_int]
         L.ulo_set_subupdate.argtypes = [P, C.c_int, C.c_int, C.c_int]
+        L.ulo_set_update_algorithm.argtypes = [P, C.c_int, C.c_double]
         L.ulo_multilevel.argtypes = [P, C.c_int, C.c_int, C.c_int, P, C.c_int]
         L.ulo_multilevel2.argtypes = [P, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, P, C.c_int]
         L.ulo_measure_begin.argtypes = [P, C.c_int, C.c_int, P, C.c_int]
@@ -136,6 +137,9 @@ class Oracle:
 
     def substep(self, kind, parity, mu, slab_d=0):
         self._ck(lib().ulo_substep(self._h, int(kind), int(parity), int(mu), int(slab_d)))
+
+    def set_update_algorithm(self, alg, delta=np.pi):
+        self._ck(lib().ulo_set_update_algorithm(self._h, int(alg), float(delta)))
 
     def set_subupdate(self, n_hb, n_or, k_sweeps=1):
         self._ck(lib().ulo_set_subupdate(self._h, int(n_hb), int(n_or), int(k_sweeps)))
