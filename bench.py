@@ -256,6 +256,25 @@ def run_ours(args, rank, local_rank, world):
         e2e_ms = distributed_max(e2e_ms, dist, dev)
     e2e_value = world * n_upd / (e2e_ms / e2e_steps * 1e-3)
 
+    # ---- auxiliary figures (untimed region above is over): whole sweeps against their algorithmic traffic
+    def ev_time(fn, n=5):
+        fn()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(n):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / n * 1e-3
+
+    t_hb, t_or = ev_time(lambda: lat.sweep(1, 0)), ev_time(lambda: lat.sweep(0, 1))
+    lat.set_subupdate(0, 0, 1)
+    t_meas = ev_time(lambda: lat.multilevel(w["slab_d"], w["n_sub"], w["r_max"]), 2)    # tables + accumulation + slab product only
+    lat.set_subupdate(w["n_hb"], w["n_or"], 1)
+    lat.set_update_algorithm(1, 1.2)
+    t_met = ev_time(lambda: lat.sweep(1, 0))
+    lat.set_update_algorithm(0)
     if rank != 0:
         return
     peak, peak_src = measured_peak_hbm()
@@ -285,6 +304,12 @@ def run_ours(args, rank, local_rank, world):
                      "algorithmic_bytes_per_launch": or_bytes, "avg_launch_us": or_launch_s * 1e6,
                      "link_updates_per_s": (V / 2) / or_launch_s, "peak_source": peak_src},
         "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": cpu_sample},
+        # whole sweeps on the same lattice, CUDA events, against S8(d)'s algorithmic bytes (HB 32, OR 36 B per update)
+        "sweeps": {"hb_sweep_ms": t_hb * 1e3, "or_sweep_ms": t_or * 1e3, "metropolis_sweep_ms": t_met * 1e3,
+                   "compound_1hb_4or_frac_of_hbm_peak": (32 + 4 * 36) * 4 * V / (t_hb + 4 * t_or) / 1e9 / peak,
+                   "compound_1hb_4or_link_updates_per_s": 5 * 4 * V / (t_hb + 4 * t_or),
+                   "paper_recipe_1metropolis_3or_frac_of_hbm_peak": 4 * 36 * 4 * V / (t_met + 3 * t_or) / 1e9 / peak,
+                   "measurement_only_ms_per_multilevel_call": t_meas * 1e3},
     }
     print(json.dumps(line), flush=True)
     if dist is not None:

@@ -92,9 +92,18 @@ int ul_set_counter(ul_ctx* h, uint64_t sweep_counter);
 int ul_sweep(ul_ctx* h, int n_hb, int n_or);
 
 /* Test hook: one sub-step.  kind 0 = heatbath (draws with the current sweep counter, does
- * not advance it), 1 = overrelaxation.  slab_d > 0 freezes spatial links (mu != 0) on time
- * layers t % slab_d == 0; 0 = no mask.  Nt % slab_d must be 0. */
+ * not advance it), 1 = overrelaxation, 2 = Metropolis (draws like a heatbath sub-step).
+ * slab_d > 0 freezes spatial links (mu != 0) on time layers t % slab_d == 0;
+ * 0 = no mask.  Nt % slab_d must be 0. */
 int ul_substep(ul_ctx* h, int kind, int parity, int mu, int slab_d);
+
+/* Algorithm of the stochastic ("n_hb") sweeps of ul_sweep and of the sub-updates: 0 = heatbath (default,
+ * BASELINE north star), 1 = the paper's Metropolis update ("standard Metropolis algorithm combined with
+ * 3 steps of overrelaxation"; DESIGN R21: one hit per link, uniform proposal theta' = theta + delta (2 u1 - 1),
+ * accepted iff u2 <= exp(beta k [cos(theta' - alpha) - cos(theta - alpha)]); Philox tag 3).  delta: proposal
+ * half-width in radians, 0 < delta <= pi (ignored for alg = 0).  ul_substep takes kind = 2 for a Metropolis
+ * sub-step whatever the setting.  UL_EINVAL otherwise. */
+int ul_set_update_algorithm(ul_ctx* h, int alg, double delta);
 
 /* Sub-update recipe used inside the multilevel calls: k_sweeps x (n_hb HB + n_or OR) masked
  * sweeps between measurements.  Default 1 HB + 3 OR, k_sweeps = 1 (DESIGN R4, R5). */

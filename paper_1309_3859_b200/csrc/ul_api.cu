@@ -80,6 +80,8 @@ struct ul_ctx {
     int* hb_qcount = nullptr;
     int hb_qblocks = 0;
     int hb_local_rounds = 2;
+    int alg = 0;             // ul_set_update_algorithm: 0 heatbath, 1 Metropolis for the stochastic sweeps
+    double met_delta = 3.14159265358979323846;
     int vec = 1, bx = 1, by = 1, bz = 1;
     int sub_hb = 1, sub_or = 3, sub_k = 1;
     int batch_cap = 0;       // ul_set_accum_batch: 0 = default depth
@@ -160,7 +162,12 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
     const dim3 block(c->bx, c->by, 2 * c->bz), grid(c->Nh / c->by, c->Ns / c->bz, n_t);   // by = x2 row PAIRS per block
     a.queue = c->hb_queue; a.qcount = c->hb_qcount; a.qblocks = (int)(grid.x * grid.y * grid.z); a.local_rounds = c->hb_local_rounds;
     if (kind == 0 && cudaMemsetAsync(c->hb_qcount, 0, sizeof(int) * (size_t)a.qblocks, c->stream) != cudaSuccess) return fail(c, UL_ECUDA, "memset straggler counters");
-    const cudaError_t e = kind == 0 ? launch_update_mu<0>(c, mu, a, grid, block) : launch_update_mu<1>(c, mu, a, grid, block);
+    {
+        const double units = c->met_delta * (4294967296.0 / 6.283185307179586476925286766559);
+        a.met_delta_bt = units >= 2147483647.0 ? 2147483647 : (int)(units + 0.5);
+    }
+    const cudaError_t e = kind == 0 ? launch_update_mu<0>(c, mu, a, grid, block)
+                        : kind == 1 ? launch_update_mu<1>(c, mu, a, grid, block) : launch_update_mu<2>(c, mu, a, grid, block);
     if (e != cudaSuccess) return fail(c, UL_ECUDA, std::string("k_update launch: ") + cudaGetErrorString(e));
     c->launches += 1;
     if (kind == 0) {                                  // finish the links the heatbath kernel queued
@@ -176,11 +183,11 @@ int one_sweep(ul_ctx* c, int kind, int slab_d) {      // O5: parity outer, direc
             const int rc = substep(c, kind, parity, mu, slab_d);
             if (rc) return rc;
         }
-    if (kind == 0) c->sweep += 1;
+    if (kind != 1) c->sweep += 1;                     // heatbath and Metropolis sweeps consume the counter
     return UL_OK;
 }
 int compound(ul_ctx* c, int n_hb, int n_or, int slab_d) {
-    for (int i = 0; i < n_hb; ++i) { const int rc = one_sweep(c, 0, slab_d); if (rc) return rc; }
+    for (int i = 0; i < n_hb; ++i) { const int rc = one_sweep(c, c->alg == 1 ? 2 : 0, slab_d); if (rc) return rc; }
     for (int i = 0; i < n_or; ++i) { const int rc = one_sweep(c, 1, slab_d); if (rc) return rc; }
     return UL_OK;
 }
@@ -459,10 +466,17 @@ int ul_sweep(ul_ctx* c, int n_hb, int n_or) {
     return compound(c, n_hb, n_or, 0);
 }
 int ul_substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
-    if (!c || (kind != 0 && kind != 1) || (parity != 0 && parity != 1) || mu < 0 || mu > 3 || slab_d < 0)
+    if (!c || kind < 0 || kind > 2 || (parity != 0 && parity != 1) || mu < 0 || mu > 3 || slab_d < 0)
         return fail(c, UL_EINVAL, "bad sub-step arguments");
     if (slab_d > 0 && c->Nt % slab_d != 0) return fail(c, UL_EINVAL, "Nt % slab_d != 0");
     return substep(c, kind, parity, mu, slab_d);
+}
+int ul_set_update_algorithm(ul_ctx* c, int alg, double delta) {
+    if (!c || (alg != 0 && alg != 1) || (alg == 1 && !(delta > 0.0 && delta <= 3.14159265358979323846)))
+        return fail(c, UL_EINVAL, "alg must be 0 (heatbath) or 1 (Metropolis with 0 < delta <= pi)");
+    c->alg = alg;
+    if (alg == 1) c->met_delta = delta;
+    return UL_OK;
 }
 int ul_set_subupdate(ul_ctx* c, int n_hb, int n_or, int k_sweeps) {
     if (!c || n_hb < 0 || n_or < 0 || k_sweeps < 1) return fail(c, UL_EINVAL, "bad sub-update recipe");

@@ -29,6 +29,7 @@ struct UpdateArgs {
     int* qcount;          // entries queued per block (zeroed before the launch); segment b = queue[b*HB_QSEG ...]
     int qblocks;          // number of segments
     int local_rounds;     // lane-local retry rounds before a link is queued
+    int met_delta_bt;     // Metropolis proposal half-width delta as a binary angle (0 < delta <= pi -> up to 2^31 - 1)
 };
 
 constexpr int HB_QSEG = 128;   // straggler-queue entries per thread block (expected use ~25 of 1024 links)
@@ -157,6 +158,36 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
 #pragma unroll
         for (int i = 0; i < VEC; ++i)                 // overrelaxation (O2): theta' = 2 alpha - theta, exact mod 2 pi
             out[i] = (int)(2u * (unsigned)ulm::atan2_bt(Sy[i], Sx[i]) - (unsigned)old[i]);
+    } else if (KIND == 2) {
+        // Metropolis (DESIGN R21): one hit, theta' = theta + delta (2 u1 - 1), accept iff
+        // u2 <= exp(beta k [cos(theta' - alpha) - cos(theta - alpha)]).  With d = theta' - theta (an exact integer
+        // number of binary-angle units: v delta 2^-23, v = 2^24 u1 - 2^23 odd) the exponent is, without alpha and
+        // without cancellation,  beta 2 sin(d/2) [Sy cos(theta + d/2) - Sx sin(theta + d/2)].
+        int old[VEC];
+        if (VEC == 4) { const int4 q = *reinterpret_cast<const int4*>(own); old[0] = q.x; old[1 % VEC] = q.y; old[2 % VEC] = q.z; old[3 % VEC] = q.w; }
+        else if (VEC == 2) { const int2 q = *reinterpret_cast<const int2*>(own); old[0] = q.x; old[1 % VEC] = q.y; }
+        else old[0] = own[0];
+        const uint32_t site0 = (uint32_t)((st.e0 - h0) * 2 + 2 * h0 + st.off);            // canonical site index
+        const uint32_t c3 = (3u << 3) | ((uint32_t)p << 2) | (uint32_t)MU;                // tag 3 = Metropolis, attempt 0
+#pragma unroll
+        for (int i = 0; i < VEC; ++i) {
+            uint32_t w[4];
+            ulm::philox4x32_10(site0 + 2u * i, P.sweep_lo, P.sweep_hi, c3, P.key0, P.key1, w);
+            const int v = (int)((w[0] >> 8) | 1u) - (1 << 23);                            // (2 u1 - 1) 2^23, odd, |v| < 2^23
+            const int d = (int)(((long long)v * (long long)P.met_delta_bt) >> 23);        // |d| <= pi
+            const int h = d >> 1;                                                         // |h| <= pi/2: no reduction needed
+            const float rh = __int2float_rn(h) * ulm::BT_TO_RAD;
+            const float zh = rh * rh;
+            float sh = fmaf(2.598120545371785e-06f, zh, -0.00019805740157607943f);        // sin(d/2), degree 9 on |r| <= pi/2
+            sh = fmaf(sh, zh, 0.008333005011081696f);
+            sh = fmaf(sh, zh, -0.16666656732559204f);
+            sh = fmaf(sh, zh * rh, rh);
+            float cm = 0.0f, sm = 0.0f;
+            ulm::cis_accumulate((int)((unsigned)old[i] + (unsigned)h), cm, sm);           // cos, sin of theta + d/2
+            const float gain = P.beta * 2.0f * sh * fmaf(Sy[i], cm, -(Sx[i] * sm));
+            const bool accept = ulm::u01(w[1]) <= ulm::mufu_ex2(gain * 1.44269504088896340736f);
+            out[i] = accept ? (int)((unsigned)old[i] + (unsigned)d) : old[i];
+        }
     } else {
         // Heatbath (O3).  Attempt n of a link is a pure function of (site, sweep, n), so the order in
         // which a thread works through its rejections is free: every link gets attempt 0 with the warp
@@ -275,8 +306,8 @@ __global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_up
     st.dxp = (h0 + VEC >= Nh) ? VEC - Nh : VEC;
     st.dxm = (h0 == 0) ? Nh - 1 : -1;
     float Sx[VEC], Sy[VEC];
-    if (KIND == 1) {
-        // overrelaxation: the short tail is compiled into both branches (56 registers, 4 blocks per SM)
+    if (KIND != 0) {
+        // overrelaxation, Metropolis: the short tail is compiled into both branches (56 registers, 4 blocks per SM)
         if (sel) { gather_staples<MU, VEC, 1>(P, st, Sx, Sy); update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy); }
         else { gather_staples<MU, VEC, 0>(P, st, Sx, Sy); update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy); }
     } else {

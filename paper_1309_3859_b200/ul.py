@@ -18,7 +18,7 @@ UL_OK, UL_EINVAL, UL_ENOMEM, UL_ECUDA, UL_ESTATE = 0, -1, -2, -3, -4
 SYMBOLS = [
     "ul_create", "ul_create_ext", "ul_workspace_bytes", "ul_destroy", "ul_init", "ul_set_beta",
     "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep",
-    "ul_set_subupdate", "ul_multilevel", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
+    "ul_set_subupdate", "ul_set_update_algorithm", "ul_multilevel", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
     "ul_measure_end", "ul_set_accum_batch", "ul_plaquette", "ul_read_correlators", "ul_read_slab_averages",
     "ul_get_launch_count", "ul_philox_selftest", "ul_sync", "ul_last_error",
 ]
@@ -58,6 +58,7 @@ def lib():
         L.ul_sweep.argtypes = [P, C.c_int, C.c_int]
         L.ul_substep.argtypes = [P, C.c_int, C.c_int, C.c_int, C.c_int]
         L.ul_set_subupdate.argtypes = [P, C.c_int, C.c_int, C.c_int]
+        L.ul_set_update_algorithm.argtypes = [P, C.c_int, C.c_double]
         L.ul_multilevel.argtypes = [P, C.c_int, C.c_int, C.c_int, P, C.c_int]
         L.ul_multilevel2.argtypes = [P, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, P, C.c_int]
         L.ul_measure_begin.argtypes = [P, C.c_int, C.c_int, P, C.c_int]
@@ -191,6 +192,9 @@ class Lattice:
 
     def substep(self, kind, parity, mu, slab_d=0):
         self._ck(lib().ul_substep(self._h, int(kind), int(parity), int(mu), int(slab_d)))
+
+    def set_update_algorithm(self, alg, delta=np.pi):
+        self._ck(lib().ul_set_update_algorithm(self._h, int(alg), float(delta)))
 
     def set_subupdate(self, n_hb, n_or, k_sweeps=1):
         self._ck(lib().ul_set_subupdate(self._h, int(n_hb), int(n_or), int(k_sweeps)))

@@ -118,7 +118,7 @@ def test_set_links_rejects_unwrapped_angles(ul):
 def test_error_codes(ul):
     g = ul.Lattice(4, 4, 1.0, 1)
     for call in (lambda: g.multilevel(3, 0, 1), lambda: g.multilevel(2, 0, 3), lambda: g.multilevel(2, -1, 1),
-                 lambda: g.multilevel2(2, 1, 3, 1, 1), lambda: g.substep(0, 0, 4), lambda: g.substep(2, 0, 0)):
+                 lambda: g.multilevel2(2, 1, 3, 1, 1), lambda: g.substep(0, 0, 4), lambda: g.substep(3, 0, 0), lambda: g.set_update_algorithm(1, 4.0)):
         with pytest.raises(ul.UlError) as e:
             call()
         assert e.value.code == ul.UL_EINVAL
@@ -606,3 +606,98 @@ def test_config4_32x32_two_level_and_sweep(ul, ulo):
     g.set_subupdate(1, 3, 1)
     o.set_subupdate(1, 3, 1)
     _whole_hb_sweep(g, o, ulo, 1.00)
+
+
+# ----------------------------------------------------------------------------- Metropolis (next row, DESIGN R21)
+@pytest.mark.parametrize("Ns,Nt,therm,delta", [(4, 4, 0, 1.0), (8, 6, 0, np.pi), (16, 4, 20, 1.3)])
+def test_metropolis_per_substep(ul, ulo, Ns, Nt, therm, delta):
+    """Every Metropolis sub-step, full and slab-masked, from the oracle's configuration: a link either moves by
+    the same proposal (within 2e-5 rad; in fact the proposal is an exact integer here) or stays bit for bit;
+    accept/reject flips at the rounding boundary are counted (< 1e-5 of links)."""
+    beta, seed = 0.99, 7
+    o = ulo.Oracle(Ns, Nt, beta, seed)
+    o.set_update_algorithm(1, delta)
+    g = ul.Lattice(Ns, Nt, beta, seed)
+    g.set_update_algorithm(1, delta)
+    for _ in range(therm):
+        o.sweep(1, 3)
+    flips = n_upd = 0
+    for d in (0, 2):
+        for parity in (0, 1):
+            for mu in range(4):
+                before = o.get_links()
+                g.set_links(before)
+                g.set_counter(o.get_counter())
+                o.substep(2, parity, mu, d)
+                g.substep(2, parity, mu, d)
+                got, want = g.get_links(), o.get_links()
+                diff = wrapdiff(got, want)
+                moved_o, moved_g = want != before, wrapdiff(got, before) > 1.3e-9
+                flips += int((moved_o != moved_g).sum())
+                same = moved_o == moved_g
+                assert diff[same].max() <= 1e-6                      # the proposal is formed exactly; fp32 store of the oracle
+                n_upd += int(moved_o.sum())
+        o.set_counter(o.get_counter() + 1)
+    assert n_upd > 0.2 * 4 * Ns ** 3 * Nt
+    assert flips <= max(1, 1e-5 * 4 * Ns ** 3 * Nt * 4), flips
+
+
+def test_metropolis_whole_sweep_and_counter(ul, ulo):
+    Ns, Nt, beta = 16, 4, 0.99
+    o = ulo.Oracle(Ns, Nt, beta, 2)
+    o.set_update_algorithm(1, 1.0)
+    for _ in range(30):
+        o.sweep(1, 3)
+    g = ul.Lattice(Ns, Nt, beta, 2)
+    g.set_update_algorithm(1, 1.0)
+    g.set_links(o.get_links())
+    g.set_counter(o.get_counter())
+    o.sweep(1, 0)
+    g.sweep(1, 0)
+    assert g.get_counter() == o.get_counter()
+    diff = wrapdiff(g.get_links(), o.get_links())
+    assert (diff > TOL).mean() < 1e-5, ((diff > TOL).sum(), diff.max())
+
+
+def test_metropolis_leaves_von_mises_stationary_on_device(ul):
+    """The pin of tests/test_oracle_metropolis.py repeated on the CUDA path (no oracle involved)."""
+    from scipy import special, stats
+    Ns, Nt, beta = 16, 8, 0.5
+    a = 6 * beta
+    rng = np.random.default_rng(5)
+    even = (np.indices((Nt, Ns, Ns, Ns)).sum(axis=0) & 1) == 0
+    g = ul.Lattice(Ns, Nt, beta, 22)
+    g.set_update_algorithm(1, 2.0)
+    links = np.zeros((4, Nt, Ns, Ns, Ns), dtype=np.float32)
+    links[0][even] = rng.uniform(-np.pi, np.pi, int(even.sum())).astype(np.float32)
+    g.set_links(links)
+    for it in range(40):
+        g.set_counter(it)
+        g.substep(2, 0, 0, 0)
+    out = g.get_links()
+    assert not out[1:].any()
+    th = out[0][even].astype(np.float64)
+    _, p = stats.kstest(th, stats.vonmises(kappa=a).cdf)
+    assert p > 1e-3, p
+    assert abs(np.cos(th).mean() - special.iv(1, a) / special.iv(0, a)) < 4 * np.sqrt(0.5 / th.size)
+
+
+def test_metropolis_ensemble_matches_oracle_and_heatbath(ul, ulo):
+    """P3 for the Metropolis chain: plaquette of independent GPU and oracle chains (the paper's recipe,
+    1 Metropolis + 3 overrelaxation) within 3 combined standard errors; and of the GPU heatbath chain."""
+    Ns, Nt, beta = 4, 4, 0.95
+    def chain(L, n):
+        vals = []
+        for _ in range(n):
+            L.sweep(1, 3)
+            vals.append(L.plaquette()[0])
+        return np.array(vals)
+    g = ul.Lattice(Ns, Nt, beta, 51); g.set_update_algorithm(1, 1.2)
+    o = ulo.Oracle(Ns, Nt, beta, 52); o.set_update_algorithm(1, 1.2)
+    h = ul.Lattice(Ns, Nt, beta, 53)
+    for L in (g, o, h):
+        L.sweep(40, 40)
+    vg, vo, vh = chain(g, 400), chain(o, 400), chain(h, 400)
+    for a_, b_ in ((vg, vo), (vg, vh)):
+        (ma, ea), (mb, eb) = binned_err(a_), binned_err(b_)
+        assert abs(ma - mb) < 3 * np.hypot(ea, eb), (ma, ea, mb, eb)
