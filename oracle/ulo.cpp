@@ -554,6 +554,35 @@ int ulo_heatbath_phi(double a, uint64_t seed, uint32_t c0, uint32_t c1, uint32_t
     *phi = heatbath_phi(a, key, c0, c1, c2, c3low & 0xffu, attempts);
     return ULO_OK;
 }
+// <P> = (1/Ns^3) sum_x prod_t U_0(x,t)  (Eqs. 15-16).  multihit = 1: every temporal link is replaced by
+// its mean over the local weight exp(beta k cos(theta - alpha)) with all other links held fixed,
+// U_0 -> (I1(beta k)/I0(beta k)) e^{i alpha} (analytic multihit, "when calculating the Polyakov loop average we
+// also apply the analytical multihit integration technique"); k e^{i alpha} is the staple sum O1.  The links
+// of one Polyakov line do not appear in each other's staples (Nt >= 2), so all Nt of them are replaced at once.
+int ulo_polyakov(ulo_ctx* c, int multihit, double* out) {
+    if (!c || !out || (multihit != 0 && multihit != 1)) return ULO_EINVAL;
+    cplx mean(0, 0);
+    for (long xs = 0; xs < c->Vs; ++xs) {
+        cplx p(1, 0);
+        for (int t = 0; t < c->Nt; ++t) {
+            const long x = xs + c->Vs * t;
+            if (!multihit) {
+                const double th = TH(c, 0, x);
+                p *= cplx(std::cos(th), std::sin(th));
+            } else {
+                double k, alpha;
+                k_alpha(staple(c, 0, x), &k, &alpha);
+                const double a = c->beta * k;
+                const double ratio = a == 0.0 ? 0.0 : std::cyl_bessel_i(1.0, a) / std::cyl_bessel_i(0.0, a);
+                p *= ratio * cplx(std::cos(alpha), std::sin(alpha));
+            }
+        }
+        mean += p;
+    }
+    mean /= (double)c->Vs;
+    out[0] = mean.real(); out[1] = mean.imag();
+    return ULO_OK;
+}
 int ulo_polyakov_naive(ulo_ctx* c, int r_max, double* corr, double* mean_P) {
     if (!c || r_max < 0 || r_max > c->Ns / 2) return ULO_EINVAL;
     std::vector<cplx> P((size_t)c->Vs);

@@ -59,6 +59,9 @@ int ulo_accumulate(ulo_ctx* h);
 int ulo_measure_end(ulo_ctx* h);
 
 int ulo_plaquette(ulo_ctx* h, double* mean_cos /*[3]: all, time-like, space-like*/);
+/* Polyakov-loop average <P> (Eqs. 15-16), out[2] = (Re, Im); multihit = 1: analytic multihit on every
+ * temporal link, U_0 -> (I1(beta k)/I0(beta k)) e^{i alpha} */
+int ulo_polyakov(ulo_ctx* h, int multihit, double* out);
 int ulo_read_correlators(ulo_ctx* h, double* corr /*[r_max][2]*/,
                          double* field /*[r_max][n_fp][12][2]*/, double* vacuum /*[12]*/);
 /* slab averages [T] of the last measurement (outer level for two-level):

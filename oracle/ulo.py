@@ -62,6 +62,7 @@ def lib():
         L.ulo_heatbath_phi.argtypes = [C.c_double, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32,
                                        C.POINTER(C.c_double), C.POINTER(C.c_int)]
         L.ulo_polyakov_naive.argtypes = [P, C.c_int, P, P]
+        L.ulo_polyakov.argtypes = [P, C.c_int, P]
         L.ulo_paper_accumulator_bytes.argtypes = [C.c_int, C.c_int, C.c_int]
         L.ulo_paper_accumulator_bytes.restype = C.c_double
     return _lib
@@ -190,6 +191,11 @@ class Oracle:
         k, a = C.c_double(), C.c_double()
         self._ck(lib().ulo_staple(self._h, int(mu), int(site), C.byref(k), C.byref(a)))
         return k.value, a.value
+
+    def polyakov(self, multihit=0):
+        out = np.zeros(2)
+        self._ck(lib().ulo_polyakov(self._h, int(multihit), _ptr(out)))
+        return complex(out[0], out[1])
 
     def polyakov_naive(self, r_max):
         corr = np.zeros((max(r_max, 1), 2))
