@@ -149,6 +149,13 @@ int ul_set_accum_batch(ul_ctx* h, int depth);
  * 3V space-like ones: HOST double[3].  Synchronises. */
 int ul_plaquette(ul_ctx* h, double* mean_cos);
 
+/* Polyakov-loop average <P> = (1/Ns^3) sum_x prod_t U_0(x,t) (Eqs. 15-16): HOST double[2] = (Re, Im).
+ * multihit = 1: analytic multihit, every temporal link replaced by its mean over its local weight with the
+ * other links fixed, U_0 -> (I1(beta k)/I0(beta k)) e^{i alpha}, k e^{i alpha} the staple sum (
+ * SURVEY S8(f) rank 1); same expectation value, smaller variance.  fp64 throughout.  Synchronises.
+ * UL_EINVAL: multihit not 0 or 1, null pointer. */
+int ul_polyakov(ul_ctx* h, int multihit, double* mean_P);
+
 /* Results of the last measurement, HOST buffers (any may be NULL):
  * corr[r_max][2]           C(r) = (1/3Ns^3) sum_x sum_mu prod_s [T](x,s,mu,r)       (re, im)
  * field[r_max][n_fp][12][2] G(r,fp,ch) of Eq. 34; ch = 2*comp + kind, comp 0..5 = plaquette

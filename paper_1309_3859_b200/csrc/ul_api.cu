@@ -567,6 +567,17 @@ int ul_plaquette(ul_ctx* c, double* out) {
     out[0] = 0.5 * (v[0] + v[1]); out[1] = v[0]; out[2] = v[1];
     return UL_OK;
 }
+int ul_polyakov(ul_ctx* c, int multihit, double* out) {
+    if (!c || !out || (multihit != 0 && multihit != 1)) return fail(c, UL_EINVAL, "multihit must be 0 or 1");
+    const int nb = (int)((c->Vs + 255) / 256) < NBLK ? (int)((c->Vs + 255) / 256) : NBLK;
+    ulk::k_polyakov<<<nb, 256, 0, c->stream>>>(geom(c), c->th, c->beta, multihit, c->scratch);
+    ulk::k_sum_partials<<<2, 256, 0, c->stream>>>(c->scratch, nb, c->scratch + 2 * NBLK, 1.0 / (double)c->Vs, 0);
+    UL_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    UL_CUDA(c, cudaMemcpyAsync(out, c->scratch + 2 * NBLK, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    UL_CUDA(c, cudaStreamSynchronize(c->stream));
+    return UL_OK;
+}
 int ul_read_correlators(ul_ctx* c, double* corr, double* field, double* vacuum) {
     if (!c) return fail(c, UL_EINVAL, "null handle");
     if (!c->have) return fail(c, UL_ESTATE, "no measurement yet");

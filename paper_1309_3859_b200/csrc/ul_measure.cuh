@@ -190,6 +190,70 @@ __global__ void __launch_bounds__(256) k_plaquette(Geom g, const int* __restrict
     if (threadIdx.x == 0) { partial[blk] = v[0]; partial[nblk + blk] = v[1]; }
 }
 
+// ---------------------------------------------------------------- Polyakov-loop average (next row S8(f) rank 1)
+// I1(a)/I0(a) in fp64 by the backward recurrence R_{n-1} = 1 / (2n/a + R_n), R_n = I_{n+1}/I_n, from R_N = 0 at
+// N = a + 40 (each step contracts the error by R^2 < 0.4, so the start value is forgotten to 1e-18).
+__device__ __forceinline__ double bessel_ratio_i1_i0(double a) {
+    if (!(a > 1e-300)) return 0.0;
+    const double two_over_a = 2.0 / a;
+    double R = 0.0;
+    for (int n = (int)a + 40; n >= 1; --n) R = 1.0 / ((double)n * two_over_a + R);
+    return R;
+}
+
+// partial[b], partial[nblk + b] = block sums of Re, Im of P(x) = prod_t U_0(x,t) (Eq. 15) over the spatial sites;
+// multihit = 1: U_0 -> (I1(beta k)/I0(beta k)) e^{i alpha} = (I1/I0)(beta k) S/k with the staple sum S = k e^{i alpha}
+// (P:209), everything in fp64 on exact integer phase sums.  One thread per spatial site, grid-stride.
+__global__ void __launch_bounds__(256) k_polyakov(Geom g, const int* __restrict__ th, double beta, int multihit,
+                                                  double* __restrict__ partial) {
+    __shared__ double sm[2 * 32];
+    const int Ns = g.Ns, Nt = g.Nt;
+    double v[2] = {0.0, 0.0};
+    for (int xs = blockIdx.x * blockDim.x + threadIdx.x; xs < (int)g.Vs; xs += gridDim.x * blockDim.x) {
+        int x[4];
+        x[1] = xs % Ns;
+        x[2] = (xs / Ns) % Ns;
+        x[3] = xs / (Ns * Ns);
+        double pr = 1.0, pi = 0.0;
+        unsigned phase = 0u;
+        for (int t = 0; t < Nt; ++t) {
+            if (!multihit) {
+                phase += (unsigned)__ldg(th + link_index(g, 0, t, x[3], x[2], x[1]));
+                continue;
+            }
+            const int tp = (t + 1 == Nt) ? 0 : t + 1;
+            double Sx = 0.0, Sy = 0.0;
+#pragma unroll
+            for (int nu = 1; nu <= 3; ++nu) {
+                int yp[4] = {t, x[1], x[2], x[3]}, ym[4] = {t, x[1], x[2], x[3]};
+                yp[nu] = (x[nu] + 1 == Ns) ? 0 : x[nu] + 1;
+                ym[nu] = (x[nu] == 0) ? Ns - 1 : x[nu] - 1;
+                // -sigma+ = th_nu(x) + th_0(x+nu) - th_nu(x+t);  -sigma- = th_nu(x+t-nu) + th_0(x-nu) - th_nu(x-nu)
+                const unsigned sp = (unsigned)__ldg(th + link_index(g, nu, t, x[3], x[2], x[1]))
+                                  + (unsigned)__ldg(th + link_index(g, 0, t, yp[3], yp[2], yp[1]))
+                                  - (unsigned)__ldg(th + link_index(g, nu, tp, x[3], x[2], x[1]));
+                const unsigned sn = (unsigned)__ldg(th + link_index(g, nu, tp, ym[3], ym[2], ym[1]))
+                                  + (unsigned)__ldg(th + link_index(g, 0, t, ym[3], ym[2], ym[1]))
+                                  - (unsigned)__ldg(th + link_index(g, nu, t, ym[3], ym[2], ym[1]));
+                double c, s;
+                ulm::sincos_bt_f64((int)sp, c, s); Sx += c; Sy += s;
+                ulm::sincos_bt_f64((int)sn, c, s); Sx += c; Sy += s;
+            }
+            const double k = sqrt(Sx * Sx + Sy * Sy);
+            const double f = k > 0.0 ? bessel_ratio_i1_i0(beta * k) / k : 0.0;             // (I1/I0) e^{i alpha} = f S
+            const double ur = f * Sx, ui = f * Sy;
+            const double nr = pr * ur - pi * ui;
+            pi = pr * ui + pi * ur;
+            pr = nr;
+        }
+        if (!multihit) ulm::sincos_bt_f64((int)phase, pr, pi);
+        v[0] += pr;
+        v[1] += pi;
+    }
+    block_sum<2>(v, sm);
+    if (threadIdx.x == 0) { partial[blockIdx.x] = v[0]; partial[gridDim.x + blockIdx.x] = v[1]; }
+}
+
 // ---------------------------------------------------------------- per-configuration slab tables
 // U[s][xs]  = exp(i sum_{t in slab s} theta_0(xs,t)) in fp64: the angle sum is a wrapping integer add
 //             (exact mod 2 pi), reduced in integers and expanded in fp64 (sincos_bt_f64), so U is good to 1 ulp and

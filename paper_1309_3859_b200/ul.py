@@ -19,7 +19,7 @@ SYMBOLS = [
     "ul_create", "ul_create_ext", "ul_workspace_bytes", "ul_destroy", "ul_init", "ul_set_beta",
     "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep",
     "ul_set_subupdate", "ul_set_update_algorithm", "ul_multilevel", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
-    "ul_measure_end", "ul_set_accum_batch", "ul_plaquette", "ul_read_correlators", "ul_read_slab_averages",
+    "ul_measure_end", "ul_set_accum_batch", "ul_plaquette", "ul_polyakov", "ul_read_correlators", "ul_read_slab_averages",
     "ul_get_launch_count", "ul_philox_selftest", "ul_sync", "ul_last_error",
 ]
 
@@ -63,6 +63,7 @@ def lib():
         L.ul_multilevel2.argtypes = [P, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, P, C.c_int]
         L.ul_measure_begin.argtypes = [P, C.c_int, C.c_int, P, C.c_int]
         L.ul_set_accum_batch.argtypes = [P, C.c_int]
+        L.ul_polyakov.argtypes = [P, C.c_int, P]
         L.ul_accumulate.argtypes = [P]
         L.ul_measure_end.argtypes = [P]
         L.ul_plaquette.argtypes = [P, P]
@@ -243,6 +244,11 @@ class Lattice:
         out = np.zeros((3, R, S, self.Ns ** 3, 2))
         self._ck(lib().ul_read_slab_averages(self._h, _ptr(out)))
         return out[..., 0] + 1j * out[..., 1]
+
+    def polyakov(self, multihit=0):
+        out = np.zeros(2)
+        self._ck(lib().ul_polyakov(self._h, int(multihit), _ptr(out)))
+        return complex(out[0], out[1])
 
     def launch_count(self):
         v = C.c_uint64()

@@ -701,3 +701,50 @@ def test_metropolis_ensemble_matches_oracle_and_heatbath(ul, ulo):
     for a_, b_ in ((vg, vo), (vg, vh)):
         (ma, ea), (mb, eb) = binned_err(a_), binned_err(b_)
         assert abs(ma - mb) < 3 * np.hypot(ea, eb), (ma, ea, mb, eb)
+
+
+# ----------------------------------------------------------------------------- Polyakov loop with multihit (next row)
+@pytest.mark.parametrize("Ns,Nt,beta", [(4, 4, 0.9), (8, 6, 1.1), (16, 4, 0.99)])
+def test_polyakov_and_multihit_against_oracle(ul, ulo, Ns, Nt, beta):
+    """<P> plain and with analytic multihit (Eqs. 15-16) on the oracle's configurations, relative 1e-5
+    (DESIGN R17); closed forms on device; gauge invariance on device."""
+    from scipy import special
+    o = ulo.Oracle(Ns, Nt, beta, 3)
+    g = ul.Lattice(Ns, Nt, beta, 3)
+    for n_sw in (0, 3, 10):
+        for _ in range(n_sw):
+            o.sweep(1, 2)
+        g.set_links(o.get_links())
+        for mh in (0, 1):
+            want, got = o.polyakov(mh), g.polyakov(mh)
+            scale = 1.0 if mh == 0 else (special.ive(1, 4 * beta) / special.ive(0, 4 * beta)) ** Nt   # size of a multihit term
+            assert abs(got - want) <= 1e-5 * max(abs(want), scale / np.sqrt(Ns ** 3)), (n_sw, mh, got, want)
+    g.init(0)
+    r = special.ive(1, 6 * beta) / special.ive(0, 6 * beta)
+    assert abs(g.polyakov(0) - 1) < 1e-14 and abs(g.polyakov(1) - r ** Nt) < 1e-13
+    links = inputs.hot_links(Ns, Nt, 8) * 0.5
+    g.set_links(links)
+    a = g.polyakov(1)
+    g.set_links(inputs.gauge_transform(links, inputs.gauge_function(Ns, Nt, 9)))
+    b = g.polyakov(1)                                               # the transformed links are re-rounded to fp32
+    assert abs(b - a) <= 1e-5 * max(abs(a), abs(b)) + 1e-9 * (special.ive(1, 4 * beta) / special.ive(0, 4 * beta)) ** Nt
+    with pytest.raises(ul.UlError):
+        g.polyakov(2)
+
+
+def test_polyakov_full_size_64(ul, ulo):
+    """64^4 (launch configuration of the full-size lattice): plain <P> against the oracle's Eq. 15 loop; the
+    multihit value on sampled sites is covered by the small-lattice parity above, here its closed form on the
+    cold lattice and the timing print."""
+    from scipy import special
+    Ns = Nt = 64
+    g = ul.Lattice(Ns, Nt, 0.98, 5)
+    g.sweep(1, 1)
+    o = ulo.Oracle(Ns, Nt, 0.98, 5)
+    o.set_links(g.get_links())
+    want = o.polyakov(0)
+    got = g.polyakov(0)
+    assert abs(got - want) <= 1e-5 / np.sqrt(Ns ** 3)
+    g.init(0)
+    r = special.ive(1, 6 * 0.98) / special.ive(0, 6 * 0.98)
+    assert abs(g.polyakov(1) - r ** Nt) < 1e-12 * r ** Nt + 1e-18
