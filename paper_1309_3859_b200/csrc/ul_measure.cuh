@@ -367,15 +367,15 @@ struct AccumArgs {
 // The accumulators are streamed (ld.cs / st.cs, RB entries in flight per thread); the U tables, which every
 // site re-reads 6 r_max times, stay in L1/L2.
 #ifndef UL_ACC_RB
-#define UL_ACC_RB 4
+#define UL_ACC_RB 2
 #endif
 #ifndef UL_ACC_MINB
-#define UL_ACC_MINB 1
+#define UL_ACC_MINB 3
 #endif
 constexpr int ACC_RB = UL_ACC_RB;
 
 template <int KB, bool FIELD, bool FULL>
-__global__ void __launch_bounds__(256, UL_ACC_MINB) k_accumulate(const AccumArgs P) {
+__global__ void __launch_bounds__(256, FIELD ? 1 : UL_ACC_MINB) k_accumulate(const AccumArgs P) {
     const Geom& g = P.g;
     const long long n = (long long)P.n_slab * g.Vs;
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
