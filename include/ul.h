@@ -124,6 +124,19 @@ int ul_set_subupdate(ul_ctx* h, int n_hb, int n_or, int k_sweeps);
 int ul_multilevel(ul_ctx* h, int slab_thickness, int n_sub, int r_max,
                   const int* field_points, int n_fp);
 
+/* Single level by REPLAY (memory formula P:378-384).  The same estimator as
+ * ul_multilevel, the same sub-update trajectory, the same outputs (correlators bit for bit, field
+ * values to fp64 rounding order) and the same final configuration and sweep counter, but without the
+ * per-site TO accumulators, which are 12 n_fp times the T accumulators (972 MB against 1.7 MB in the
+ * paper's own example): the estimator is linear in O and the counter-based RNG makes the trajectory
+ * repeatable, so pass 1 accumulates only the sums of T, and pass 2 replays the sub-updates from the
+ * saved start configuration and adds W(x,s) T_j(x,s) sum_t O_j(x+off,t), W = prod_{s' != s} [T](x,s'),
+ * straight into lattice sums.  Costs the sub-update sweeps twice; workspace ul_workspace_bytes_replay
+ * (two T-sized arrays).  n_fp = 0 is the same as ul_multilevel.  Errors as ul_multilevel. */
+int ul_multilevel_replay(ul_ctx* h, int slab_thickness, int n_sub, int r_max,
+                         const int* field_points, int n_fp);
+size_t ul_workspace_bytes_replay(int Ns, int Nt, int slab_thickness, int r_max, int n_fp);
+
 /* Two levels (Eq. 27, Eqs. 32-33 P:343-347 with DESIGN R7, Alg. 1 lines 5-18):
  * n_out x { sub-update masked with d_out; n_in x { sub-update masked with d_in; accumulate
  * T^(d_in), TO^(d_in) }; combine the m = d_out/d_in inner slab averages of each outer slab

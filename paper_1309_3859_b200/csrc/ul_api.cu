@@ -31,23 +31,25 @@ struct Workspace {           // byte offsets into the measurement workspace
 
 size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
 
-Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_fp) {
+Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_fp, bool replay = false) {
     Workspace w;
     const size_t Vs = (size_t)Ns * Ns * Ns;
     const size_t n_in = (size_t)(Nt / d_in), n_out = d_out > 0 ? (size_t)(Nt / d_out) : 0;
     const size_t F12 = (size_t)n_fp * 12, R = (size_t)r_max;
+    const size_t FB = replay ? 1 : F12;          // replay: the B2 slot holds the weights W (one A-sized array), no TO sums
+    const size_t ot_slots = replay ? 1 : 0;      // replay: one Ot table (pass 2 is not batched); else kb slots
     // batch depth: KBATCH, reduced if the per-configuration tables would outgrow the accumulators they feed
-    const size_t table = n_in * Vs * (16 + (n_fp > 0 ? 48 : 0));
-    const size_t accum = 3 * R * n_in * Vs * 16 * (1 + F12);
+    const size_t table = n_in * Vs * (16 + (n_fp > 0 && !replay ? 48 : 0));
+    const size_t accum = 3 * R * n_in * Vs * 16 * (1 + FB);
     int kb = KBATCH;
     while (kb > 1 && (size_t)kb * table > accum / 2 + ((size_t)64 << 20)) kb >>= 1;
     w.kb = kb;
     size_t o = 0;
     w.U = o;   o = align_up(o + (size_t)kb * n_in * Vs * 16);
-    w.Ot = o;  o = align_up(o + (n_fp > 0 ? (size_t)kb * 12 * n_in * Vs * sizeof(float) : 0));
+    w.Ot = o;  o = align_up(o + (n_fp > 0 ? (ot_slots ? ot_slots : (size_t)kb) * 12 * n_in * Vs * sizeof(float) : 0));
     w.fps = o; o = align_up(o + (size_t)(n_fp > 0 ? n_fp : 1) * 3 * sizeof(int));
     w.A2 = o;  o = align_up(o + 3 * R * n_in * Vs * 16);
-    w.B2 = o;  o = align_up(o + 3 * R * n_in * F12 * Vs * 16);
+    w.B2 = o;  o = align_up(o + 3 * R * n_in * FB * Vs * 16);
     w.A4 = o;  o = align_up(o + 3 * R * n_out * Vs * 16);
     w.B4 = o;  o = align_up(o + 3 * R * n_out * F12 * Vs * 16);
     const size_t n_entries = R * (1 + F12);
@@ -90,6 +92,7 @@ struct ul_ctx {
     int d = 0, r_max = 0, n_fp = 0, n_slab = 0, d_out = 0, n_outer = 0;
     long long n_acc = 0;
     int n_pending = 0;       // configurations tabulated but not yet added to the accumulators
+    bool replay = false;     // ul_multilevel_replay in progress: no TO sums, fields reduced on the fly in pass 2
     bool acc_fresh = true;   // the inner sums A2, B2 hold nothing yet: the next pass writes instead of adding
     Workspace ws;
     // last result
@@ -203,7 +206,7 @@ template <typename T> T* wsp(ul_ctx* c, size_t off) { return reinterpret_cast<T*
 
 // reserve the workspace, upload the field points, zero the accumulators
 int open_measurement(ul_ctx* c, int d_in, int d_out, int r_max, const int* fps, int n_fp) {
-    const Workspace w = plan_workspace(c->Ns, c->Nt, d_in, d_out, r_max, n_fp);
+    const Workspace w = plan_workspace(c->Ns, c->Nt, d_in, d_out, r_max, n_fp, c->replay);
     if (w.total > c->work_bytes) {
         if (!c->own_work && c->work) return fail(c, UL_ENOMEM, "accumulators exceed the caller's workspace");
         if (c->work) { UL_CUDA(c, cudaStreamSynchronize(c->stream)); cudaFree(c->work); c->work = nullptr; c->work_bytes = 0; }
@@ -244,7 +247,7 @@ int flush(ul_ctx* c) {
         if (a.nk == KB) ulk::k_accumulate<KB, FIELD, true><<<nb, 256, 0, c->stream>>>(a);           \
         else ulk::k_accumulate<KB, FIELD, false><<<nb, 256, 0, c->stream>>>(a);                     \
     } while (0)
-    if (c->n_fp > 0) {
+    if (c->n_fp > 0 && !c->replay) {
         if (a.nk == 1) UL_ACC_LAUNCH(1, true);
         else if (a.nk <= 4) UL_ACC_LAUNCH(4, true);
         else UL_ACC_LAUNCH(KBATCH, true);
@@ -268,7 +271,7 @@ int accumulate(ul_ctx* c) {
     ulk::TableArgs t;
     t.g = geom(c); t.th = c->th; t.d = c->d; t.n_slab = c->n_slab;
     t.U = wsp<double2>(c, c->ws.U) + (size_t)c->n_pending * n;
-    t.Ot = c->n_fp > 0 ? wsp<float>(c, c->ws.Ot) + (size_t)c->n_pending * 12 * n : nullptr;
+    t.Ot = (c->n_fp > 0 && !c->replay) ? wsp<float>(c, c->ws.Ot) + (size_t)c->n_pending * 12 * n : nullptr;
     t.partial = wsp<double>(c, c->ws.partial);
     const int gx = (c->Ns * c->Ns + 255) / 256, rows = c->n_slab * c->Ns;
     const int gy = rows < TBLK / gx ? rows : (TBLK / gx > 0 ? TBLK / gx : 1);
@@ -290,12 +293,13 @@ int finish(ul_ctx* c, const double2* A, const double2* B, int n_slab, double inv
     a.Vs = c->Vs; a.r_max = R; a.n_fp = F; a.n_slab = n_slab; a.inv = inv; a.A = A; a.B = B;
     a.partial = wsp<double>(c, c->ws.partial);
     ulk::k_slab_product<false><<<dim3(NBLK, R), 256, 0, c->stream>>>(a, 0);
-    if (F > 0) { ulk::k_slab_product<true><<<dim3(NBLK, n_entries - R), 256, 0, c->stream>>>(a, R); c->launches += 1; }
+    const bool stored = F > 0 && !c->replay;       // replay: the field sums were reduced on the fly into the result buffer
+    if (stored) { ulk::k_slab_product<true><<<dim3(NBLK, n_entries - R), 256, 0, c->stream>>>(a, R); c->launches += 1; }
     double* res = wsp<double>(c, c->ws.result);
     // C /= 3 Vs ; G /= 3 Vs Nt (DESIGN R9)
     ulk::k_sum_partials<<<2 * R, 256, 0, c->stream>>>(a.partial, NBLK, res, 1.0 / (3.0 * (double)c->Vs), 0);
     c->launches += 2;
-    if (F > 0) {
+    if (stored) {
         ulk::k_sum_partials<<<2 * (n_entries - R), 256, 0, c->stream>>>(a.partial + (size_t)2 * R * NBLK, NBLK, res + 2 * R,
                                                                         1.0 / (3.0 * (double)c->Vs * (double)c->Nt), 0);
         c->launches += 1;
@@ -386,6 +390,10 @@ size_t ul_workspace_bytes(int Ns, int Nt, int d_in, int d_out, int r_max, int n_
         r_max < 1 || n_fp < 0)
         return 0;
     return plan_workspace(Ns, Nt, d_in, d_out, r_max, n_fp).total;
+}
+size_t ul_workspace_bytes_replay(int Ns, int Nt, int d, int r_max, int n_fp) {
+    if (Ns < 2 || Nt < 2 || d < 1 || Nt % d != 0 || r_max < 1 || n_fp < 0) return 0;
+    return plan_workspace(Ns, Nt, d, 0, r_max, n_fp, n_fp > 0).total;
 }
 int ul_destroy(ul_ctx* c) {
     if (!c) return UL_OK;
@@ -520,6 +528,73 @@ int ul_multilevel(ul_ctx* c, int d, int n_sub, int r_max, const int* fps, int n_
         if (rc) return rc;
     }
     return ul_measure_end(c);
+}
+
+// Single-level measurement by replay: the same estimator, trajectory and results as
+// ul_multilevel (to fp64 rounding order), with 2x the sweeps and none of the per-site TO accumulators.
+int ul_multilevel_replay(ul_ctx* c, int d, int n_sub, int r_max, const int* fps, int n_fp) {
+    if (!c || n_sub < 0) return fail(c, UL_EINVAL, "n_sub must be >= 0");
+    if (n_fp == 0) return ul_multilevel(c, d, n_sub, r_max, fps, n_fp);                  // nothing is linear in O: nothing to replay
+    int rc = check_meas_args(c, d, r_max, fps, n_fp);
+    if (rc) return rc;
+    rc = ensure_staging(c);
+    if (rc) return rc;
+    const size_t link_bytes = sizeof(float) * 4 * (size_t)c->V;
+    UL_CUDA(c, cudaMemcpyAsync(c->staging, c->th, link_bytes, cudaMemcpyDeviceToDevice, c->stream));   // start configuration
+    const uint64_t sweep0 = c->sweep;
+    c->replay = true;
+    rc = open_measurement(c, d, 0, r_max, fps, n_fp);
+    if (rc) { c->replay = false; return rc; }
+    auto bail = [&](int code) { c->replay = false; c->open = false; return code; };
+    // pass 1: sums of T only
+    if (n_sub == 0) { rc = accumulate(c); if (rc) return bail(rc); }
+    for (int j = 0; j < n_sub; ++j) {
+        for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d); if (rc) return bail(rc); }
+        rc = accumulate(c);
+        if (rc) return bail(rc);
+    }
+    rc = flush(c);
+    if (rc) return bail(rc);
+    const double inv = 1.0 / (double)c->n_acc;
+    ulk::WeightArgs wa;
+    wa.Vs = c->Vs; wa.r_max = r_max; wa.n_slab = c->n_slab; wa.inv = inv;
+    wa.A = wsp<double2>(c, c->ws.A2); wa.W = wsp<double2>(c, c->ws.B2);
+    const long long nw = 3LL * r_max * c->Vs;
+    ulk::k_slab_weights<<<(unsigned)((nw + 255) / 256), 256, 0, c->stream>>>(wa);
+    if (cudaGetLastError() != cudaSuccess) return bail(fail(c, UL_ECUDA, "k_slab_weights launch"));
+    c->launches += 1;
+    // pass 2: the same trajectory again, fields reduced on the fly
+    if (n_sub > 0) {
+        if (cudaMemcpyAsync(c->th, c->staging, link_bytes, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return bail(fail(c, UL_ECUDA, "restore links"));
+        c->sweep = sweep0;
+    }
+    const long long n = (long long)c->n_slab * c->Vs;
+    const int n_entries = r_max * (1 + 12 * n_fp);
+    double* res = wsp<double>(c, c->ws.result);
+    ulk::TableArgs t;
+    t.g = geom(c); t.th = c->th; t.d = c->d; t.n_slab = c->n_slab;
+    t.U = wsp<double2>(c, c->ws.U); t.Ot = wsp<float>(c, c->ws.Ot); t.partial = wsp<double>(c, c->ws.partial);
+    ulk::ReplayArgs ra;
+    ra.g = geom(c); ra.n_slab = c->n_slab; ra.r_max = r_max; ra.n_fp = n_fp;
+    ra.U = t.U; ra.Ot = t.Ot; ra.fps = wsp<int>(c, c->ws.fps); ra.W = wa.W; ra.partial = wsp<double>(c, c->ws.partial);
+    const int gx = (c->Ns * c->Ns + 255) / 256, rows = c->n_slab * c->Ns;
+    const int gy = rows < TBLK / gx ? rows : (TBLK / gx > 0 ? TBLK / gx : 1);
+    // blocks per (r, field point): >= 16 sites per thread and direction, so that the 24-value block reduction is amortised
+    int nb = (int)(n / (256 * 16));
+    nb = nb < 1 ? 1 : (nb > NBLK ? NBLK : nb);
+    const double scale = inv / (3.0 * (double)c->Vs * (double)c->Nt);                    // Eq. 34 normalisation and 1/n_sub
+    for (int j = 0; j < (n_sub > 0 ? n_sub : 1); ++j) {
+        if (n_sub > 0)
+            for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d); if (rc) return bail(rc); }
+        ulk::k_slab_tables<<<dim3(gx, gy), 256, 0, c->stream>>>(t);                      // column sums were taken in pass 1
+        ulk::k_replay_reduce<<<dim3(nb, r_max * n_fp), 256, 0, c->stream>>>(ra);
+        ulk::k_sum_partials<<<2 * (n_entries - r_max), 256, 0, c->stream>>>(ra.partial + (size_t)2 * r_max * nb, nb, res + 2 * r_max, scale, 1);
+        if (cudaGetLastError() != cudaSuccess) return bail(fail(c, UL_ECUDA, "replay pass launch"));
+        c->launches += 3;
+    }
+    rc = finish(c, wsp<double2>(c, c->ws.A2), nullptr, c->n_slab, inv, inv);
+    c->replay = false;
+    return rc;
 }
 
 int ul_multilevel2(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, int r_max, const int* fps, int n_fp) {

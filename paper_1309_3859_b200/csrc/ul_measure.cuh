@@ -417,14 +417,14 @@ __global__ void __launch_bounds__(256, FIELD ? 1 : UL_ACC_MINB) k_accumulate(con
 #pragma unroll
                 for (int k = 0; k < KB; ++k)
                     if (FULL || k < P.nk) {
-                        if (FIELD) {
+                        if (FIELD) {                               // T itself is needed for the TO sums
                             T[k].x = fma(v[k].x, u0[k].x, v[k].y * u0[k].y);
                             T[k].y = fma(v[k].y, u0[k].x, -(v[k].x * u0[k].y));
-                            a[i].x += T[k].x; a[i].y += T[k].y;
-                        } else {                                   // the same term folded into the sum: 4 DFMA instead of 6 ops
-                            a[i].x = fma(v[k].y, u0[k].y, fma(v[k].x, u0[k].x, a[i].x));
-                            a[i].y = fma(-v[k].x, u0[k].y, fma(v[k].y, u0[k].x, a[i].y));
                         }
+                        // the term folded into the sum (4 DFMA); the same arithmetic with and without field points,
+                        // so the slab sums of T do not depend on what else is measured
+                        a[i].x = fma(v[k].y, u0[k].y, fma(v[k].x, u0[k].x, a[i].x));
+                        a[i].y = fma(-v[k].x, u0[k].y, fma(v[k].y, u0[k].x, a[i].y));
                     }
                 __stcs(Ap + i * stepA, a[i]);
                 if (FIELD) {
@@ -573,6 +573,102 @@ __global__ void __launch_bounds__(256) k_slab_product(const ReduceArgs P, int o_
     if (threadIdx.x == 0) {
         P.partial[(long long)(2 * o) * gridDim.x + blockIdx.x] = v[0];
         P.partial[(long long)(2 * o + 1) * gridDim.x + blockIdx.x] = v[1];
+    }
+}
+
+// ---------------------------------------------------------------- replay estimator of the field correlators
+// The estimator G(r,fp,ch) = (1/(3 Vs Nt)) sum_{x,mu,s} [TO](x,s) prod_{s' != s} [T](x,s')  (Eq. 34) is linear
+// in O, and the sub-update trajectory can be replayed bit for bit (counter-based RNG).  Pass 1 accumulates only the
+// sums of T; k_slab_weights turns them into W(x,s,mu,r) = prod_{s' != s} [T](x,s'); pass 2 replays the sub-updates and
+// k_replay_reduce adds sum_{x,mu,s} W T_j sum_{t in slab} O_ch(x + off) of every configuration j straight into
+// lattice sums: no per-site TO accumulators (12 n_fp times the memory and traffic of the T accumulators).
+struct WeightArgs {
+    long long Vs;
+    int r_max, n_slab;
+    double inv;           // 1 / n_sub
+    const double2* A;     // sums of T, [mu][r][s][xs]
+    double2* W;           // out, same layout
+};
+__global__ void __launch_bounds__(256) k_slab_weights(const WeightArgs P) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;            // over (mu, r, xs)
+    if (idx >= 3LL * P.r_max * P.Vs) return;
+    const long long mr = idx / P.Vs, xs = idx - mr * P.Vs;
+    const double2* Ap = P.A + mr * P.n_slab * P.Vs + xs;
+    double2* Wp = P.W + mr * P.n_slab * P.Vs + xs;
+    double2 run = make_double2(1.0, 0.0);
+    for (int s = 0; s < P.n_slab; ++s) {                                                // prefix products
+        Wp[(long long)s * P.Vs] = run;
+        double2 a = Ap[(long long)s * P.Vs];
+        a.x *= P.inv; a.y *= P.inv;
+        run = cmul(run, a);
+    }
+    run = make_double2(1.0, 0.0);
+    for (int s = P.n_slab - 1; s >= 0; --s) {                                           // times suffix products
+        Wp[(long long)s * P.Vs] = cmul(Wp[(long long)s * P.Vs], run);
+        double2 a = Ap[(long long)s * P.Vs];
+        a.x *= P.inv; a.y *= P.inv;
+        run = cmul(run, a);
+    }
+}
+
+struct ReplayArgs {
+    Geom g;
+    int n_slab, r_max, n_fp;
+    const double2* U;     // [n_slab*Vs]  this configuration
+    const float* Ot;      // [12][n_slab*Vs]
+    const int* fps;
+    const double2* W;
+    double* partial;      // [(2*o + reim)*gridDim.x + b], o = r_max + ((r-1)*n_fp + fp)*12 + ch  (the layout of k_slab_product)
+};
+// grid (nblk, r_max * n_fp): block (b, e) sums its share of the sites for separation r = e / n_fp + 1, field point e % n_fp
+__global__ void __launch_bounds__(256) k_replay_reduce(const ReplayArgs P) {
+    __shared__ double sm[24 * 32];
+    const Geom& g = P.g;
+    const int Ns = g.Ns;
+    const int r = blockIdx.y / P.n_fp + 1, fp = blockIdx.y - (r - 1) * P.n_fp;
+    const long long n = (long long)P.n_slab * g.Vs;
+    const int fa = P.fps[3 * fp], fb = P.fps[3 * fp + 1], fc = P.fps[3 * fp + 2];
+    double acc[24];
+#pragma unroll
+    for (int i = 0; i < 24; ++i) acc[i] = 0.0;
+    const int stride[4] = {0, 1, Ns, Ns * Ns};
+#pragma unroll
+    for (int mu = 1; mu <= 3; ++mu) {
+        const int nu = 1 + (mu % 3), rho = 1 + ((mu + 1) % 3);
+        const double2* Wm = P.W + ((long long)(mu - 1) * P.r_max + (r - 1)) * n;
+        for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) {
+            const int s = (int)(j / g.Vs);
+            const int xs = (int)(j - (long long)s * g.Vs);
+            int x[4] = {0, xs % Ns, (xs / Ns) % Ns, xs / (Ns * Ns)};
+            const int ys = xs + (wrapc(x[mu] + r, Ns) - x[mu]) * stride[mu];
+            const double2 u = P.U[j], v = P.U[(long long)s * g.Vs + ys], w = Wm[j];
+            const double2 T = make_double2(fma(v.x, u.x, v.y * u.y), fma(v.y, u.x, -(v.x * u.y)));   // U(x + r mu) conj U(x)
+            const double2 Z = cmul(w, T);
+            int z[4] = {0, x[1], x[2], x[3]};
+            z[mu] = modc(z[mu] + r / 2 + fa, Ns);                                        // anchor, DESIGN R10
+            z[nu] = modc(z[nu] + fb, Ns);
+            z[rho] = modc(z[rho] + fc, Ns);
+            const long long zs = z[1] + (long long)Ns * (z[2] + (long long)Ns * z[3]) + (long long)s * g.Vs;
+#pragma unroll
+            for (int comp = 0; comp < 6; ++comp) {
+                int pa, pb, o;
+                float sgn;
+                comp_dirs(mu, comp, pa, pb);
+                orient_of(pa, pb, o, sgn);
+                const double Oc = (double)P.Ot[(long long)(2 * o) * n + zs];
+                const double Os = (double)(sgn * P.Ot[(long long)(2 * o + 1) * n + zs]);
+                acc[4 * comp + 0] = fma(Z.x, Oc, acc[4 * comp + 0]);
+                acc[4 * comp + 1] = fma(Z.y, Oc, acc[4 * comp + 1]);
+                acc[4 * comp + 2] = fma(Z.x, Os, acc[4 * comp + 2]);
+                acc[4 * comp + 3] = fma(Z.y, Os, acc[4 * comp + 3]);
+            }
+        }
+    }
+    block_sum<24>(acc, sm);
+    if (threadIdx.x == 0) {
+        const long long o0 = P.r_max + ((long long)(r - 1) * P.n_fp + fp) * 12;          // ch = 2 comp + kind; acc = [ch][reim]
+#pragma unroll
+        for (int i = 0; i < 24; ++i) P.partial[(2 * (o0 + i / 2) + (i & 1)) * gridDim.x + blockIdx.x] = acc[i];
     }
 }
 

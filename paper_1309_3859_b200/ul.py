@@ -18,7 +18,7 @@ UL_OK, UL_EINVAL, UL_ENOMEM, UL_ECUDA, UL_ESTATE = 0, -1, -2, -3, -4
 SYMBOLS = [
     "ul_create", "ul_create_ext", "ul_workspace_bytes", "ul_destroy", "ul_init", "ul_set_beta",
     "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep",
-    "ul_set_subupdate", "ul_set_update_algorithm", "ul_multilevel", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
+    "ul_set_subupdate", "ul_set_update_algorithm", "ul_multilevel", "ul_multilevel_replay", "ul_workspace_bytes_replay", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
     "ul_measure_end", "ul_set_accum_batch", "ul_plaquette", "ul_polyakov", "ul_read_correlators", "ul_read_slab_averages",
     "ul_get_launch_count", "ul_philox_selftest", "ul_sync", "ul_last_error",
 ]
@@ -61,6 +61,9 @@ def lib():
         L.ul_set_update_algorithm.argtypes = [P, C.c_int, C.c_double]
         L.ul_multilevel.argtypes = [P, C.c_int, C.c_int, C.c_int, P, C.c_int]
         L.ul_multilevel2.argtypes = [P, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, P, C.c_int]
+        L.ul_multilevel_replay.argtypes = [P, C.c_int, C.c_int, C.c_int, P, C.c_int]
+        L.ul_workspace_bytes_replay.argtypes = [C.c_int] * 5
+        L.ul_workspace_bytes_replay.restype = C.c_size_t
         L.ul_measure_begin.argtypes = [P, C.c_int, C.c_int, P, C.c_int]
         L.ul_set_accum_batch.argtypes = [P, C.c_int]
         L.ul_polyakov.argtypes = [P, C.c_int, P]
@@ -89,6 +92,10 @@ def _fps(field_points):
 
 def workspace_bytes(Ns, Nt, d_in, d_out, r_max, n_fp):
     return int(lib().ul_workspace_bytes(int(Ns), int(Nt), int(d_in), int(d_out), int(r_max), int(n_fp)))
+
+
+def workspace_bytes_replay(Ns, Nt, d, r_max, n_fp):
+    return int(lib().ul_workspace_bytes_replay(int(Ns), int(Nt), int(d), int(r_max), int(n_fp)))
 
 
 def philox_selftest(ctr, key):
@@ -206,6 +213,11 @@ class Lattice:
     def multilevel(self, slab_thickness, n_sub, r_max, field_points=None):
         fp, n = _fps(field_points)
         self._ck(lib().ul_multilevel(self._h, int(slab_thickness), int(n_sub), int(r_max), _ptr(fp), n))
+        self._meas = (int(r_max), n, self.Nt // int(slab_thickness))
+
+    def multilevel_replay(self, slab_thickness, n_sub, r_max, field_points=None):
+        fp, n = _fps(field_points)
+        self._ck(lib().ul_multilevel_replay(self._h, int(slab_thickness), int(n_sub), int(r_max), _ptr(fp), n))
         self._meas = (int(r_max), n, self.Nt // int(slab_thickness))
 
     def multilevel2(self, d_in, n_in, d_out, n_out, r_max, field_points=None):

@@ -748,3 +748,59 @@ def test_polyakov_full_size_64(ul, ulo):
     g.init(0)
     r = special.ive(1, 6 * 0.98) / special.ive(0, 6 * 0.98)
     assert abs(g.polyakov(1) - r ** Nt) < 1e-12 * r ** Nt + 1e-18
+
+
+# ----------------------------------------------------------------------------- replay estimator (next row)
+@pytest.mark.parametrize("Ns,Nt,d,n_sub", [(4, 4, 2, 5), (8, 4, 2, 9), (8, 8, 4, 3), (6, 4, 1, 2)])
+def test_replay_equals_stored_accumulators(ul, Ns, Nt, d, n_sub):
+    """ul_multilevel_replay: the same trajectory (bit-identical final links and counter), the same correlators
+    bit for bit, the same field values and vacuum to fp64 rounding order, as the stored-accumulator path."""
+    R = min(3, Ns // 2)
+    res = []
+    for mode in ("stored", "replay"):
+        g = ul.Lattice(Ns, Nt, 0.99, 31)
+        g.sweep(3, 2)
+        (g.multilevel if mode == "stored" else g.multilevel_replay)(d, n_sub, R, FPS)
+        res.append((g.get_links_raw(), g.get_counter(), g.read_slab_averages()) + tuple(g.read_correlators()))
+    a, b = res
+    assert np.array_equal(a[0], b[0]) and a[1] == b[1]
+    assert np.array_equal(a[2], b[2]) and np.array_equal(a[3], b[3]) and np.array_equal(a[5], b[5])
+    scale = np.abs(a[4]).max()
+    assert scale > 0 and np.abs(a[4] - b[4]).max() <= 1e-12 * max(scale, 1e-3)
+
+
+def test_replay_frozen_configuration_against_oracle(ul, ulo):
+    """P2 for the replay path: n_sub = 0 on an oracle configuration, fields and correlators to relative 1e-5."""
+    Ns, Nt, d, R = 8, 4, 2, 4
+    o = ulo.Oracle(Ns, Nt, 0.99, 4)
+    for _ in range(10):
+        o.sweep(1, 3)
+    g = ul.Lattice(Ns, Nt, 0.99, 4)
+    g.set_links(o.get_links())
+    o.multilevel(d, 0, R, FPS)
+    g.multilevel_replay(d, 0, R, FPS)
+    co, fo, vo = o.read_correlators()
+    cg, fg, vg = g.read_correlators()
+    Vs = Ns ** 3
+    for got, want, n in ((cg, co, 3 * Vs), (fg, fo, 3 * Vs * Nt), (vg, vo, 3 * Vs * Nt)):
+        ok, worst = rel_ok(got, want, n)
+        assert ok, worst
+
+
+def test_replay_config3_memory_and_agreement(ul):
+    """BJ config 3 shape (24^3 x 8, r <= 12, mid-plane offsets 0..10 and on-axis points): the replay workspace is
+    ~40x smaller than the stored accumulators, and both give the same numbers from the same start."""
+    Ns, Nt, d, R = 24, 8, 2, 12
+    fps = [(0, b, 0) for b in range(11)] + [(a, 0, 0) for a in (-2, -1, 1, 2)]
+    big, small = ul.workspace_bytes(Ns, Nt, d, 0, R, len(fps)), ul.workspace_bytes_replay(Ns, Nt, d, R, len(fps))
+    assert big > 30 * small
+    out = []
+    for mode in ("stored", "replay"):
+        g = ul.Lattice(Ns, Nt, 1.0, 3)
+        g.init(0)
+        for _ in range(30):
+            g.sweep(1, 3)
+        (g.multilevel if mode == "stored" else g.multilevel_replay)(d, 4, R, fps)
+        out.append(g.read_correlators())
+    assert np.array_equal(out[0][0], out[1][0])
+    assert np.abs(out[0][1] - out[1][1]).max() <= 1e-12 * np.abs(out[0][1]).max()
