@@ -31,6 +31,13 @@ struct Workspace {           // byte offsets into the measurement workspace
 
 size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
 
+// blocks per (r, field point) of k_replay_reduce: >= 16 sites per thread and direction, so that the 24-value block
+// reduction is amortised
+int replay_blocks(long long n_slab_sites) {
+    const long long nb = n_slab_sites / (256 * 16);
+    return nb < 1 ? 1 : (nb > NBLK ? NBLK : (int)nb);
+}
+
 Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_fp, bool replay = false) {
     Workspace w;
     const size_t Vs = (size_t)Ns * Ns * Ns;
@@ -55,7 +62,13 @@ Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_f
     const size_t n_entries = R * (1 + F12);
     size_t np = 2 * n_entries;
     if (np < 12 * (TBLK / NBLK)) np = 12 * (TBLK / NBLK);
-    w.partial = o; o = align_up(o + np * NBLK * sizeof(double));
+    size_t partial_doubles = np * NBLK;
+    if (replay) {                                   // fields: replay_blocks() partials per entry; correlators: NBLK per entry
+        const size_t nb = replay_blocks((long long)(n_in * Vs));
+        partial_doubles = 2 * R * NBLK + 2 * R * F12 * nb;
+        if (partial_doubles < (size_t)12 * TBLK) partial_doubles = (size_t)12 * TBLK;
+    }
+    w.partial = o; o = align_up(o + partial_doubles * sizeof(double));
     w.result = o;  o = align_up(o + (2 * n_entries + 12 + 12) * sizeof(double));   // corr|field, vacuum, column sums
     w.total = o;
     return w;
@@ -579,9 +592,7 @@ int ul_multilevel_replay(ul_ctx* c, int d, int n_sub, int r_max, const int* fps,
     ra.U = t.U; ra.Ot = t.Ot; ra.fps = wsp<int>(c, c->ws.fps); ra.W = wa.W; ra.partial = wsp<double>(c, c->ws.partial);
     const int gx = (c->Ns * c->Ns + 255) / 256, rows = c->n_slab * c->Ns;
     const int gy = rows < TBLK / gx ? rows : (TBLK / gx > 0 ? TBLK / gx : 1);
-    // blocks per (r, field point): >= 16 sites per thread and direction, so that the 24-value block reduction is amortised
-    int nb = (int)(n / (256 * 16));
-    nb = nb < 1 ? 1 : (nb > NBLK ? NBLK : nb);
+    const int nb = replay_blocks(n);
     const double scale = inv / (3.0 * (double)c->Vs * (double)c->Nt);                    // Eq. 34 normalisation and 1/n_sub
     for (int j = 0; j < (n_sub > 0 ? n_sub : 1); ++j) {
         if (n_sub > 0)

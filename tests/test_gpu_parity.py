@@ -804,3 +804,27 @@ def test_replay_config3_memory_and_agreement(ul):
         out.append(g.read_correlators())
     assert np.array_equal(out[0][0], out[1][0])
     assert np.abs(out[0][1] - out[1][1]).max() <= 1e-12 * np.abs(out[0][1]).max()
+
+
+def test_replay_full_mid_plane_against_oracle(ul, ulo):
+    """A FULL mid-plane of field points (all 64 transverse offsets of an 8^3 x 4 lattice, 12 channels, r = 1..4):
+    the map BJ config 4 asks for, at a size where the oracle's stored accumulators still fit; frozen
+    configuration, relative 1e-5 (DESIGN R17)."""
+    Ns, Nt, d, R = 8, 4, 2, 4
+    fps = [(0, b, c) for c in range(Ns) for b in range(Ns)]
+    o = ulo.Oracle(Ns, Nt, 1.0, 9)
+    for _ in range(12):
+        o.sweep(1, 3)
+    g = ul.Lattice(Ns, Nt, 1.0, 9)
+    g.set_links(o.get_links())
+    o.multilevel(d, 0, R, fps)
+    g.multilevel_replay(d, 0, R, fps)
+    co, fo, vo = o.read_correlators()
+    cg, fg, vg = g.read_correlators()
+    Vs = Ns ** 3
+    for got, want, n in ((cg, co, 3 * Vs), (fg, fo, 3 * Vs * Nt), (vg, vo, 3 * Vs * Nt)):
+        ok, worst = rel_ok(got, want, n)
+        assert ok, worst
+    assert ul.workspace_bytes(Ns, Nt, d, 0, R, len(fps)) > 100 * ul.workspace_bytes_replay(Ns, Nt, d, R, len(fps))
+    g.multilevel_replay(d, 3, R, fps)                               # and a short run through the sub-updates
+    assert np.all(np.isfinite(g.read_correlators()[1]))
