@@ -8,7 +8,6 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -338,10 +337,7 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     *h = nullptr;
     if (Ns < 2 || Nt < 2 || (Ns & 1) || (Nt & 1) || !(beta >= 0.0)) return fail(nullptr, UL_EINVAL, "need even Ns, Nt >= 2 and beta >= 0");
     const int Nh = Ns / 2;
-    int vec = (Nh % 4 == 0) ? 4 : ((Nh % 2 == 0) ? 2 : 1);
-#ifdef UL_DBG_VEC
-    if (vec > UL_DBG_VEC) vec = UL_DBG_VEC;
-#endif
+    const int vec = (Nh % 4 == 0) ? 4 : ((Nh % 2 == 0) ? 2 : 1);
     if (Nh / vec > 128 || 4.0 * (double)Ns * Ns * Ns * Nt >= 2147483648.0) return fail(nullptr, UL_EINVAL, "lattice too large for this build");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(nullptr, UL_ECUDA, "no CUDA device");
@@ -378,9 +374,6 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     if (cudaMalloc(&q, (sizeof(int4) * ulk::HB_QSEG + sizeof(int)) * (size_t)c->hb_qblocks) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ENOMEM, "cudaMalloc straggler queue"); }
     c->hb_queue = (int4*)q;
     c->hb_qcount = (int*)(c->hb_queue + (size_t)ulk::HB_QSEG * c->hb_qblocks);
-#ifdef UL_DBG_TUNE
-    if (const char* ev = getenv("UL_HB_LOCAL_ROUNDS")) c->hb_local_rounds = atoi(ev);
-#endif
     *h = c;
     const int rc = ul_init(c, 1);
     if (rc) { g_err = c->err; ul_destroy(c); *h = nullptr; }

@@ -95,24 +95,6 @@ __device__ __forceinline__ void staple_pair(const int* __restrict__ th, int Vh, 
     }
 }
 
-template <int MU, int NU, int VEC, int OFF>
-__device__ __forceinline__ void staple_angles(const int* __restrict__ th, int Vh, int p, const Site& st, int Pa[VEC], int Qa[VEC]) {
-    constexpr int m1 = (MU == 1), n1 = (NU == 1);
-    const int a_nu_p = (NU * 2 + p) * Vh, a_nu_q = (NU * 2 + 1 - p) * Vh, a_mu_q = (MU * 2 + 1 - p) * Vh;
-    int A[VEC], B[VEC], C[VEC], D[VEC], E[VEC], F[VEC];
-    load_row<VEC, 0, OFF>(th, a_nu_p + st.e0, st, A);
-    load_row<VEC, n1, OFF>(th, a_mu_q + st.e0 + st.dp[NU], st, B);
-    load_row<VEC, m1, OFF>(th, a_nu_q + st.e0 + st.dp[MU], st, C);
-    load_row<VEC, m1 - n1, OFF>(th, a_nu_p + st.e0 + st.dp[MU] + st.dm[NU], st, D);
-    load_row<VEC, -n1, OFF>(th, a_mu_q + st.e0 + st.dm[NU], st, E);
-    load_row<VEC, -n1, OFF>(th, a_nu_q + st.e0 + st.dm[NU], st, F);
-#pragma unroll
-    for (int i = 0; i < VEC; ++i) {
-        Pa[i] = (int)((unsigned)A[i] + (unsigned)B[i] - (unsigned)C[i]);
-        Qa[i] = (int)((unsigned)D[i] + (unsigned)E[i] - (unsigned)F[i]);
-    }
-}
-
 template <typename T, int VEC>
 __device__ __forceinline__ T pick(const T v[VEC], int j) {        // v[j] without dynamic register indexing
     T r = v[0];
@@ -128,20 +110,9 @@ template <int MU, int VEC, int OFF>
 __device__ __forceinline__ void gather_staples(const UpdateArgs& P, const Site& st, float Sx[VEC], float Sy[VEC]) {
 #pragma unroll
     for (int i = 0; i < VEC; ++i) { Sx[i] = 0.0f; Sy[i] = 0.0f; }
-#ifdef UL_LOADS_FIRST
-    int Pa[3][VEC], Qa[3][VEC];
-    staple_angles<MU, (MU + 1) & 3, VEC, OFF>(P.th, P.Vh, P.parity, st, Pa[0], Qa[0]);
-    staple_angles<MU, (MU + 2) & 3, VEC, OFF>(P.th, P.Vh, P.parity, st, Pa[1], Qa[1]);
-    staple_angles<MU, (MU + 3) & 3, VEC, OFF>(P.th, P.Vh, P.parity, st, Pa[2], Qa[2]);
-#pragma unroll
-    for (int j = 0; j < 3; ++j)
-#pragma unroll
-        for (int i = 0; i < VEC; ++i) ulm::cis_pair_accumulate(Pa[j][i], Qa[j][i], Sx[i], Sy[i]);
-#else
     staple_pair<MU, (MU + 1) & 3, VEC, OFF>(P.th, P.Vh, P.parity, st, Sx, Sy);
     staple_pair<MU, (MU + 2) & 3, VEC, OFF>(P.th, P.Vh, P.parity, st, Sx, Sy);
     staple_pair<MU, (MU + 3) & 3, VEC, OFF>(P.th, P.Vh, P.parity, st, Sx, Sy);
-#endif
 }
 
 // The update proper from the staple sums.  KIND 0 = heatbath, 1 = overrelaxation.
