@@ -169,6 +169,20 @@ int ul_plaquette(ul_ctx* h, double* mean_cos);
  * UL_EINVAL: multihit not 0 or 1, null pointer. */
 int ul_polyakov(ul_ctx* h, int multihit, double* mean_P);
 
+/* ---- slab sharding over GPUs -------------------------
+ * While the boundary layers are frozen the slabs are dynamically independent, so a lattice can be cut
+ * in t into shards of whole slabs, one ul_ctx per GPU, with NO communication inside the sub-update loop:
+ * a shard is a lattice of Nt_loc + d time layers whose last slab is a ghost (its first layer holds a copy
+ * of the next shard's frozen spatial links; nothing a shard owns depends on the rest of the ghost slab).
+ * ul_set_site_offset makes the Philox counters those of the global lattice (offset = t0 * Ns^3 added to
+ * the local site index; offset + local volume <= 2^29), so a sharded run reproduces the unsharded one bit
+ * for bit.  ul_slab_partial_product writes prod_{s_begin <= s < s_end} [T](x,s) of the last measurement
+ * to a DEVICE buffer double[3][r_max][Ns^3][2] (caller-owned, e.g. a torch tensor): the one array the
+ * shards exchange (all-gather) before the slab product of row a10.  paper_1309_3859_b200/sharded.py holds
+ * the partition arithmetic and the exchange over torch.distributed. */
+int ul_set_site_offset(ul_ctx* h, uint64_t offset);
+int ul_slab_partial_product(ul_ctx* h, int s_begin, int s_end, void* dev_out);
+
 /* Results of the last measurement, HOST buffers (any may be NULL):
  * corr[r_max][2]           C(r) = (1/3Ns^3) sum_x sum_mu prod_s [T](x,s,mu,r)       (re, im)
  * field[r_max][n_fp][12][2] G(r,fp,ch) of Eq. 34; ch = 2*comp + kind, comp 0..5 = plaquette

@@ -94,6 +94,7 @@ struct ul_ctx {
     int* hb_qcount = nullptr;
     int hb_qblocks = 0;
     int hb_local_rounds = 2;
+    uint32_t site_offset = 0; // ul_set_site_offset
     int alg = 0;             // ul_set_update_algorithm: 0 heatbath, 1 Metropolis for the stochastic sweeps
     double met_delta = 3.14159265358979323846;
     int vec = 1, bx = 1, by = 1, bz = 1;
@@ -175,6 +176,7 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
     a.key0 = (uint32_t)(c->seed & 0xffffffffu); a.key1 = (uint32_t)(c->seed >> 32);
     a.sweep_lo = (uint32_t)(c->sweep & 0xffffffffu); a.sweep_hi = (uint32_t)(c->sweep >> 32);
     const dim3 block(c->bx, c->by, 2 * c->bz), grid(c->Nh / c->by, c->Ns / c->bz, n_t);   // by = x2 row PAIRS per block
+    a.site_offset = c->site_offset;
     a.queue = c->hb_queue; a.qcount = c->hb_qcount; a.qblocks = (int)(grid.x * grid.y * grid.z); a.local_rounds = c->hb_local_rounds;
     if (kind == 0 && cudaMemsetAsync(c->hb_qcount, 0, sizeof(int) * (size_t)a.qblocks, c->stream) != cudaSuccess) return fail(c, UL_ECUDA, "memset straggler counters");
     {
@@ -672,6 +674,24 @@ int ul_read_slab_averages(ul_ctx* c, double* out) {
     UL_CUDA(c, cudaMemcpyAsync(out, c->res_A, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
     UL_CUDA(c, cudaStreamSynchronize(c->stream));
     for (size_t i = 0; i < n; ++i) out[i] *= c->res_inv;
+    return UL_OK;
+}
+int ul_set_site_offset(ul_ctx* c, uint64_t offset) {
+    if (!c || offset + (uint64_t)c->V > ((uint64_t)1 << 29)) return fail(c, UL_EINVAL, "site offset + local volume must be <= 2^29");
+    c->site_offset = (uint32_t)offset;
+    return UL_OK;
+}
+int ul_slab_partial_product(ul_ctx* c, int s_begin, int s_end, void* dev_out) {
+    if (!c || !dev_out) return fail(c, UL_EINVAL, "null pointer");
+    if (!c->have) return fail(c, UL_ESTATE, "no measurement yet");
+    if (s_begin < 0 || s_end > c->res_n_slab || s_begin > s_end) return fail(c, UL_EINVAL, "bad slab range");
+    ulk::WeightArgs wa;
+    wa.Vs = c->Vs; wa.r_max = c->res_r_max; wa.n_slab = c->res_n_slab; wa.inv = c->res_inv;
+    wa.A = c->res_A; wa.W = (double2*)dev_out;
+    const long long nw = 3LL * wa.r_max * c->Vs;
+    ulk::k_slab_partial_product<<<(unsigned)((nw + 255) / 256), 256, 0, c->stream>>>(wa, s_begin, s_end);
+    UL_CUDA(c, cudaGetLastError());
+    c->launches += 1;
     return UL_OK;
 }
 int ul_get_launch_count(ul_ctx* c, uint64_t* n) { if (!c || !n) return fail(c, UL_EINVAL, "null pointer"); *n = c->launches; return UL_OK; }

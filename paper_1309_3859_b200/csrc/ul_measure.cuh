@@ -611,6 +611,22 @@ __global__ void __launch_bounds__(256) k_slab_weights(const WeightArgs P) {
     }
 }
 
+// product of the slab averages [T](x,s) over the slabs s_begin <= s < s_end, per (mu, r, xs): the piece of the slab
+// product (row a10) that one shard of a t-partitioned lattice owns
+__global__ void __launch_bounds__(256) k_slab_partial_product(const WeightArgs P, int s_begin, int s_end) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;            // over (mu, r, xs)
+    if (idx >= 3LL * P.r_max * P.Vs) return;
+    const long long mr = idx / P.Vs, xs = idx - mr * P.Vs;
+    const double2* Ap = P.A + mr * P.n_slab * P.Vs + xs;
+    double2 run = make_double2(1.0, 0.0);
+    for (int s = s_begin; s < s_end; ++s) {
+        double2 a = Ap[(long long)s * P.Vs];
+        a.x *= P.inv; a.y *= P.inv;
+        run = cmul(run, a);
+    }
+    P.W[idx] = run;
+}
+
 struct ReplayArgs {
     Geom g;
     int n_slab, r_max, n_fp;

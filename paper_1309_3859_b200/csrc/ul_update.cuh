@@ -29,6 +29,7 @@ struct UpdateArgs {
     int* qcount;          // entries queued per block (zeroed before the launch); segment b = queue[b*HB_QSEG ...]
     int qblocks;          // number of segments
     int local_rounds;     // lane-local retry rounds before a link is queued
+    uint32_t site_offset; // added to the local canonical site index in the Philox counter (slab sharding: t0 * Ns^3)
     int met_delta_bt;     // Metropolis proposal half-width delta as a binary angle (0 < delta <= pi -> up to 2^31 - 1)
 };
 
@@ -138,7 +139,7 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
         if (VEC == 4) { const int4 q = *reinterpret_cast<const int4*>(own); old[0] = q.x; old[1 % VEC] = q.y; old[2 % VEC] = q.z; old[3 % VEC] = q.w; }
         else if (VEC == 2) { const int2 q = *reinterpret_cast<const int2*>(own); old[0] = q.x; old[1 % VEC] = q.y; }
         else old[0] = own[0];
-        const uint32_t site0 = (uint32_t)((st.e0 - h0) * 2 + 2 * h0 + st.off);            // canonical site index
+        const uint32_t site0 = (uint32_t)((st.e0 - h0) * 2 + 2 * h0 + st.off) + P.site_offset;            // canonical site index
         const uint32_t c3 = (3u << 3) | ((uint32_t)p << 2) | (uint32_t)MU;                // tag 3 = Metropolis, attempt 0
 #pragma unroll
         for (int i = 0; i < VEC; ++i) {
@@ -164,7 +165,7 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
         // which a thread works through its rejections is free: every link gets attempt 0 with the warp
         // converged; a lane then retries its own rejected links one at a time (lane-local queue), which
         // bounds the warp's extra rounds by the worst lane's total instead of the sum of per-link maxima.
-        const uint32_t site0 = (uint32_t)((st.e0 - h0) * 2 + 2 * h0 + st.off);            // canonical site index
+        const uint32_t site0 = (uint32_t)((st.e0 - h0) * 2 + 2 * h0 + st.off) + P.site_offset;            // canonical site index
         const uint32_t c3 = ((uint32_t)p << 2) | (uint32_t)MU;                            // tag 0 = heatbath
         float pa[VEC], pq[VEC], pc[VEC], sn[VEC], cs[VEC];
         uint32_t pend = 0u, neg = 0u, tries = 0u, zero = 0u;                              // tries: 8 bits per link

@@ -1,0 +1,163 @@
+"""Slab sharding of ONE lattice over GPUs for the multilevel sub-update loop.
+
+While the spatial links of the boundary layers t = 0 mod d are frozen, the time slabs are dynamically
+independent ("hold their spatial links constant [and] isolate the dynamics of the sublattice from the
+rest of the lattice"), so the lattice is cut in t into shards of whole slabs, one process and one ul_ctx per GPU:
+
+  * a shard is a lattice of nt_loc + ghost time layers; its last slab is a ghost whose first layer carries a copy
+    of the next shard's frozen spatial links, which is all the last own temporal links need; nothing a shard owns
+    depends on the rest of the ghost slab (its links move, harmlessly);
+  * ul_set_site_offset(t0 Ns^3) makes the Philox counters those of the global lattice, so a sharded run
+    reproduces the unsharded trajectory of the own layers bit for bit (tested on one GPU, shard after shard);
+  * the sub-update loop (masked sweeps + accumulation) needs NO communication;
+  * one exchange per measurement: every rank forms prod_{own slabs} [T](x,s) on its device
+    (ul_slab_partial_product) and the ranks all-gather these arrays (torch.distributed: NCCL on GPUs, gloo in the
+    CPU tests), multiply them in rank order and average over the lattice: row a10, Eq. 24.
+
+This module holds the partition arithmetic and that exchange; every arithmetic step of the method still runs in
+the CUDA kernels.  Full (unmasked) sweeps would need a halo layer per sub-step and are not sharded here.
+"""
+import numpy as np
+
+
+def partition(Nt, d, world):
+    """[(t0, nt_loc)] per rank: whole slabs of thickness d, as even as possible, in t order."""
+    if d < 1 or Nt % d != 0:
+        raise ValueError("Nt must be a multiple of the slab thickness")
+    n_slab = Nt // d
+    if world < 1 or n_slab < world:
+        raise ValueError("need at least one slab per rank")
+    base, extra = divmod(n_slab, world)
+    out, t0 = [], 0
+    for r in range(world):
+        n = (base + (1 if r < extra else 0)) * d
+        if t0 % 2:
+            raise ValueError("shards must start on an even time layer (the checkerboard parity is global)")
+        out.append((t0, n))
+        t0 += n
+    return out
+
+
+def ghost_layers(nt_loc, d):
+    """Thickness of the ghost slab(s): a multiple of d that keeps the local time extent even."""
+    g = d
+    while (nt_loc + g) % 2:
+        g += d
+    return g
+
+
+def shard_links(links, t0, nt_loc, d):
+    """Canonical global links [4][Nt][Ns][Ns][Ns] -> the shard's [4][nt_loc + ghost][...]: own layers, then the
+    layers that follow them in the global lattice (periodic in t)."""
+    Nt = links.shape[1]
+    t = (t0 + np.arange(nt_loc + ghost_layers(nt_loc, d))) % Nt
+    return np.ascontiguousarray(links[:, t])
+
+
+def unshard_links(shards, parts):
+    """Own layers of every shard back into one canonical global array."""
+    return np.concatenate([s[:, :n] for s, (_, n) in zip(shards, parts)], axis=1)
+
+
+def combine_partial_products(local, dist=None, gathered=None):
+    """local: complex128 tensor [3][r_max][Ns^3] = product of the own slab averages.  All-gathers over the ranks
+    (or takes `gathered`, the list in rank order, when the caller already holds it), multiplies in rank order
+    and returns (C(r) = lattice and direction average, Eq. 26, as a numpy array; the full product)."""
+    import torch
+    if gathered is None:
+        if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+            parts = [torch.empty_like(local) for _ in range(dist.get_world_size())]
+            re = [torch.view_as_real(p) for p in parts]                    # collectives on real views: every backend has them
+            dist.all_gather(re, torch.view_as_real(local.contiguous()))
+            gathered = parts
+        else:
+            gathered = [local]
+    full = gathered[0].clone()
+    for p in gathered[1:]:
+        full = full * p
+    return full.mean(dim=(0, 2)).cpu().numpy(), full
+
+
+class ShardedLattice:
+    """One rank's shard.  `links`: canonical global configuration (the same on every rank); `counter`: the global
+    sweep counter.  After multilevel(), correlators() returns the global C(r)."""
+
+    def __init__(self, Ns, Nt, beta, seed, d, rank, world, links, counter=0, device="cuda:0", workspace_bytes=0):
+        from . import ul
+        self.parts = partition(Nt, d, world)
+        self.t0, self.nt_loc = self.parts[rank]
+        self.d, self.Ns, self.Nt, self.rank, self.world = d, Ns, Nt, rank, world
+        self.ghost = ghost_layers(self.nt_loc, d)
+        self.lat = ul.Lattice(Ns, self.nt_loc + self.ghost, beta, seed, workspace_bytes=workspace_bytes, device=device)
+        self.lat.set_site_offset(self.t0 * Ns ** 3)
+        self.lat.set_links(shard_links(links, self.t0, self.nt_loc, d))
+        self.lat.set_counter(counter)
+
+    def multilevel(self, n_sub, r_max):
+        """The sub-update loop and the accumulation on the own slabs: no communication."""
+        self.lat.multilevel(self.d, n_sub, r_max)
+
+    def own_slab_averages(self):
+        return self.lat.read_slab_averages()[:, :, : self.nt_loc // self.d]
+
+    def partial_product(self):
+        return self.lat.slab_partial_product(0, self.nt_loc // self.d)
+
+    def correlators(self, dist=None):
+        return combine_partial_products(self.partial_product(), dist)[0]
+
+    def own_links(self):
+        return self.lat.get_links()[:, : self.nt_loc]
+
+
+def main():
+    """torchrun entry: `python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1
+    -m paper_1309_3859_b200.sharded [Ns Nt d n_sub r_max]`: one shard per GPU, times the communication-free
+    sub-update loop (max over ranks) and the one exchange, prints C(r) on rank 0."""
+    import os
+    import sys
+    import torch
+    import torch.distributed as dist
+    from . import build, ul
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    Ns, Nt, d, n_sub, r_max = [int(v) for v in sys.argv[1:6]] if len(sys.argv) >= 6 else (32, 32, 2, 20, 8)
+    if rank == 0:
+        build.build()
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist.barrier()
+    # the same global start on every rank: a hot start of the global lattice cannot be drawn shard by shard
+    # through ul_create (its counters are local), so rank 0's configuration is broadcast once
+    if rank == 0:
+        g = ul.Lattice(Ns, Nt, 1.0, 4, device=f"cuda:{local}")
+        for _ in range(20):
+            g.sweep(1, 3)
+        links, ctr = torch.from_numpy(g.get_links()).cuda(), g.get_counter()
+        del g
+    else:
+        links, ctr = torch.empty((4, Nt, Ns, Ns, Ns), dtype=torch.float32, device="cuda"), 20
+    if world > 1:
+        dist.broadcast(links, 0)
+    sh = ShardedLattice(Ns, Nt, 1.0, 4, d, rank, world, links.cpu().numpy(), ctr, device=f"cuda:{local}")
+    torch.cuda.synchronize()
+    e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+    e0.record()
+    sh.multilevel(n_sub, r_max)
+    e1.record()
+    C = sh.correlators(dist if world > 1 else None)
+    e2.record()
+    torch.cuda.synchronize()
+    t = torch.tensor([e0.elapsed_time(e1), e1.elapsed_time(e2)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    if rank == 0:
+        print({"world": world, "lattice": f"{Ns}^3x{Nt}", "d": d, "n_sub": n_sub, "subupdate_loop_ms": float(t[0]),
+               "exchange_ms": float(t[1]), "C": [complex(c) for c in C]})
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

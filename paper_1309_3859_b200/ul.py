@@ -19,7 +19,7 @@ SYMBOLS = [
     "ul_create", "ul_create_ext", "ul_workspace_bytes", "ul_destroy", "ul_init", "ul_set_beta",
     "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep",
     "ul_set_subupdate", "ul_set_update_algorithm", "ul_multilevel", "ul_multilevel_replay", "ul_workspace_bytes_replay", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
-    "ul_measure_end", "ul_set_accum_batch", "ul_plaquette", "ul_polyakov", "ul_read_correlators", "ul_read_slab_averages",
+    "ul_measure_end", "ul_set_accum_batch", "ul_plaquette", "ul_polyakov", "ul_set_site_offset", "ul_slab_partial_product", "ul_read_correlators", "ul_read_slab_averages",
     "ul_get_launch_count", "ul_philox_selftest", "ul_sync", "ul_last_error",
 ]
 
@@ -67,6 +67,8 @@ def lib():
         L.ul_measure_begin.argtypes = [P, C.c_int, C.c_int, P, C.c_int]
         L.ul_set_accum_batch.argtypes = [P, C.c_int]
         L.ul_polyakov.argtypes = [P, C.c_int, P]
+        L.ul_set_site_offset.argtypes = [P, C.c_uint64]
+        L.ul_slab_partial_product.argtypes = [P, C.c_int, C.c_int, P]
         L.ul_accumulate.argtypes = [P]
         L.ul_measure_end.argtypes = [P]
         L.ul_plaquette.argtypes = [P, P]
@@ -261,6 +263,18 @@ class Lattice:
         out = np.zeros(2)
         self._ck(lib().ul_polyakov(self._h, int(multihit), _ptr(out)))
         return complex(out[0], out[1])
+
+    def set_site_offset(self, offset):
+        self._ck(lib().ul_set_site_offset(self._h, int(offset)))
+
+    def slab_partial_product(self, s_begin, s_end):
+        """prod_{s_begin <= s < s_end} [T](x,s) of the last measurement: complex128 device tensor [3][r_max][Ns^3]."""
+        torch = self._torch
+        R = self._meas[0]
+        out = torch.empty((3, R, self.Ns ** 3), dtype=torch.complex128, device=self.device)
+        self._ck(lib().ul_slab_partial_product(self._h, int(s_begin), int(s_end), C.c_void_p(out.data_ptr())))
+        self.sync()
+        return out
 
     def launch_count(self):
         v = C.c_uint64()

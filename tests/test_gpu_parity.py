@@ -828,3 +828,37 @@ def test_replay_full_mid_plane_against_oracle(ul, ulo):
     assert ul.workspace_bytes(Ns, Nt, d, 0, R, len(fps)) > 100 * ul.workspace_bytes_replay(Ns, Nt, d, R, len(fps))
     g.multilevel_replay(d, 3, R, fps)                               # and a short run through the sub-updates
     assert np.all(np.isfinite(g.read_correlators()[1]))
+
+
+# ----------------------------------------------------------------------------- slab sharding (next row)
+@pytest.mark.parametrize("world", [2, 4])
+@pytest.mark.parametrize("alg", [0, 1])
+def test_slab_sharding_reproduces_the_unsharded_run(ul, world, alg):
+    """The shards of a t-partitioned lattice, run ONE AFTER THE OTHER on this GPU (no kernel waits on another),
+    reproduce the unsharded multilevel run bit for bit on the links and slab averages they own (global Philox
+    counters through ul_set_site_offset, frozen boundary layer in the ghost slab, no communication in the
+    sub-update loop); the product of the per-shard slab products gives the unsharded C(r)."""
+    from paper_1309_3859_b200 import sharded
+    Ns, Nt, d, R, n_sub, beta, seed = 8, 16, 2, 3, 6, 0.99, 77
+    full = ul.Lattice(Ns, Nt, beta, seed)
+    full.set_update_algorithm(alg, 1.1)
+    for _ in range(10):
+        full.sweep(1, 3)
+    links0, ctr0 = full.get_links(), full.get_counter()
+    full.set_links(links0)                                          # both runs start from the fp32-rounded angles
+    full.multilevel(d, n_sub, R)
+    A_full, C_full = full.read_slab_averages(), full.read_correlators()[0]
+    links1 = full.get_links_raw()
+    parts = sharded.partition(Nt, d, world)
+    prods = []
+    for rank in range(world):
+        sh = sharded.ShardedLattice(Ns, Nt, beta, seed, d, rank, world, links0, ctr0)
+        sh.lat.set_update_algorithm(alg, 1.1)
+        sh.multilevel(n_sub, R)
+        t0, n = parts[rank]
+        assert np.array_equal(sh.own_slab_averages(), A_full[:, :, t0 // d:(t0 + n) // d])
+        assert np.array_equal(sh.lat.get_links_raw()[:, :n], links1[:, t0:t0 + n])
+        assert sh.lat.get_counter() == full.get_counter()
+        prods.append(sh.partial_product())
+    C, _ = sharded.combine_partial_products(prods[0], gathered=prods)
+    assert np.abs(C - C_full).max() <= 1e-13 * max(1.0, np.abs(C_full).max())
