@@ -75,6 +75,21 @@ Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_f
 
 }  // namespace
 
+struct GraphKey {
+    int n_hb, n_or, slab_d, alg, local_rounds;
+    double beta, met_delta;
+    uint32_t site_offset;
+    bool operator==(const GraphKey& o) const {
+        return n_hb == o.n_hb && n_or == o.n_or && slab_d == o.slab_d && alg == o.alg && local_rounds == o.local_rounds &&
+               beta == o.beta && met_delta == o.met_delta && site_offset == o.site_offset;
+    }
+};
+struct CachedGraph {
+    GraphKey key;
+    cudaGraphExec_t exec = nullptr;
+    uint64_t launches = 0;
+};
+
 struct ul_ctx {
     int Ns = 0, Nt = 0, Nh = 0;
     long long Vs = 0, V = 0, Vh = 0;
@@ -94,6 +109,11 @@ struct ul_ctx {
     int* hb_qcount = nullptr;
     int hb_qblocks = 0;
     int hb_local_rounds = 2;
+    uint32_t* d_sweep = nullptr;      // device copy of the sweep counter for graph replays
+    bool d_sweep_stale = true;
+    bool use_graphs = false, capturing = false;
+    cudaStream_t cap_stream = nullptr;
+    std::vector<CachedGraph> graphs;
     uint32_t site_offset = 0; // ul_set_site_offset
     int alg = 0;             // ul_set_update_algorithm: 0 heatbath, 1 Metropolis for the stochastic sweeps
     double met_delta = 3.14159265358979323846;
@@ -149,9 +169,9 @@ int largest_divisor_le(int n, int cap) {
 template <int KIND, int MU>
 cudaError_t launch_update_vec(const ul_ctx* c, const ulk::UpdateArgs& a, dim3 grid, dim3 block) {
     switch (c->vec) {
-        case 4: ulk::k_update<KIND, MU, 4><<<grid, block, 0, c->stream>>>(a); break;
-        case 2: ulk::k_update<KIND, MU, 2><<<grid, block, 0, c->stream>>>(a); break;
-        default: ulk::k_update<KIND, MU, 1><<<grid, block, 0, c->stream>>>(a); break;
+        case 4: if (c->capturing) ulk::k_update<KIND, MU, 4, true><<<grid, block, 0, c->stream>>>(a); else ulk::k_update<KIND, MU, 4, false><<<grid, block, 0, c->stream>>>(a); break;
+        case 2: if (c->capturing) ulk::k_update<KIND, MU, 2, true><<<grid, block, 0, c->stream>>>(a); else ulk::k_update<KIND, MU, 2, false><<<grid, block, 0, c->stream>>>(a); break;
+        default: if (c->capturing) ulk::k_update<KIND, MU, 1, true><<<grid, block, 0, c->stream>>>(a); else ulk::k_update<KIND, MU, 1, false><<<grid, block, 0, c->stream>>>(a); break;
     }
     return cudaGetLastError();
 }
@@ -174,11 +194,10 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
     a.th = c->th; a.Vh = (int)c->Vh; a.Ns = c->Ns; a.Nh = c->Nh; a.Nt = c->Nt;
     a.parity = parity; a.slab_d = slab_d; a.beta = (float)c->beta;
     a.key0 = (uint32_t)(c->seed & 0xffffffffu); a.key1 = (uint32_t)(c->seed >> 32);
-    a.sweep_lo = (uint32_t)(c->sweep & 0xffffffffu); a.sweep_hi = (uint32_t)(c->sweep >> 32);
+    a.sweep_lo = (uint32_t)(c->sweep & 0xffffffffu); a.sweep_hi = (uint32_t)(c->sweep >> 32); a.sweep_dev = c->d_sweep;
     const dim3 block(c->bx, c->by, 2 * c->bz), grid(c->Nh / c->by, c->Ns / c->bz, n_t);   // by = x2 row PAIRS per block
     a.site_offset = c->site_offset;
     a.queue = c->hb_queue; a.qcount = c->hb_qcount; a.qblocks = (int)(grid.x * grid.y * grid.z); a.local_rounds = c->hb_local_rounds;
-    if (kind == 0 && cudaMemsetAsync(c->hb_qcount, 0, sizeof(int) * (size_t)a.qblocks, c->stream) != cudaSuccess) return fail(c, UL_ECUDA, "memset straggler counters");
     {
         const double units = c->met_delta * (4294967296.0 / 6.283185307179586476925286766559);
         a.met_delta_bt = units >= 2147483647.0 ? 2147483647 : (int)(units + 0.5);
@@ -188,7 +207,9 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
     if (e != cudaSuccess) return fail(c, UL_ECUDA, std::string("k_update launch: ") + cudaGetErrorString(e));
     c->launches += 1;
     if (kind == 0) {                                  // finish the links the heatbath kernel queued
-        ulk::k_hb_stragglers<<<(a.qblocks * ulk::HB_QSEG + 255) / 256, 256, 0, c->stream>>>(a, mu);
+        const int nb = (a.qblocks * ulk::HB_QSEG + 255) / 256;        // it also zeroes the counters for the next sub-step
+        if (c->capturing) ulk::k_hb_stragglers<true><<<nb, 256, 0, c->stream>>>(a, mu);
+        else ulk::k_hb_stragglers<false><<<nb, 256, 0, c->stream>>>(a, mu);
         if (cudaGetLastError() != cudaSuccess) return fail(c, UL_ECUDA, "k_hb_stragglers launch");
         c->launches += 1;
     }
@@ -200,12 +221,57 @@ int one_sweep(ul_ctx* c, int kind, int slab_d) {      // O5: parity outer, direc
             const int rc = substep(c, kind, parity, mu, slab_d);
             if (rc) return rc;
         }
-    if (kind != 1) c->sweep += 1;                     // heatbath and Metropolis sweeps consume the counter
+    if (kind != 1) {                                  // heatbath and Metropolis sweeps consume the counter
+        if (c->capturing) { ulk::k_bump_sweep<<<1, 1, 0, c->stream>>>(c->d_sweep); c->launches += 1; }
+        else { c->sweep += 1; c->d_sweep_stale = true; }
+    }
     return UL_OK;
 }
-int compound(ul_ctx* c, int n_hb, int n_or, int slab_d) {
+int compound_direct(ul_ctx* c, int n_hb, int n_or, int slab_d) {
     for (int i = 0; i < n_hb; ++i) { const int rc = one_sweep(c, c->alg == 1 ? 2 : 0, slab_d); if (rc) return rc; }
     for (int i = 0; i < n_or; ++i) { const int rc = one_sweep(c, 1, slab_d); if (rc) return rc; }
+    return UL_OK;
+}
+
+// Small lattices (the paper's 24^3 x Nt) are launch-bound: ~5 us per launch against ~1 us of work.  There a
+// compound sweep (8 (n_hb + n_or) sub-steps, straggler kernels, counter bump) is captured ONCE per recipe into a
+// CUDA graph -- on a side stream, with kernels that read the sweep counter from device memory, so that the graph
+// never changes -- and replayed on the caller's stream.  Same kernels, same arithmetic, same results.
+int compound(ul_ctx* c, int n_hb, int n_or, int slab_d) {
+    if (!c->use_graphs || n_hb + n_or == 0) return compound_direct(c, n_hb, n_or, slab_d);
+    GraphKey key{n_hb, n_or, slab_d, c->alg, c->hb_local_rounds, c->beta, c->met_delta, c->site_offset};
+    CachedGraph* g = nullptr;
+    for (auto& e : c->graphs) if (e.key == key) g = &e;
+    if (!g) {
+        cudaStream_t user = c->stream;
+        const uint64_t launches0 = c->launches;
+        c->stream = c->cap_stream; c->capturing = true;
+        cudaGraph_t graph = nullptr;
+        int rc = UL_OK;
+        if (cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) rc = UL_ECUDA;
+        if (!rc) rc = compound_direct(c, n_hb, n_or, slab_d);
+        const cudaError_t ee = cudaStreamEndCapture(c->cap_stream, &graph);
+        c->stream = user; c->capturing = false;
+        CachedGraph ng;
+        ng.key = key; ng.launches = c->launches - launches0;
+        c->launches = launches0;
+        if (rc || ee != cudaSuccess || !graph || cudaGraphInstantiate(&ng.exec, graph, 0) != cudaSuccess) {
+            if (graph) cudaGraphDestroy(graph);
+            cudaGetLastError();
+            c->use_graphs = false;                    // no graphs on this context: launch directly (same kernels)
+            return compound_direct(c, n_hb, n_or, slab_d);
+        }
+        cudaGraphDestroy(graph);
+        c->graphs.push_back(ng);
+        g = &c->graphs.back();
+    }
+    if (c->d_sweep_stale) {
+        ulk::k_set_sweep<<<1, 1, 0, c->stream>>>(c->d_sweep, (uint32_t)(c->sweep & 0xffffffffu), (uint32_t)(c->sweep >> 32));
+        c->d_sweep_stale = false;
+    }
+    if (cudaGraphLaunch(g->exec, c->stream) != cudaSuccess) return fail(c, UL_ECUDA, "cudaGraphLaunch");
+    c->sweep += (uint64_t)n_hb;                       // the graph bumped the device counter n_hb times
+    c->launches += g->launches;
     return UL_OK;
 }
 
@@ -376,6 +442,9 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     if (cudaMalloc(&q, (sizeof(int4) * ulk::HB_QSEG + sizeof(int)) * (size_t)c->hb_qblocks) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ENOMEM, "cudaMalloc straggler queue"); }
     c->hb_queue = (int4*)q;
     c->hb_qcount = (int*)(c->hb_queue + (size_t)ulk::HB_QSEG * c->hb_qblocks);
+    if (cudaMemset(c->hb_qcount, 0, sizeof(int) * (size_t)c->hb_qblocks) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ECUDA, "memset straggler counters"); }
+    c->d_sweep = (uint32_t*)(c->d_bad + 2);
+    c->use_graphs = c->V <= (1LL << 21) && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) == cudaSuccess;
     *h = c;
     const int rc = ul_init(c, 1);
     if (rc) { g_err = c->err; ul_destroy(c); *h = nullptr; }
@@ -411,6 +480,8 @@ int ul_destroy(ul_ctx* c) {
     if (c->staging) cudaFree(c->staging);
     if (c->scratch) cudaFree(c->scratch);
     if (c->hb_queue) cudaFree(c->hb_queue);
+    for (auto& e : c->graphs) if (e.exec) cudaGraphExecDestroy(e.exec);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
     delete c;
     return UL_OK;
@@ -475,7 +546,7 @@ int ul_get_links(ul_ctx* c, float* host) { return links_out(c, host, 0); }
 int ul_set_links_raw(ul_ctx* c, const int32_t* host) { return links_in(c, host, 3); }
 int ul_get_links_raw(ul_ctx* c, int32_t* host) { return links_out(c, host, 2); }
 int ul_get_counter(ul_ctx* c, uint64_t* v) { if (!c || !v) return fail(c, UL_EINVAL, "null pointer"); *v = c->sweep; return UL_OK; }
-int ul_set_counter(ul_ctx* c, uint64_t v) { if (!c) return fail(c, UL_EINVAL, "null handle"); c->sweep = v; return UL_OK; }
+int ul_set_counter(ul_ctx* c, uint64_t v) { if (!c) return fail(c, UL_EINVAL, "null handle"); c->sweep = v; c->d_sweep_stale = true; return UL_OK; }
 
 int ul_sweep(ul_ctx* c, int n_hb, int n_or) {
     if (!c || n_hb < 0 || n_or < 0) return fail(c, UL_EINVAL, "n_hb, n_or must be >= 0");
@@ -575,6 +646,7 @@ int ul_multilevel_replay(ul_ctx* c, int d, int n_sub, int r_max, const int* fps,
     if (n_sub > 0) {
         if (cudaMemcpyAsync(c->th, c->staging, link_bytes, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return bail(fail(c, UL_ECUDA, "restore links"));
         c->sweep = sweep0;
+        c->d_sweep_stale = true;
     }
     const long long n = (long long)c->n_slab * c->Vs;
     const int n_entries = r_max * (1 + 12 * n_fp);

@@ -25,6 +25,7 @@ struct UpdateArgs {
     float beta;
     uint32_t key0, key1;  // Philox key = seed
     uint32_t sweep_lo, sweep_hi;
+    const uint32_t* sweep_dev;   // DEVCTR kernels (CUDA-graph replays) read the sweep counter from here instead
     int4* queue;          // heatbath stragglers: (element offset, site | tries << 29, Sx, Sy), see k_hb_stragglers
     int* qcount;          // entries queued per block (zeroed before the launch); segment b = queue[b*HB_QSEG ...]
     int qblocks;          // number of segments
@@ -118,7 +119,8 @@ __device__ __forceinline__ void gather_staples(const UpdateArgs& P, const Site& 
 
 // The update proper from the staple sums.  KIND 0 = heatbath, 1 = overrelaxation.
 template <int KIND, int MU, int VEC>
-__device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st, const int h0, float Sx[VEC], float Sy[VEC]) {
+__device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st, const int h0, float Sx[VEC], float Sy[VEC],
+                                             const uint32_t sweep_lo, const uint32_t sweep_hi) {
     const int p = P.parity;
     int* own = P.th + ((MU * 2 + p) * P.Vh + st.e0);
     int out[VEC];
@@ -144,7 +146,7 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
 #pragma unroll
         for (int i = 0; i < VEC; ++i) {
             uint32_t w[4];
-            ulm::philox4x32_10(site0 + 2u * i, P.sweep_lo, P.sweep_hi, c3, P.key0, P.key1, w);
+            ulm::philox4x32_10(site0 + 2u * i, sweep_lo, sweep_hi, c3, P.key0, P.key1, w);
             const int v = (int)((w[0] >> 8) | 1u) - (1 << 23);                            // (2 u1 - 1) 2^23, odd, |v| < 2^23
             const int d = (int)(((long long)v * (long long)P.met_delta_bt) >> 23);        // |d| <= pi
             const int h = d >> 1;                                                         // |h| <= pi/2: no reduction needed
@@ -176,7 +178,7 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
             const ulm::HbParams hp = ulm::hb_setup(P.beta * ulm::mufu_sqrt(k2));
             pa[i] = hp.a; pq[i] = hp.q; pc[i] = hp.c0;
             uint32_t w[4];
-            ulm::philox4x32_10(site0 + 2u * i, P.sweep_lo, P.sweep_hi, c3, P.key0, P.key1, w);
+            ulm::philox4x32_10(site0 + 2u * i, sweep_lo, sweep_hi, c3, P.key0, P.key1, w);
             const bool ok = ulm::hb_attempt(hp, w[0], w[1], sn[i], cs[i]);
             neg |= (w[2] >> 31) << i;
             pend |= (ok ? 0u : 1u) << i;
@@ -188,7 +190,7 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
             hp.a = pick<float, VEC>(pa, j); hp.q = pick<float, VEC>(pq, j); hp.c0 = pick<float, VEC>(pc, j);
             const uint32_t n = (tries >> (8 * j)) & 0xffu;
             uint32_t w[4];
-            ulm::philox4x32_10(site0 + 2u * (uint32_t)j, P.sweep_lo, P.sweep_hi, (n << 8) | c3, P.key0, P.key1, w);
+            ulm::philox4x32_10(site0 + 2u * (uint32_t)j, sweep_lo, sweep_hi, (n << 8) | c3, P.key0, P.key1, w);
             float s1, c1;
             const bool ok = ulm::hb_attempt(hp, w[0], w[1], s1, c1);
 #pragma unroll
@@ -241,6 +243,13 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
 }
 
 
+__global__ void k_bump_sweep(uint32_t* sweep) {                 // ++counter (64 bit) at the end of a stochastic sweep of a graph
+    const uint32_t lo = sweep[0] + 1u;
+    sweep[0] = lo;
+    if (lo == 0u) sweep[1] += 1u;
+}
+__global__ void k_set_sweep(uint32_t* sweep, uint32_t lo, uint32_t hi) { sweep[0] = lo; sweep[1] = hi; }
+
 // Block (Nh/VEC, BYH, 2 BZ); grid (Ns/2/BYH, Ns/BZ, n_t) with n_t = Nt, or Nt*(d-1)/d active time layers for
 // a masked spatial direction.  The x2 rows are taken in pairs (2j, 2j+1): threads with threadIdx.z < BZ
 // take the row of the pair whose offset bit is 0, the others the row whose offset bit is 1, so the offset
@@ -252,8 +261,10 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
 #ifndef UL_OR_MINB
 #define UL_OR_MINB 0   // 0 = unspecified
 #endif
-template <int KIND, int MU, int VEC>
+template <int KIND, int MU, int VEC, bool DEVCTR>
 __global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_update(const UpdateArgs P) {
+    // the sweep counter: a kernel argument (uniform registers), or, for launches replayed from a CUDA graph, device memory
+    const uint32_t sweep_lo = DEVCTR ? __ldg(P.sweep_dev) : P.sweep_lo, sweep_hi = DEVCTR ? __ldg(P.sweep_dev + 1) : P.sweep_hi;
     const int Ns = P.Ns, Nh = P.Nh, Nt = P.Nt;
     const int h0 = threadIdx.x * VEC;
     const int bz = blockDim.z >> 1;
@@ -280,24 +291,30 @@ __global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_up
     float Sx[VEC], Sy[VEC];
     if (KIND != 0) {
         // overrelaxation, Metropolis: the short tail is compiled into both branches (56 registers, 4 blocks per SM)
-        if (sel) { gather_staples<MU, VEC, 1>(P, st, Sx, Sy); update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy); }
-        else { gather_staples<MU, VEC, 0>(P, st, Sx, Sy); update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy); }
+        if (sel) { gather_staples<MU, VEC, 1>(P, st, Sx, Sy); update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy, sweep_lo, sweep_hi); }
+        else { gather_staples<MU, VEC, 0>(P, st, Sx, Sy); update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy, sweep_lo, sweep_hi); }
     } else {
         // heatbath: one copy of the sampler after the branch keeps it at 64 registers (4 blocks per SM)
         if (sel) gather_staples<MU, VEC, 1>(P, st, Sx, Sy);
         else gather_staples<MU, VEC, 0>(P, st, Sx, Sy);
-        update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy);
+        update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy, sweep_lo, sweep_hi);
     }
 }
 
 // Finishes the heatbath links that k_update<0,...> queued: one thread per entry, attempts n = tries, tries+1, ...
 // with the same Philox counters and the same device functions as the main kernel (so the result does not
 // depend on where a link is finished), until accept or the cap of 64 attempts (O3).
+template <bool DEVCTR>
 __global__ void __launch_bounds__(256) k_hb_stragglers(const UpdateArgs P, int mu) {
     const uint32_t c3 = ((uint32_t)P.parity << 2) | (uint32_t)mu;
+    const uint32_t sweep_lo = DEVCTR ? __ldg(P.sweep_dev) : P.sweep_lo, sweep_hi = DEVCTR ? __ldg(P.sweep_dev + 1) : P.sweep_hi;
     {   // one thread per queue slot: grid = qblocks * HB_QSEG / 256 blocks, most of which leave at once
         const int e = blockIdx.x * blockDim.x + threadIdx.x;
-        if (e >= P.qblocks * HB_QSEG || (e % HB_QSEG) >= P.qcount[e / HB_QSEG]) return;   // a count above HB_QSEG: the rest was finished in place
+        const int seg = e / HB_QSEG;
+        const int cnt = seg < P.qblocks ? P.qcount[seg] : 0;                              // a count above HB_QSEG: the rest was finished in place
+        __syncthreads();                                                                  // every thread of the block holds its count:
+        if (e % HB_QSEG == 0 && seg < P.qblocks) P.qcount[seg] = 0;                       // zero it for the next heatbath sub-step
+        if ((e % HB_QSEG) >= cnt) return;
         const int4 q = P.queue[e];
         const uint32_t site = (uint32_t)q.y & 0x1fffffffu;
         uint32_t n = (uint32_t)q.y >> 29;
@@ -309,7 +326,7 @@ __global__ void __launch_bounds__(256) k_hb_stragglers(const UpdateArgs P, int m
         float sn, cs;
         uint32_t w[4];
         for (;;) {
-            ulm::philox4x32_10(site, P.sweep_lo, P.sweep_hi, (n << 8) | c3, P.key0, P.key1, w);
+            ulm::philox4x32_10(site, sweep_lo, sweep_hi, (n << 8) | c3, P.key0, P.key1, w);
             const bool ok = ulm::hb_attempt(hp, w[0], w[1], sn, cs);
             if (ok || n == 63u) break;
             ++n;
