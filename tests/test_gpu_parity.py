@@ -862,3 +862,40 @@ def test_slab_sharding_reproduces_the_unsharded_run(ul, world, alg):
         prods.append(sh.partial_product())
     C, _ = sharded.combine_partial_products(prods[0], gathered=prods)
     assert np.abs(C - C_full).max() <= 1e-13 * max(1.0, np.abs(C_full).max())
+
+
+def test_graph_replayed_sweeps_equal_directly_launched_substeps(ul):
+    """Lattices of <= 2^21 sites replay their compound sweeps from a CUDA graph whose kernels read the sweep counter
+    from device memory; ul_substep launches the same kernels directly with the counter as an argument.  Both must
+    give the same bits, sweep after sweep, full and slab-masked, heatbath and Metropolis."""
+    Ns, Nt = 8, 8
+    for alg in (0, 1):
+        a = ul.Lattice(Ns, Nt, 0.99, 13)
+        b = ul.Lattice(Ns, Nt, 0.99, 13)
+        for L in (a, b):
+            L.set_update_algorithm(alg, 1.3)
+        a.set_counter(2 ** 32 - 2)                                  # crosses the 32-bit boundary of the device counter
+        b.set_counter(2 ** 32 - 2)
+        for it in range(4):
+            a.sweep(2, 1)                                           # graph (captured at it = 0, replayed after)
+            for _ in range(2):
+                for parity in range(2):
+                    for mu in range(4):
+                        b.substep(2 if alg else 0, parity, mu, 0)
+                b.set_counter(b.get_counter() + 1)
+            for parity in range(2):
+                for mu in range(4):
+                    b.substep(1, parity, mu, 0)
+            assert a.get_counter() == b.get_counter() == 2 ** 32 - 2 + 2 * (it + 1)
+            assert np.array_equal(a.get_links_raw(), b.get_links_raw()), (alg, it)
+        a.multilevel(2, 3, 2)                                       # masked recipe: another graph
+        a.set_subupdate(1, 3, 1)
+        for _ in range(3):
+            for kind, n in ((2 if alg else 0, 1), (1, 3)):
+                for _ in range(n):
+                    for parity in range(2):
+                        for mu in range(4):
+                            b.substep(kind, parity, mu, 2)
+                    if kind != 1:
+                        b.set_counter(b.get_counter() + 1)
+        assert np.array_equal(a.get_links_raw(), b.get_links_raw()) and a.get_counter() == b.get_counter()
