@@ -29,6 +29,7 @@ struct ulo_ctx {
     int sub_hb = 1, sub_or = 3, sub_k = 1;  // sub-update recipe (DESIGN R5)
     int alg = 0;                   // 0 = heatbath (north star), 1 = Metropolis (DESIGN R21) for the "n_hb" sweeps
     double met_delta = PI;         // Metropolis proposal half-width (radians)
+    int multihit = 0;              // 1: two-link operators at r >= 2 are built from multihit temporal links
     // open single-level measurement
     bool open = false;
     int d = 0, r_max = 0, n_fp = 0, n_slab = 0;
@@ -248,6 +249,14 @@ static void open_measurement(ulo_ctx* c, int d, int r_max, const int* fps, int n
     c->n_acc = 0;
     c->open = true;
 }
+// Ubar_0(x) = (I1(beta k)/I0(beta k)) e^{i alpha}, k e^{i alpha} the staple sum of the temporal link at site x
+static cplx multihit_link(const ulo_ctx* c, long x) {
+    double k, alpha;
+    k_alpha(staple(c, 0, x), &k, &alpha);
+    const double a = c->beta * k;
+    const double ratio = a == 0.0 ? 0.0 : std::cyl_bessel_i(1.0, a) / std::cyl_bessel_i(0.0, a);
+    return ratio * cplx(std::cos(alpha), std::sin(alpha));
+}
 // add the current configuration: A += T^(d), B += TO^(d)   (Eq. 25, Eq. 31 P:340 generalised to thickness d)
 static void accumulate(ulo_ctx* c) {
     const int Ns = c->Ns;
@@ -267,7 +276,19 @@ static void accumulate(ulo_ctx* c) {
                                 phase += TH(c, 0, hop(c, x, mu, r)) - TH(c, 0, x);
                             }
                             const cplx T2(std::cos(phase), std::sin(phase));
-                            c->A[A_idx(c, mu, r, s, xs)] += T2;
+                            cplx TA = T2;
+                            if (c->multihit && r >= 2) {
+                                // analytic multihit: every temporal link of the two
+                                // lines is replaced by its mean over its own local weight, Ubar = (I1/I0)(beta k) e^{i alpha};
+                                // for r >= 2 no link of one line appears in the staple of a link of the other, and the
+                                // links of one line never share a plaquette, so all 2 d replacements are independent
+                                TA = cplx(1.0, 0.0);
+                                for (int t = s * c->d; t < (s + 1) * c->d; ++t) {
+                                    const long x = site_of(c, x1, x2, x3, t);
+                                    TA *= std::conj(multihit_link(c, x)) * multihit_link(c, hop(c, x, mu, r));
+                                }
+                            }
+                            c->A[A_idx(c, mu, r, s, xs)] += TA;
                             for (int fp = 0; fp < c->n_fp; ++fp) {
                                 const int a = c->fps[3 * fp], b = c->fps[3 * fp + 1], cc = c->fps[3 * fp + 2];
                                 for (int ch = 0; ch < 12; ++ch) {
@@ -415,6 +436,11 @@ int ulo_set_update_algorithm(ulo_ctx* c, int alg, double delta) {
     if (!c || (alg != 0 && alg != 1) || (alg == 1 && !(delta > 0.0 && delta <= PI))) return ULO_EINVAL;
     c->alg = alg;
     if (alg == 1) c->met_delta = delta;
+    return ULO_OK;
+}
+int ulo_set_multihit(ulo_ctx* c, int on) {
+    if (!c || (on != 0 && on != 1)) return ULO_EINVAL;
+    c->multihit = on;
     return ULO_OK;
 }
 int ulo_set_subupdate(ulo_ctx* c, int n_hb, int n_or, int k_sweeps) {

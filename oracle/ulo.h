@@ -47,6 +47,8 @@ int ulo_substep(ulo_ctx* h, int kind /*0 HB, 1 OR, 2 Metropolis*/, int parity, i
  * Metropolis with a uniform proposal of half-width delta in (0, pi] (DESIGN R21) */
 int ulo_set_update_algorithm(ulo_ctx* h, int alg, double delta);
 int ulo_set_subupdate(ulo_ctx* h, int n_hb, int n_or, int k_sweeps);
+/* on = 1: the sums of T (row a7) use multihit temporal links for r >= 2; the TO sums keep the plain T */
+int ulo_set_multihit(ulo_ctx* h, int on);
 
 /* multilevel measurement: S8(c)-O6, O7; Alg. 1 */
 int ulo_multilevel(ulo_ctx* h, int slab_thickness, int n_sub, int r_max,

@@ -45,6 +45,7 @@ def lib():
         L.ulo_sweep.argtypes = [P, C.c_int, C.c_int]
         L.ulo_substep.argtypes = [P, C.c_int, C.c_int, C.c_int, C.c_int]
         L.ulo_set_subupdate.argtypes = [P, C.c_int, C.c_int, C.c_int]
+        L.ulo_set_multihit.argtypes = [P, C.c_int]
         L.ulo_set_update_algorithm.argtypes = [P, C.c_int, C.c_double]
         L.ulo_multilevel.argtypes = [P, C.c_int, C.c_int, C.c_int, P, C.c_int]
         L.ulo_multilevel2.argtypes = [P, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, P, C.c_int]
@@ -141,6 +142,9 @@ class Oracle:
 
     def set_update_algorithm(self, alg, delta=np.pi):
         self._ck(lib().ulo_set_update_algorithm(self._h, int(alg), float(delta)))
+
+    def set_multihit(self, on):
+        self._ck(lib().ulo_set_multihit(self._h, int(on)))
 
     def set_subupdate(self, n_hb, n_or, k_sweeps=1):
         self._ck(lib().ulo_set_subupdate(self._h, int(n_hb), int(n_or), int(k_sweeps)))

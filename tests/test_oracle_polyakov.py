@@ -76,3 +76,71 @@ def test_multihit_has_the_same_mean_and_less_noise(ulo):
     assert abs(d.mean()) < 4 * err + 1e-3, (d.mean(), err)
     assert abs(plain.mean()) > 0.05                                      # there is a signal to speak of
     assert np.abs(d).mean() < 0.5 * np.abs(plain).mean()                 # and the two estimators track each other
+
+
+# ----------------------------------------------------------------- multihit inside the two-link operators (r >= 2)
+def test_multihit_two_link_closed_forms_and_gauge_invariance(ulo):
+    Ns, Nt, beta, R = 6, 4, 0.8, 3
+    o = ulo.Oracle(Ns, Nt, beta, 1)
+    o.init(0)
+    o.set_multihit(1)
+    o.multilevel(2, 0, R)
+    c = o.read_correlators()[0]
+    r = _ratio(6 * beta)
+    assert abs(c[0] - 1) < 1e-14                                       # r = 1 keeps the plain links (they share plaquettes)
+    assert np.abs(c[1:] - r ** (2 * Nt)).max() < 1e-13                 # 2 Nt multihit links per pair of lines
+    links = inputs.hot_links(Ns, Nt, 3) * 0.6
+    lam = inputs.gauge_function(Ns, Nt, 4)
+    vals = []
+    for cfg in (links, inputs.gauge_transform(links, lam)):
+        o.set_links(cfg)
+        o.multilevel(2, 0, R)
+        vals.append(o.read_correlators()[0])
+    assert np.abs(vals[0] - vals[1]).max() < 2e-6 and np.abs(vals[0][1:]).max() > 1e-6
+
+
+def test_multihit_two_link_numpy_restatement(ulo):
+    Ns, Nt, beta, d, R = 4, 4, 0.9, 2, 2
+    o = ulo.Oracle(Ns, Nt, beta, 5)
+    o.sweep(3, 1)
+    o.set_multihit(1)
+    o.multilevel(d, 0, R)
+    got = o.read_slab_averages()                                        # [3][R][n_slab][Vs]
+    Vs = Ns ** 3
+    ubar = np.empty((Nt, Vs), dtype=complex)
+    for t in range(Nt):
+        for xs in range(Vs):
+            k, alpha = o.staple(0, xs + Vs * t)
+            ubar[t, xs] = _ratio(beta * k) * np.exp(1j * alpha)
+    ubar = ubar.reshape(Nt, Ns, Ns, Ns)                                 # [t][x3][x2][x1]
+    for mu in (1, 2, 3):
+        shifted = np.roll(ubar, -2, axis=inputs.AXIS[mu])               # Ubar(x + 2 mu)
+        T = (np.conj(ubar) * shifted).reshape(Nt // d, d, Vs).prod(axis=1)
+        assert np.abs(got[mu - 1, 1] - T).max() < 1e-13
+    o.set_multihit(0)
+    o.multilevel(d, 0, R)
+    plain = o.read_slab_averages()
+    assert np.array_equal(plain[:, 0], got[:, 0]) and not np.allclose(plain[:, 1], got[:, 1])
+
+
+def test_multihit_two_link_same_mean_smaller_error(ulo):
+    """The estimator of C(2) with multihit links has the same expectation value and a smaller error (4^3 x 4,
+    beta = 0.7: signal ~1e-3)."""
+    Ns, Nt, beta = 4, 4, 0.7
+    res = {}
+    for on in (0, 1):
+        o = ulo.Oracle(Ns, Nt, beta, 23)
+        o.set_subupdate(1, 2, 1)
+        o.set_multihit(on)
+        o.sweep(20, 20)
+        vals = []
+        for _ in range(150):
+            o.sweep(1, 2)
+            o.multilevel(2, 6, 2)
+            vals.append(o.read_correlators()[0][1].real)
+        v = np.array(vals)
+        b = v.reshape(10, -1).mean(axis=1)
+        res[on] = (v.mean(), b.std(ddof=1) / np.sqrt(10))
+    (m0, e0), (m1, e1) = res[0], res[1]
+    assert abs(m0 - m1) < 4 * np.hypot(e0, e1), res
+    assert e1 < e0, res
