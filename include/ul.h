@@ -150,6 +150,15 @@ int ul_measure_begin(ul_ctx* h, int slab_thickness, int r_max, const int* field_
 int ul_accumulate(ul_ctx* h);
 int ul_measure_end(ul_ctx* h);
 
+/* Analytic multihit inside the two-link operators: with on = 1 the sums of
+ * T^(d)(x,s,r mu) for r >= 2 are built from multihit temporal links Ubar_0 = (I1(beta k)/I0(beta k)) e^{i alpha}
+ * (k e^{i alpha} the staple sum) instead of U_0: the same expectation value, a smaller variance.  r = 1 keeps the
+ * plain links (the two lines share plaquettes there), and so do all TO sums (a plaquette next to a line would be
+ * biased).  Applies to ul_multilevel, ul_multilevel2, ul_multilevel_replay and the ul_accumulate hook; needs
+ * 16 * depth * (Nt/d) * Ns^3 more workspace bytes than ul_workspace_bytes (depth = accumulation batch depth).
+ * UL_EINVAL: on not 0 or 1; UL_ESTATE: a measurement is open. */
+int ul_set_multihit(ul_ctx* h, int on);
+
 /* Accumulation batch depth (rows a7, a8).  The library tabulates up to `depth` configurations
  * (exp(i sum_t theta_0) per slab and site, and the plaquette sums) and adds them to the slab sums
  * in ONE read-modify-write pass, in sub-update order: the same sequence of fp64 additions as

@@ -24,7 +24,7 @@ constexpr int TBLK = 8 * NBLK;   // blocks of the slab-table kernel (grid-stride
 constexpr int KBATCH = 8;   // configurations accumulated per read-modify-write pass over the accumulators
 
 struct Workspace {           // byte offsets into the measurement workspace
-    size_t U = 0, Ot = 0, fps = 0, A2 = 0, B2 = 0, A4 = 0, B4 = 0, partial = 0, result = 0, total = 0;
+    size_t U = 0, Um = 0, Ot = 0, fps = 0, A2 = 0, B2 = 0, A4 = 0, B4 = 0, partial = 0, result = 0, total = 0;
     int kb = 1;              // batch depth: slots of U (and of Ot when field points are measured)
 };
 
@@ -37,7 +37,7 @@ int replay_blocks(long long n_slab_sites) {
     return nb < 1 ? 1 : (nb > NBLK ? NBLK : (int)nb);
 }
 
-Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_fp, bool replay = false) {
+Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_fp, bool replay = false, bool multihit = false) {
     Workspace w;
     const size_t Vs = (size_t)Ns * Ns * Ns;
     const size_t n_in = (size_t)(Nt / d_in), n_out = d_out > 0 ? (size_t)(Nt / d_out) : 0;
@@ -52,6 +52,7 @@ Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_f
     w.kb = kb;
     size_t o = 0;
     w.U = o;   o = align_up(o + (size_t)kb * n_in * Vs * 16);
+    w.Um = o;  o = align_up(o + (multihit ? (size_t)kb * n_in * Vs * 16 : 0));
     w.Ot = o;  o = align_up(o + (n_fp > 0 ? (ot_slots ? ot_slots : (size_t)kb) * 12 * n_in * Vs * sizeof(float) : 0));
     w.fps = o; o = align_up(o + (size_t)(n_fp > 0 ? n_fp : 1) * 3 * sizeof(int));
     w.A2 = o;  o = align_up(o + 3 * R * n_in * Vs * 16);
@@ -125,6 +126,7 @@ struct ul_ctx {
     int d = 0, r_max = 0, n_fp = 0, n_slab = 0, d_out = 0, n_outer = 0;
     long long n_acc = 0;
     int n_pending = 0;       // configurations tabulated but not yet added to the accumulators
+    bool multihit = false;   // ul_set_multihit: sums of T at r >= 2 from multihit temporal links
     bool replay = false;     // ul_multilevel_replay in progress: no TO sums, fields reduced on the fly in pass 2
     bool acc_fresh = true;   // the inner sums A2, B2 hold nothing yet: the next pass writes instead of adding
     Workspace ws;
@@ -286,7 +288,7 @@ template <typename T> T* wsp(ul_ctx* c, size_t off) { return reinterpret_cast<T*
 
 // reserve the workspace, upload the field points, zero the accumulators
 int open_measurement(ul_ctx* c, int d_in, int d_out, int r_max, const int* fps, int n_fp) {
-    const Workspace w = plan_workspace(c->Ns, c->Nt, d_in, d_out, r_max, n_fp, c->replay);
+    const Workspace w = plan_workspace(c->Ns, c->Nt, d_in, d_out, r_max, n_fp, c->replay, c->multihit);
     if (w.total > c->work_bytes) {
         if (!c->own_work && c->work) return fail(c, UL_ENOMEM, "accumulators exceed the caller's workspace");
         if (c->work) { UL_CUDA(c, cudaStreamSynchronize(c->stream)); cudaFree(c->work); c->work = nullptr; c->work_bytes = 0; }
@@ -326,19 +328,36 @@ int flush(ul_ctx* c) {
     do {                                                                                            \
         if (a.nk == KB) ulk::k_accumulate<KB, FIELD, true><<<nb, 256, 0, c->stream>>>(a);           \
         else ulk::k_accumulate<KB, FIELD, false><<<nb, 256, 0, c->stream>>>(a);                     \
+        c->launches += 1;                                                                           \
     } while (0)
-    if (c->n_fp > 0 && !c->replay) {
-        if (a.nk == 1) UL_ACC_LAUNCH(1, true);
-        else if (a.nk <= 4) UL_ACC_LAUNCH(4, true);
-        else UL_ACC_LAUNCH(KBATCH, true);
+    const bool fields = c->n_fp > 0 && !c->replay;
+    auto launch = [&](bool with_fields) {
+        if (with_fields) {
+            if (a.nk == 1) UL_ACC_LAUNCH(1, true);
+            else if (a.nk <= 4) UL_ACC_LAUNCH(4, true);
+            else UL_ACC_LAUNCH(KBATCH, true);
+        } else {
+            if (a.nk == 1) UL_ACC_LAUNCH(1, false);
+            else if (a.nk <= 4) UL_ACC_LAUNCH(4, false);
+            else UL_ACC_LAUNCH(KBATCH, false);
+        }
+    };
+    a.r_begin = 1; a.r_end = c->r_max; a.a_r_max = c->r_max;
+    if (!c->multihit) {
+        launch(fields);
     } else {
-        if (a.nk == 1) UL_ACC_LAUNCH(1, false);
-        else if (a.nk <= 4) UL_ACC_LAUNCH(4, false);
-        else UL_ACC_LAUNCH(KBATCH, false);
+        // multihit: the sums of T at r >= 2 come from the Um tables; r = 1 (the two lines share plaquettes) and every
+        // TO sum keep the plain T
+        if (fields) { a.a_r_max = 1; launch(true); }                                    // TO for all r, T for r = 1
+        else { a.r_end = 1; launch(false); }                                             // T for r = 1
+        if (c->r_max >= 2) {
+            a.U = wsp<double2>(c, c->ws.Um);
+            a.r_begin = 2; a.r_end = c->r_max; a.a_r_max = c->r_max;
+            launch(false);                                                               // T for r >= 2
+        }
     }
 #undef UL_ACC_LAUNCH
     UL_CUDA(c, cudaGetLastError());
-    c->launches += 1;
     c->n_pending = 0;
     c->acc_fresh = false;
     return UL_OK;
@@ -351,6 +370,8 @@ int accumulate(ul_ctx* c) {
     ulk::TableArgs t;
     t.g = geom(c); t.th = c->th; t.d = c->d; t.n_slab = c->n_slab;
     t.U = wsp<double2>(c, c->ws.U) + (size_t)c->n_pending * n;
+    t.Um = c->multihit ? wsp<double2>(c, c->ws.Um) + (size_t)c->n_pending * n : nullptr;
+    t.beta = (float)c->beta;
     t.Ot = (c->n_fp > 0 && !c->replay) ? wsp<float>(c, c->ws.Ot) + (size_t)c->n_pending * 12 * n : nullptr;
     t.partial = wsp<double>(c, c->ws.partial);
     const int gx = (c->Ns * c->Ns + 255) / 256, rows = c->n_slab * c->Ns;
@@ -565,6 +586,12 @@ int ul_set_update_algorithm(ul_ctx* c, int alg, double delta) {
     if (alg == 1) c->met_delta = delta;
     return UL_OK;
 }
+int ul_set_multihit(ul_ctx* c, int on) {
+    if (!c || (on != 0 && on != 1)) return fail(c, UL_EINVAL, "on must be 0 or 1");
+    if (c->open) return fail(c, UL_ESTATE, "a measurement is open");
+    c->multihit = on != 0;
+    return UL_OK;
+}
 int ul_set_subupdate(ul_ctx* c, int n_hb, int n_or, int k_sweeps) {
     if (!c || n_hb < 0 || n_or < 0 || k_sweeps < 1) return fail(c, UL_EINVAL, "bad sub-update recipe");
     c->sub_hb = n_hb; c->sub_or = n_or; c->sub_k = k_sweeps;
@@ -653,7 +680,8 @@ int ul_multilevel_replay(ul_ctx* c, int d, int n_sub, int r_max, const int* fps,
     double* res = wsp<double>(c, c->ws.result);
     ulk::TableArgs t;
     t.g = geom(c); t.th = c->th; t.d = c->d; t.n_slab = c->n_slab;
-    t.U = wsp<double2>(c, c->ws.U); t.Ot = wsp<float>(c, c->ws.Ot); t.partial = wsp<double>(c, c->ws.partial);
+    t.U = wsp<double2>(c, c->ws.U); t.Um = nullptr; t.beta = (float)c->beta;       // the TO sums use the plain T
+    t.Ot = wsp<float>(c, c->ws.Ot); t.partial = wsp<double>(c, c->ws.partial);
     ulk::ReplayArgs ra;
     ra.g = geom(c); ra.n_slab = c->n_slab; ra.r_max = r_max; ra.n_fp = n_fp;
     ra.U = t.U; ra.Ot = t.Ot; ra.fps = wsp<int>(c, c->ws.fps); ra.W = wa.W; ra.partial = wsp<double>(c, c->ws.partial);

@@ -267,9 +267,22 @@ struct TableArgs {
     const int* th;
     int d, n_slab;
     double2* U;
+    double2* Um;          // multihit table (nullptr: off): prod_t Ubar_0(xs,t), Ubar = (I1/I0)(beta k) e^{i alpha}
+    float beta;
     float* Ot;
     double* partial;
 };
+
+// I1(a)/I0(a) in fp32 by the backward recurrence R_{n-1} = 1/(2n/a + R_n) from R_N = 0, N = a + 20 (the start value is
+// forgotten to 1e-8: every step contracts the error by R^2 < 0.4); MUFU.RCP per step, ~2e-7 relative
+__device__ __forceinline__ float bessel_ratio_i1_i0_f32(float a) {
+    if (!(a > 1e-30f)) return 0.0f;
+    const float two_over_a = 2.0f * ulm::mufu_rcp(a);
+    float R = 0.0f;
+    for (int n = min((int)a, 1000) + 20; n >= 1; --n) R = ulm::mufu_rcp(fmaf((float)n, two_over_a, R));
+    return R;
+}
+
 __global__ void __launch_bounds__(256) k_slab_tables(const TableArgs P) {
     __shared__ double sm[12 * 32];
     const Geom& g = P.g;
@@ -289,6 +302,7 @@ __global__ void __launch_bounds__(256) k_slab_tables(const TableArgs P) {
         if (!in) continue;
         const long long idx = (long long)row * (Ns * Ns) + i2;
         unsigned acc = 0u;
+        double mhr = 1.0, mhi = 0.0;                              // running product of the multihit factors f S' over the slab
         float o_c[6], o_s[6];
 #pragma unroll
         for (int o = 0; o < 6; ++o) { o_c[o] = 0.0f; o_s[o] = 0.0f; }
@@ -297,17 +311,41 @@ __global__ void __launch_bounds__(256) k_slab_tables(const TableArgs P) {
             int pl[6], th0;
             site_plaquettes(g, P.th, x, pl, th0);
             acc += (unsigned)th0;
-#pragma unroll
+            float Sx = 0.0f, Sy = 0.0f;                           // S' = sum_i [e^{-i P_i} + e^{+i Q_i}]: the staple sum of theta_0(x,t)
+#pragma unroll                                                    // is e^{i theta_0} S', P_i = theta_P(0,i)(x), Q_i = theta_P(0,i)(x - i)
             for (int o = 0; o < 6; ++o) {
                 float c, sn;
                 ulm::sincos_bt(pl[o], c, sn);
                 o_c[o] += 1.0f - c;
                 o_s[o] += sn;
+                if (o < 3) { Sx += c; Sy -= sn; }
+            }
+            if (P.Um) {
+                const int tp = (t + 1 == g.Nt) ? 0 : t + 1;
+#pragma unroll
+                for (int i = 1; i <= 3; ++i) {
+                    int y[4] = {t, x[1], x[2], x[3]};
+                    y[i] = (x[i] == 0) ? (int)Ns - 1 : x[i] - 1;
+                    const unsigned q = (unsigned)__ldg(P.th + link_index(g, 0, t, y[3], y[2], y[1]))
+                                     + (unsigned)__ldg(P.th + link_index(g, i, tp, y[3], y[2], y[1]))
+                                     - (unsigned)th0 - (unsigned)__ldg(P.th + link_index(g, i, t, y[3], y[2], y[1]));
+                    float c, sn;
+                    ulm::sincos_bt((int)q, c, sn);
+                    Sx += c; Sy += sn;
+                }
+                const float k2 = fmaf(Sx, Sx, Sy * Sy);
+                const float k = ulm::mufu_sqrt(k2);
+                const float f = k2 > 0.0f ? bessel_ratio_i1_i0_f32(P.beta * k) * ulm::mufu_rcp(k) : 0.0f;   // (I1/I0) e^{i alpha} = f e^{i theta_0} S'
+                const double fr = (double)(f * Sx), fi = (double)(f * Sy);
+                const double nr = mhr * fr - mhi * fi;
+                mhi = mhr * fi + mhi * fr;
+                mhr = nr;
             }
         }
         double us, uc;
         ulm::sincos_bt_f64((int)acc, uc, us);
         P.U[idx] = make_double2(uc, us);
+        if (P.Um) P.Um[idx] = make_double2(uc * mhr - us * mhi, uc * mhi + us * mhr);
 #pragma unroll
         for (int o = 0; o < 6; ++o) {
             if (P.Ot) {
@@ -352,6 +390,8 @@ struct AccumArgs {
     Geom g;
     int d, n_slab, r_max, n_fp;
     int nk;               // configurations in this batch (1..KB), slots 0..nk-1 in sub-update order
+    int r_begin, r_end;   // separations handled by this launch (multihit: r = 1 from the plain table, r >= 2 from Um)
+    int a_r_max;          // the sums of T are written only for r <= a_r_max (field launch with multihit: r = 1 only)
     int first;            // 1: first pass of a measurement: the sums start from zero (no read, no memset)
     const double2* U;     // [nk][n_slab*Vs]
     const float* Ot;      // [nk][12][n_slab*Vs]   (n_fp > 0 only)
@@ -398,16 +438,16 @@ __global__ void __launch_bounds__(256, FIELD ? 1 : UL_ACC_MINB) k_accumulate(con
 #pragma unroll
     for (int mu = 1; mu <= 3; ++mu) {
         const int nu = 1 + (mu % 3), rho = 1 + ((mu + 1) % 3);
-        double2* Ap = P.A + ((long long)(mu - 1) * P.r_max * P.n_slab + s) * g.Vs + xs;
-        for (int r0 = 1; r0 <= P.r_max; r0 += ACC_RB) {
+        double2* Ap = P.A + (((long long)(mu - 1) * P.r_max + (P.r_begin - 1)) * P.n_slab + s) * g.Vs + xs;
+        for (int r0 = P.r_begin; r0 <= P.r_end; r0 += ACC_RB) {
             double2 a[ACC_RB];
 #pragma unroll
             for (int i = 0; i < ACC_RB; ++i)
-                if (r0 + i <= P.r_max) a[i] = P.first ? make_double2(0.0, 0.0) : __ldcs(Ap + i * stepA);
+                if (r0 + i <= P.r_end) a[i] = (P.first || r0 + i > P.a_r_max) ? make_double2(0.0, 0.0) : __ldcs(Ap + i * stepA);
 #pragma unroll
             for (int i = 0; i < ACC_RB; ++i) {
                 const int r = r0 + i;
-                if (r > P.r_max) break;
+                if (r > P.r_end) break;
                 // T^(d)(x,s,r mu) = U(x + r mu) conj(U(x))  (Eqs. 22, 25)
                 const int ys = xs + (wrapc(x[mu] + r, Ns) - x[mu]) * stride[mu];         // r <= Ns/2
                 double2 T[KB], v[KB];
@@ -426,7 +466,7 @@ __global__ void __launch_bounds__(256, FIELD ? 1 : UL_ACC_MINB) k_accumulate(con
                         a[i].x = fma(v[k].y, u0[k].y, fma(v[k].x, u0[k].x, a[i].x));
                         a[i].y = fma(-v[k].x, u0[k].y, fma(v[k].y, u0[k].x, a[i].y));
                     }
-                __stcs(Ap + i * stepA, a[i]);
+                if (r <= P.a_r_max) __stcs(Ap + i * stepA, a[i]);
                 if (FIELD) {
                     for (int fp = 0; fp < P.n_fp; ++fp) {
                         // anchor y = x + (floor(r/2)+a) mu + b nu + c rho  (DESIGN R10)

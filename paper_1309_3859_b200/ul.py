@@ -19,7 +19,7 @@ SYMBOLS = [
     "ul_create", "ul_create_ext", "ul_workspace_bytes", "ul_destroy", "ul_init", "ul_set_beta",
     "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep",
     "ul_set_subupdate", "ul_set_update_algorithm", "ul_multilevel", "ul_multilevel_replay", "ul_workspace_bytes_replay", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
-    "ul_measure_end", "ul_set_accum_batch", "ul_plaquette", "ul_polyakov", "ul_set_site_offset", "ul_slab_partial_product", "ul_read_correlators", "ul_read_slab_averages",
+    "ul_measure_end", "ul_set_accum_batch", "ul_set_multihit", "ul_plaquette", "ul_polyakov", "ul_set_site_offset", "ul_slab_partial_product", "ul_read_correlators", "ul_read_slab_averages",
     "ul_get_launch_count", "ul_philox_selftest", "ul_sync", "ul_last_error",
 ]
 
@@ -66,6 +66,7 @@ def lib():
         L.ul_workspace_bytes_replay.restype = C.c_size_t
         L.ul_measure_begin.argtypes = [P, C.c_int, C.c_int, P, C.c_int]
         L.ul_set_accum_batch.argtypes = [P, C.c_int]
+        L.ul_set_multihit.argtypes = [P, C.c_int]
         L.ul_polyakov.argtypes = [P, C.c_int, P]
         L.ul_set_site_offset.argtypes = [P, C.c_uint64]
         L.ul_slab_partial_product.argtypes = [P, C.c_int, C.c_int, P]
@@ -208,6 +209,9 @@ class Lattice:
 
     def set_subupdate(self, n_hb, n_or, k_sweeps=1):
         self._ck(lib().ul_set_subupdate(self._h, int(n_hb), int(n_or), int(k_sweeps)))
+
+    def set_multihit(self, on):
+        self._ck(lib().ul_set_multihit(self._h, int(on)))
 
     def set_accum_batch(self, depth):
         self._ck(lib().ul_set_accum_batch(self._h, int(depth)))

@@ -899,3 +899,67 @@ def test_graph_replayed_sweeps_equal_directly_launched_substeps(ul):
                     if kind != 1:
                         b.set_counter(b.get_counter() + 1)
         assert np.array_equal(a.get_links_raw(), b.get_links_raw()) and a.get_counter() == b.get_counter()
+
+
+# ----------------------------------------------------------------------------- multihit inside the two-link operators
+@pytest.mark.parametrize("Ns,Nt,d", [(4, 4, 2), (8, 4, 2), (8, 8, 4), (6, 4, 1)])
+def test_multihit_two_link_against_oracle(ul, ulo, Ns, Nt, d):
+    """P2 with ul_set_multihit(1): slab averages, C(r), field values and vacuum on oracle configurations to relative
+    1e-5 (the staple sums are fp32 here, fp64 in the oracle); r = 1 and all TO sums are the plain ones bit for bit."""
+    from scipy import special
+    R, beta = min(3, Ns // 2), 0.95
+    o = ulo.Oracle(Ns, Nt, beta, 6)
+    for _ in range(8):
+        o.sweep(1, 3)
+    g = ul.Lattice(Ns, Nt, beta, 6)
+    g.set_links(o.get_links())
+    g.multilevel(d, 0, R, FPS)
+    plain = (g.read_slab_averages(),) + tuple(g.read_correlators())
+    o.set_multihit(1)
+    g.set_multihit(1)
+    o.multilevel(d, 0, R, FPS)
+    g.multilevel(d, 0, R, FPS)
+    ao, ag = o.read_slab_averages(), g.read_slab_averages()
+    co, fo, vo = o.read_correlators()
+    cg, fg, vg = g.read_correlators()
+    size = (special.ive(1, 4 * beta) / special.ive(0, 4 * beta)) ** (2 * d)          # magnitude of a multihit T^(d)
+    assert np.abs(ag - ao).max() < 2e-5 * size
+    assert np.array_equal(ag[:, 0], plain[0][:, 0]) and not np.allclose(ag[:, 1:], plain[0][:, 1:])
+    Vs = Ns ** 3
+    ok, worst = rel_ok(cg, co, 3 * Vs, rms_term=size ** (Nt // d))
+    assert ok, worst
+    for got, want, n in ((fg, fo, 3 * Vs * Nt), (vg, vo, 3 * Vs * Nt)):
+        ok, worst = rel_ok(got, want, n)
+        assert ok, worst
+    g.init(0)                                                                          # closed form on device
+    g.multilevel(d, 0, R)
+    c = g.read_correlators()[0]
+    r = special.ive(1, 6 * beta) / special.ive(0, 6 * beta)
+    assert abs(c[0] - 1) < 1e-12 and np.abs(c[1:] - r ** (2 * Nt)).max() < 2e-5 * r ** (2 * Nt)
+
+
+def test_multihit_two_link_paths_agree(ul):
+    """With multihit on: batch depths, the replay path and the two-level path (n_in = n_out = 1, frozen) give the
+    same numbers as the single-level stored path."""
+    Ns, Nt, d, R = 8, 8, 2, 3
+    ref = None
+    for depth, mode in ((0, "stored"), (1, "stored"), (3, "stored"), (0, "replay")):
+        g = ul.Lattice(Ns, Nt, 0.99, 41)
+        g.sweep(3, 2)
+        g.set_multihit(1)
+        g.set_accum_batch(depth)
+        (g.multilevel if mode == "stored" else g.multilevel_replay)(d, 7, R, FPS)
+        cur = (g.read_slab_averages(),) + tuple(g.read_correlators()) + (g.get_links_raw(),)
+        if ref is None:
+            ref = cur
+            continue
+        assert np.array_equal(cur[0], ref[0]) and np.array_equal(cur[1], ref[1]) and np.array_equal(cur[4], ref[4])
+        assert np.abs(cur[2] - ref[2]).max() <= 1e-12 * np.abs(ref[2]).max()
+    g = ul.Lattice(Ns, Nt, 0.99, 41)
+    g.sweep(3, 2)
+    g.set_multihit(1)
+    g.set_subupdate(0, 0, 1)
+    g.multilevel(d, 0, R)
+    c1 = g.read_correlators()[0]
+    g.multilevel2(2, 1, 4, 1, R)
+    assert np.allclose(g.read_correlators()[0], c1, rtol=1e-12, atol=1e-18)
