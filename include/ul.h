@@ -137,6 +137,16 @@ int ul_multilevel_replay(ul_ctx* h, int slab_thickness, int n_sub, int r_max,
                          const int* field_points, int n_fp);
 size_t ul_workspace_bytes_replay(int Ns, int Nt, int slab_thickness, int r_max, int n_fp);
 
+/* Two levels by REPLAY (for BJ config 4's field maps): the same estimator, trajectory, outputs and final state as
+ * ul_multilevel2 without its TO accumulators.  The weights of the linear-in-O form need the inner averages of the
+ * same outer iteration and the outer averages of the whole measurement: pass 1 runs the measurement with the sums
+ * of T only; pass 2 restarts from the saved configuration and runs the inner loop of every outer iteration twice
+ * (once for [T^(d_in)] and the weights, once to reduce weight x T x O on the fly): about three times the
+ * sub-update sweeps.  Workspace: ul_workspace_bytes_replay2 (plus two configuration copies the library allocates). */
+int ul_multilevel2_replay(ul_ctx* h, int d_in, int n_in, int d_out, int n_out, int r_max,
+                          const int* field_points, int n_fp);
+size_t ul_workspace_bytes_replay2(int Ns, int Nt, int d_in, int d_out, int r_max, int n_fp);
+
 /* Two levels (Eq. 27, Eqs. 32-33 P:343-347 with DESIGN R7, Alg. 1 lines 5-18):
  * n_out x { sub-update masked with d_out; n_in x { sub-update masked with d_in; accumulate
  * T^(d_in), TO^(d_in) }; combine the m = d_out/d_in inner slab averages of each outer slab

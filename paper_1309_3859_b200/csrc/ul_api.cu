@@ -58,7 +58,7 @@ Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_f
     w.A2 = o;  o = align_up(o + 3 * R * n_in * Vs * 16);
     w.B2 = o;  o = align_up(o + 3 * R * n_in * FB * Vs * 16);
     w.A4 = o;  o = align_up(o + 3 * R * n_out * Vs * 16);
-    w.B4 = o;  o = align_up(o + 3 * R * n_out * F12 * Vs * 16);
+    w.B4 = o;  o = align_up(o + 3 * R * n_out * FB * Vs * 16);
     const size_t n_entries = R * (1 + F12);
     size_t np = 2 * n_entries;
     if (np < 12 * (TBLK / NBLK)) np = 12 * (TBLK / NBLK);
@@ -127,6 +127,8 @@ struct ul_ctx {
     long long n_acc = 0;
     int n_pending = 0;       // configurations tabulated but not yet added to the accumulators
     bool multihit = false;   // ul_set_multihit: sums of T at r >= 2 from multihit temporal links
+    bool skip_colsum = false; // replayed configurations: their plaquette column sums are already in the vacuum sums
+    float* staging2 = nullptr; // second configuration copy (two-level replay)
     bool replay = false;     // ul_multilevel_replay in progress: no TO sums, fields reduced on the fly in pass 2
     bool acc_fresh = true;   // the inner sums A2, B2 hold nothing yet: the next pass writes instead of adding
     Workspace ws;
@@ -377,9 +379,9 @@ int accumulate(ul_ctx* c) {
     const int gx = (c->Ns * c->Ns + 255) / 256, rows = c->n_slab * c->Ns;
     const int gy = rows < TBLK / gx ? rows : (TBLK / gx > 0 ? TBLK / gx : 1);
     ulk::k_slab_tables<<<dim3(gx, gy), 256, 0, c->stream>>>(t);
-    ulk::k_sum_partials<<<12, 256, 0, c->stream>>>(t.partial, gx * gy, res_colsum(c), 1.0, 1);
+    if (!c->skip_colsum) { ulk::k_sum_partials<<<12, 256, 0, c->stream>>>(t.partial, gx * gy, res_colsum(c), 1.0, 1); c->launches += 1; }
     UL_CUDA(c, cudaGetLastError());
-    c->launches += 2;
+    c->launches += 1;
     c->n_acc += 1;
     c->n_pending += 1;
     if (c->n_pending == c->ws.kb) return flush(c);
@@ -493,12 +495,17 @@ size_t ul_workspace_bytes_replay(int Ns, int Nt, int d, int r_max, int n_fp) {
     if (Ns < 2 || Nt < 2 || d < 1 || Nt % d != 0 || r_max < 1 || n_fp < 0) return 0;
     return plan_workspace(Ns, Nt, d, 0, r_max, n_fp, n_fp > 0).total;
 }
+size_t ul_workspace_bytes_replay2(int Ns, int Nt, int d_in, int d_out, int r_max, int n_fp) {
+    if (Ns < 2 || Nt < 2 || d_in < 1 || Nt % d_in != 0 || d_out < d_in || d_out % d_in != 0 || Nt % d_out != 0 || r_max < 1 || n_fp < 0) return 0;
+    return plan_workspace(Ns, Nt, d_in, d_out, r_max, n_fp, n_fp > 0).total;
+}
 int ul_destroy(ul_ctx* c) {
     if (!c) return UL_OK;
     cudaStreamSynchronize(c->stream);
     if (c->own_th && c->th) cudaFree(c->th);
     if (c->own_work && c->work) cudaFree(c->work);
     if (c->staging) cudaFree(c->staging);
+    if (c->staging2) cudaFree(c->staging2);
     if (c->scratch) cudaFree(c->scratch);
     if (c->hb_queue) cudaFree(c->hb_queue);
     for (auto& e : c->graphs) if (e.exec) cudaGraphExecDestroy(e.exec);
@@ -731,6 +738,103 @@ int ul_multilevel2(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, int r_ma
         c->launches += 1;
     }
     return finish(c, a.A4, a.B4, c->n_outer, 1.0 / (double)n_out, 1.0 / ((double)n_in * (double)n_out));
+}
+
+// Two levels by replay (S8(f) rank 2 for BJ config 4): G is linear in O, with weights that need the inner averages of
+// the same outer iteration and the outer averages of the whole measurement.  Pass 1 runs the two-level measurement with
+// the sums of T only (-> [T4], C(r), W4).  Pass 2 restarts from the saved configuration; in every outer iteration the
+// inner loop is run twice from a saved configuration: once to form [T2] and the combined weights Wc, once to reduce
+// Wc T2 O on the fly.  About three times the sub-update sweeps of ul_multilevel2, none of its TO accumulators.
+int ul_multilevel2_replay(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, int r_max, const int* fps, int n_fp) {
+    if (!c || n_in < 1 || n_out < 1) return fail(c, UL_EINVAL, "n_in, n_out must be >= 1");
+    if (n_fp == 0) return ul_multilevel2(c, d_in, n_in, d_out, n_out, r_max, fps, n_fp);
+    int rc = check_meas_args(c, d_in, r_max, fps, n_fp);
+    if (rc) return rc;
+    if (d_out < d_in || d_out % d_in != 0 || c->Nt % d_out != 0) return fail(c, UL_EINVAL, "need d_in | d_out | Nt");
+    rc = ensure_staging(c);
+    if (rc) return rc;
+    const size_t link_bytes = sizeof(float) * 4 * (size_t)c->V;
+    if (!c->staging2) { void* p = nullptr; UL_CUDA(c, cudaMalloc(&p, link_bytes)); c->staging2 = (float*)p; }
+    UL_CUDA(c, cudaMemcpyAsync(c->staging, c->th, link_bytes, cudaMemcpyDeviceToDevice, c->stream));
+    const uint64_t sweep0 = c->sweep;
+    c->replay = true;
+    rc = open_measurement(c, d_in, d_out, r_max, fps, n_fp);
+    if (rc) { c->replay = false; return rc; }
+    auto bail = [&](int code) { c->replay = false; c->skip_colsum = false; c->open = false; return code; };
+    const Workspace& w = c->ws;
+    ulk::CombineArgs ca;
+    ca.Vs = c->Vs; ca.r_max = r_max; ca.n_fp = 0; ca.n_inner = c->n_slab; ca.n_outer = c->n_outer; ca.m = d_out / d_in;
+    ca.inv = 1.0 / (double)n_in;
+    ca.A2 = wsp<double2>(c, w.A2); ca.B2 = nullptr; ca.A4 = wsp<double2>(c, w.A4); ca.B4 = nullptr;
+    const long long total = 3LL * r_max * c->n_outer * c->Vs;
+    auto inner_pass = [&]() {                                      // n_in inner sub-updates, sums of T into A2
+        c->acc_fresh = true;
+        for (int j = 0; j < n_in; ++j) {
+            for (int k = 0; k < c->sub_k; ++k) { const int e = compound(c, c->sub_hb, c->sub_or, d_in); if (e) return e; }
+            const int e = accumulate(c);
+            if (e) return e;
+        }
+        return flush(c);
+    };
+    // pass 1
+    for (int J = 0; J < n_out; ++J) {
+        for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d_out); if (rc) return bail(rc); }
+        rc = inner_pass();
+        if (rc) return bail(rc);
+        ulk::k_combine<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>(ca);
+        c->launches += 1;
+    }
+    ulk::WeightArgs wa;
+    wa.Vs = c->Vs; wa.r_max = r_max; wa.n_slab = c->n_outer; wa.inv = 1.0 / (double)n_out;
+    wa.A = ca.A4; wa.W = wsp<double2>(c, w.B4);                    // W4 in the (A4-sized) B4 slot
+    const long long nw = 3LL * r_max * c->Vs;
+    ulk::k_slab_weights<<<(unsigned)((nw + 255) / 256), 256, 0, c->stream>>>(wa);
+    c->launches += 1;
+    if (cudaGetLastError() != cudaSuccess) return bail(fail(c, UL_ECUDA, "two-level replay, pass 1"));
+    // pass 2
+    if (cudaMemcpyAsync(c->th, c->staging, link_bytes, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return bail(fail(c, UL_ECUDA, "restore links"));
+    c->sweep = sweep0; c->d_sweep_stale = true;
+    c->skip_colsum = true;
+    const long long n = (long long)c->n_slab * c->Vs;
+    const int n_entries = r_max * (1 + 12 * n_fp);
+    double* res = wsp<double>(c, w.result);
+    ulk::GroupWeightArgs ga;
+    ga.Vs = c->Vs; ga.r_max = r_max; ga.n_inner = c->n_slab; ga.n_outer = c->n_outer; ga.m = d_out / d_in; ga.inv = 1.0 / (double)n_in;
+    ga.A2 = ca.A2; ga.W4 = wa.W; ga.Wc = wsp<double2>(c, w.B2);    // Wc in the (A2-sized) B2 slot
+    ulk::TableArgs t;
+    t.g = geom(c); t.th = c->th; t.d = c->d; t.n_slab = c->n_slab;
+    t.U = wsp<double2>(c, w.U); t.Um = nullptr; t.beta = (float)c->beta;
+    t.Ot = wsp<float>(c, w.Ot); t.partial = wsp<double>(c, w.partial);
+    ulk::ReplayArgs ra;
+    ra.g = geom(c); ra.n_slab = c->n_slab; ra.r_max = r_max; ra.n_fp = n_fp;
+    ra.U = t.U; ra.Ot = t.Ot; ra.fps = wsp<int>(c, w.fps); ra.W = ga.Wc; ra.partial = wsp<double>(c, w.partial);
+    const int gx = (c->Ns * c->Ns + 255) / 256, rows = c->n_slab * c->Ns;
+    const int gy = rows < TBLK / gx ? rows : (TBLK / gx > 0 ? TBLK / gx : 1);
+    const int nb = replay_blocks(n);
+    const double scale = 1.0 / ((double)n_in * (double)n_out * 3.0 * (double)c->Vs * (double)c->Nt);
+    for (int J = 0; J < n_out; ++J) {
+        for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d_out); if (rc) return bail(rc); }
+        if (cudaMemcpyAsync(c->staging2, c->th, link_bytes, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return bail(fail(c, UL_ECUDA, "save links"));
+        const uint64_t sweepJ = c->sweep;
+        rc = inner_pass();                                         // (a) the inner averages of this outer iteration
+        if (rc) return bail(rc);
+        ulk::k_group_weights<<<(unsigned)((nw + 255) / 256), 256, 0, c->stream>>>(ga);
+        c->launches += 1;
+        if (cudaMemcpyAsync(c->th, c->staging2, link_bytes, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return bail(fail(c, UL_ECUDA, "restore links"));
+        c->sweep = sweepJ; c->d_sweep_stale = true;
+        for (int j = 0; j < n_in; ++j) {                           // (b) the same inner sub-updates again, fields reduced on the fly
+            for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d_in); if (rc) return bail(rc); }
+            ulk::k_slab_tables<<<dim3(gx, gy), 256, 0, c->stream>>>(t);
+            ulk::k_replay_reduce<<<dim3(nb, r_max * n_fp), 256, 0, c->stream>>>(ra);
+            ulk::k_sum_partials<<<2 * (n_entries - r_max), 256, 0, c->stream>>>(ra.partial + (size_t)2 * r_max * nb, nb, res + 2 * r_max, scale, 1);
+            c->launches += 3;
+        }
+        if (cudaGetLastError() != cudaSuccess) return bail(fail(c, UL_ECUDA, "two-level replay, pass 2"));
+    }
+    c->skip_colsum = false;
+    rc = finish(c, ca.A4, nullptr, c->n_outer, 1.0 / (double)n_out, 1.0 / ((double)n_in * (double)n_out));
+    c->replay = false;
+    return rc;
 }
 
 int ul_plaquette(ul_ctx* c, double* out) {

@@ -667,6 +667,44 @@ __global__ void __launch_bounds__(256) k_slab_partial_product(const WeightArgs P
     P.W[idx] = run;
 }
 
+// Two-level replay weights: for the inner slab s = S m + i of outer slab S,
+//   Wc(x,s) = W4(x,S) prod_{i' != i} [T2](x, S m + i'),  W4(x,S) = prod_{S' != S} [T4](x,S')   (Eqs. 32-34 with the TO term
+// factored out: G is linear in O), [T2] = A2 * inv (inner sums of THIS outer iteration).  One thread per (mu, r, xs).
+struct GroupWeightArgs {
+    long long Vs;
+    int r_max, n_inner, n_outer, m;
+    double inv;           // 1 / n_in
+    const double2* A2;    // [mu][r][n_inner][xs]
+    const double2* W4;    // [mu][r][n_outer][xs]
+    double2* Wc;          // out [mu][r][n_inner][xs]
+};
+__global__ void __launch_bounds__(256) k_group_weights(const GroupWeightArgs P) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= 3LL * P.r_max * P.Vs) return;
+    const long long mr = idx / P.Vs, xs = idx - mr * P.Vs;
+    const double2* Ap = P.A2 + mr * P.n_inner * P.Vs + xs;
+    double2* Wp = P.Wc + mr * P.n_inner * P.Vs + xs;
+    for (int S = 0; S < P.n_outer; ++S) {
+        const double2 w4 = P.W4[(mr * P.n_outer + S) * P.Vs + xs];
+        double2 run = w4;
+        for (int i = 0; i < P.m; ++i) {                                                 // W4 times the prefix products
+            const long long s = (long long)S * P.m + i;
+            Wp[s * P.Vs] = run;
+            double2 a = Ap[s * P.Vs];
+            a.x *= P.inv; a.y *= P.inv;
+            run = cmul(run, a);
+        }
+        run = make_double2(1.0, 0.0);
+        for (int i = P.m - 1; i >= 0; --i) {                                            // times the suffix products
+            const long long s = (long long)S * P.m + i;
+            Wp[s * P.Vs] = cmul(Wp[s * P.Vs], run);
+            double2 a = Ap[s * P.Vs];
+            a.x *= P.inv; a.y *= P.inv;
+            run = cmul(run, a);
+        }
+    }
+}
+
 struct ReplayArgs {
     Geom g;
     int n_slab, r_max, n_fp;

@@ -18,7 +18,7 @@ UL_OK, UL_EINVAL, UL_ENOMEM, UL_ECUDA, UL_ESTATE = 0, -1, -2, -3, -4
 SYMBOLS = [
     "ul_create", "ul_create_ext", "ul_workspace_bytes", "ul_destroy", "ul_init", "ul_set_beta",
     "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep",
-    "ul_set_subupdate", "ul_set_update_algorithm", "ul_multilevel", "ul_multilevel_replay", "ul_workspace_bytes_replay", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
+    "ul_set_subupdate", "ul_set_update_algorithm", "ul_multilevel", "ul_multilevel_replay", "ul_workspace_bytes_replay", "ul_multilevel2_replay", "ul_workspace_bytes_replay2", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
     "ul_measure_end", "ul_set_accum_batch", "ul_set_multihit", "ul_plaquette", "ul_polyakov", "ul_set_site_offset", "ul_slab_partial_product", "ul_read_correlators", "ul_read_slab_averages",
     "ul_get_launch_count", "ul_philox_selftest", "ul_sync", "ul_last_error",
 ]
@@ -64,6 +64,9 @@ def lib():
         L.ul_multilevel_replay.argtypes = [P, C.c_int, C.c_int, C.c_int, P, C.c_int]
         L.ul_workspace_bytes_replay.argtypes = [C.c_int] * 5
         L.ul_workspace_bytes_replay.restype = C.c_size_t
+        L.ul_multilevel2_replay.argtypes = [P, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, P, C.c_int]
+        L.ul_workspace_bytes_replay2.argtypes = [C.c_int] * 6
+        L.ul_workspace_bytes_replay2.restype = C.c_size_t
         L.ul_measure_begin.argtypes = [P, C.c_int, C.c_int, P, C.c_int]
         L.ul_set_accum_batch.argtypes = [P, C.c_int]
         L.ul_set_multihit.argtypes = [P, C.c_int]
@@ -99,6 +102,10 @@ def workspace_bytes(Ns, Nt, d_in, d_out, r_max, n_fp):
 
 def workspace_bytes_replay(Ns, Nt, d, r_max, n_fp):
     return int(lib().ul_workspace_bytes_replay(int(Ns), int(Nt), int(d), int(r_max), int(n_fp)))
+
+
+def workspace_bytes_replay2(Ns, Nt, d_in, d_out, r_max, n_fp):
+    return int(lib().ul_workspace_bytes_replay2(int(Ns), int(Nt), int(d_in), int(d_out), int(r_max), int(n_fp)))
 
 
 def philox_selftest(ctr, key):
@@ -229,6 +236,11 @@ class Lattice:
     def multilevel2(self, d_in, n_in, d_out, n_out, r_max, field_points=None):
         fp, n = _fps(field_points)
         self._ck(lib().ul_multilevel2(self._h, int(d_in), int(n_in), int(d_out), int(n_out), int(r_max), _ptr(fp), n))
+        self._meas = (int(r_max), n, self.Nt // int(d_out))
+
+    def multilevel2_replay(self, d_in, n_in, d_out, n_out, r_max, field_points=None):
+        fp, n = _fps(field_points)
+        self._ck(lib().ul_multilevel2_replay(self._h, int(d_in), int(n_in), int(d_out), int(n_out), int(r_max), _ptr(fp), n))
         self._meas = (int(r_max), n, self.Nt // int(d_out))
 
     def measure_begin(self, slab_thickness, r_max, field_points=None):

@@ -963,3 +963,57 @@ def test_multihit_two_link_paths_agree(ul):
     c1 = g.read_correlators()[0]
     g.multilevel2(2, 1, 4, 1, R)
     assert np.allclose(g.read_correlators()[0], c1, rtol=1e-12, atol=1e-18)
+
+
+@pytest.mark.parametrize("Ns,Nt,n_in,n_out", [(4, 8, 3, 2), (8, 8, 9, 3), (6, 4, 2, 2)])
+def test_two_level_replay_equals_stored_accumulators(ul, Ns, Nt, n_in, n_out):
+    """ul_multilevel2_replay against ul_multilevel2 from the same start: bit-identical final links, counter,
+    correlators and outer slab averages; field values and vacuum to fp64 rounding order."""
+    R = min(3, Ns // 2)
+    res = []
+    for mode in ("stored", "replay"):
+        g = ul.Lattice(Ns, Nt, 0.99, 33)
+        g.sweep(3, 2)
+        (g.multilevel2 if mode == "stored" else g.multilevel2_replay)(2, n_in, 4, n_out, R, FPS)
+        res.append((g.get_links_raw(), g.get_counter(), g.read_slab_averages()) + tuple(g.read_correlators()))
+    a, b = res
+    assert np.array_equal(a[0], b[0]) and a[1] == b[1]
+    assert np.array_equal(a[2], b[2]) and np.array_equal(a[3], b[3])
+    assert np.abs(a[5] - b[5]).max() <= 1e-12
+    scale = np.abs(a[4]).max()
+    assert scale > 0 and np.abs(a[4] - b[4]).max() <= 1e-12 * max(scale, 1e-3)
+    # BJ config 4 with a 64-point field map: 0.46 TB of stored accumulators against ~2 GB for the replay
+    assert ul.workspace_bytes(32, 32, 2, 4, 16, 64) > 200 * ul.workspace_bytes_replay2(32, 32, 2, 4, 16, 64)
+
+
+def test_config4_full_mid_plane_field_map_by_replay(ul):
+    """BJ config 4 as stated: 32^4, two levels (d = 2 and 4), r = 1..16, the FULL mid-plane of field points
+    (32 x 32 transverse offsets, 12 channels).  Stored accumulators would need ~7 TB; the replay needs 1.6 GB.
+    Reduced n_in = n_out = 2 here.  The correlators equal those of ul_multilevel2 without fields bit for bit, and
+    the map at sampled points equals the stored path run with just those points."""
+    import time
+    Ns = Nt = 32
+    R = 16
+    plane = [(0, b, c) for c in range(Ns) for b in range(Ns)]
+    sample = [plane[0], plane[5 + 32 * 3], plane[17 + 32 * 30]]
+    assert ul.workspace_bytes_replay2(Ns, Nt, 2, 4, R, len(plane)) < 2 * 2 ** 30 < 1000 * 2 ** 30 < ul.workspace_bytes(Ns, Nt, 2, 4, R, len(plane))
+    out = {}
+    for mode in ("map", "sampled", "nofields"):
+        g = ul.Lattice(Ns, Nt, 1.0, 4)
+        for _ in range(10):
+            g.sweep(1, 3)
+        t0 = time.perf_counter()
+        if mode == "map":
+            g.multilevel2_replay(2, 2, 4, 2, R, plane)
+        elif mode == "sampled":
+            g.multilevel2(2, 2, 4, 2, R, sample)
+        else:
+            g.multilevel2(2, 2, 4, 2, R)
+        out[mode] = g.read_correlators() + (g.get_links_raw(), time.perf_counter() - t0)
+    print("config 4 full mid-plane map by replay (n_in = n_out = 2): %.2f s" % out["map"][4])
+    assert np.array_equal(out["map"][0], out["nofields"][0]) and np.array_equal(out["map"][3], out["nofields"][3])
+    fmap = out["map"][1]                                            # [r][fp][12]
+    idx = [plane.index(p) for p in sample]
+    assert np.all(np.isfinite(fmap))
+    ref = out["sampled"][1]
+    assert np.abs(fmap[:, idx] - ref).max() <= 1e-11 * np.abs(ref).max()
