@@ -409,13 +409,16 @@ struct AccumArgs {
 #ifndef UL_ACC_RB
 #define UL_ACC_RB 2
 #endif
+#ifndef UL_ACCF_MINB
+#define UL_ACCF_MINB 1
+#endif
 #ifndef UL_ACC_MINB
 #define UL_ACC_MINB 3
 #endif
 constexpr int ACC_RB = UL_ACC_RB;
 
 template <int KB, bool FIELD, bool FULL>
-__global__ void __launch_bounds__(256, FIELD ? 1 : UL_ACC_MINB) k_accumulate(const AccumArgs P) {
+__global__ void __launch_bounds__(256, FIELD ? UL_ACCF_MINB : UL_ACC_MINB) k_accumulate(const AccumArgs P) {
     const Geom& g = P.g;
     const long long n = (long long)P.n_slab * g.Vs;
     const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
