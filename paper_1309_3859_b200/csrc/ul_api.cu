@@ -64,7 +64,8 @@ Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_f
     if (np < 12 * (TBLK / NBLK)) np = 12 * (TBLK / NBLK);
     size_t partial_doubles = np * NBLK;
     if (replay) {                                   // fields: replay_blocks() partials per entry; correlators: NBLK per entry
-        const size_t nb = replay_blocks((long long)(n_in * Vs));
+        size_t nb = replay_blocks((long long)(n_in * Vs));
+        if (nb < 12) nb = 12;                       // the plane kernel writes up to 3 * 4 partials per entry
         partial_doubles = 2 * R * NBLK + 2 * R * F12 * nb;
         if (partial_doubles < (size_t)12 * TBLK) partial_doubles = (size_t)12 * TBLK;
     }
@@ -643,6 +644,38 @@ int ul_multilevel(ul_ctx* c, int d, int n_sub, int r_max, const int* fps, int n_
     return ul_measure_end(c);
 }
 
+// the field points are a full transverse plane fp = b + Ns c <-> (a, b, c) with one a?  (host array)
+bool full_plane(const ul_ctx* c, const int* fps, int n_fp, int* a_out) {
+    if (c->Ns > ulk::PLANE_MAX_NS || n_fp != c->Ns * c->Ns) return false;
+    for (int fp = 0; fp < n_fp; ++fp)
+        if (fps[3 * fp] != fps[0] || fps[3 * fp + 1] != fp % c->Ns || fps[3 * fp + 2] != fp / c->Ns) return false;
+    *a_out = fps[0];
+    return true;
+}
+// one configuration's W T O reduction into the result sums: k_replay_reduce, or the tiled plane kernel for full planes
+int reduce_fields(ul_ctx* c, const ulk::ReplayArgs& ra, bool plane, int plane_a, int n_entries, double scale) {
+    double* res = wsp<double>(c, c->ws.result);
+    const long long n = (long long)c->n_slab * c->Vs;
+    int nb;
+    if (plane) {
+        const int N2 = c->Ns * c->Ns, tiles = (N2 + 255) / 256, n_planes = c->n_slab * c->Ns;
+        int splits = NBLK / (tiles * ra.r_max * 3) + 1;
+        splits = splits > 4 ? 4 : splits;
+        splits = splits > n_planes ? n_planes : splits;
+        const size_t smem = (size_t)N2 * (sizeof(double2) + 12 * sizeof(double));
+        static bool attr_set = false;
+        if (!attr_set) { cudaFuncSetAttribute(ulk::k_replay_reduce_plane, cudaFuncAttributeMaxDynamicSharedMemorySize, ulk::PLANE_MAX_NS * ulk::PLANE_MAX_NS * 112); attr_set = true; }
+        ulk::k_replay_reduce_plane<<<dim3(tiles, ra.r_max, 3 * splits), 256, smem, c->stream>>>(ra, plane_a, splits);
+        nb = 3 * splits;
+    } else {
+        nb = replay_blocks(n);
+        ulk::k_replay_reduce<<<dim3(nb, ra.r_max * ra.n_fp), 256, 0, c->stream>>>(ra);
+    }
+    ulk::k_sum_partials<<<2 * (n_entries - ra.r_max), 256, 0, c->stream>>>(ra.partial + (size_t)2 * ra.r_max * nb, nb, res + 2 * ra.r_max, scale, 1);
+    c->launches += 2;
+    return cudaGetLastError() == cudaSuccess ? UL_OK : fail(c, UL_ECUDA, "field reduction launch");
+}
+
 // Single-level measurement by replay: the same estimator, trajectory and results as
 // ul_multilevel (to fp64 rounding order), with 2x the sweeps and none of the per-site TO accumulators.
 int ul_multilevel_replay(ul_ctx* c, int d, int n_sub, int r_max, const int* fps, int n_fp) {
@@ -650,6 +683,8 @@ int ul_multilevel_replay(ul_ctx* c, int d, int n_sub, int r_max, const int* fps,
     if (n_fp == 0) return ul_multilevel(c, d, n_sub, r_max, fps, n_fp);                  // nothing is linear in O: nothing to replay
     int rc = check_meas_args(c, d, r_max, fps, n_fp);
     if (rc) return rc;
+    int plane_a = 0;
+    const bool plane = full_plane(c, fps, n_fp, &plane_a);
     rc = ensure_staging(c);
     if (rc) return rc;
     const size_t link_bytes = sizeof(float) * 4 * (size_t)c->V;
@@ -700,10 +735,9 @@ int ul_multilevel_replay(ul_ctx* c, int d, int n_sub, int r_max, const int* fps,
         if (n_sub > 0)
             for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d); if (rc) return bail(rc); }
         ulk::k_slab_tables<<<dim3(gx, gy), 256, 0, c->stream>>>(t);                      // column sums were taken in pass 1
-        ulk::k_replay_reduce<<<dim3(nb, r_max * n_fp), 256, 0, c->stream>>>(ra);
-        ulk::k_sum_partials<<<2 * (n_entries - r_max), 256, 0, c->stream>>>(ra.partial + (size_t)2 * r_max * nb, nb, res + 2 * r_max, scale, 1);
-        if (cudaGetLastError() != cudaSuccess) return bail(fail(c, UL_ECUDA, "replay pass launch"));
-        c->launches += 3;
+        c->launches += 1;
+        rc = reduce_fields(c, ra, plane, plane_a, n_entries, scale);
+        if (rc) return bail(rc);
     }
     rc = finish(c, wsp<double2>(c, c->ws.A2), nullptr, c->n_slab, inv, inv);
     c->replay = false;
@@ -750,6 +784,8 @@ int ul_multilevel2_replay(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, i
     if (n_fp == 0) return ul_multilevel2(c, d_in, n_in, d_out, n_out, r_max, fps, n_fp);
     int rc = check_meas_args(c, d_in, r_max, fps, n_fp);
     if (rc) return rc;
+    int plane_a = 0;
+    const bool plane = full_plane(c, fps, n_fp, &plane_a);
     if (d_out < d_in || d_out % d_in != 0 || c->Nt % d_out != 0) return fail(c, UL_EINVAL, "need d_in | d_out | Nt");
     rc = ensure_staging(c);
     if (rc) return rc;
@@ -825,9 +861,9 @@ int ul_multilevel2_replay(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, i
         for (int j = 0; j < n_in; ++j) {                           // (b) the same inner sub-updates again, fields reduced on the fly
             for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d_in); if (rc) return bail(rc); }
             ulk::k_slab_tables<<<dim3(gx, gy), 256, 0, c->stream>>>(t);
-            ulk::k_replay_reduce<<<dim3(nb, r_max * n_fp), 256, 0, c->stream>>>(ra);
-            ulk::k_sum_partials<<<2 * (n_entries - r_max), 256, 0, c->stream>>>(ra.partial + (size_t)2 * r_max * nb, nb, res + 2 * r_max, scale, 1);
-            c->launches += 3;
+            c->launches += 1;
+            rc = reduce_fields(c, ra, plane, plane_a, n_entries, scale);
+            if (rc) return bail(rc);
         }
         if (cudaGetLastError() != cudaSuccess) return bail(fail(c, UL_ECUDA, "two-level replay, pass 2"));
     }

@@ -769,6 +769,84 @@ __global__ void __launch_bounds__(256) k_replay_reduce(const ReplayArgs P) {
     }
 }
 
+// The same reduction when the field points are a FULL transverse plane, fp = b + Ns c <-> offset (a, b, c) with one a
+// (BJ config 4's "full mid-plane maps"): for every plane (s, x_mu) of the lattice the map is the 2-d cross-correlation
+//   G(b,c) += sum_{p,q} Z(p,q) O(p + b, q + c),   Z = W T on the plane x_mu, O on the plane x_mu + floor(r/2) + a,
+// a dense contraction.  A block owns 256 outputs (b,c) of one (mu, r) for all 12 channels (24 fp64 accumulators per
+// thread), stages Z (fp64 complex) and the 12 O planes (as fp64, transposed so that the lanes of a warp read consecutive
+// words) in shared memory, and walks over its share of the planes: ~1.5 instructions per DFMA instead of ~4 for
+// k_replay_reduce.  Ns <= 32 (shared memory); gridDim = (Ns^2/256, r_max, 3 * splits).
+constexpr int PLANE_MAX_NS = 32;
+__global__ void __launch_bounds__(256) k_replay_reduce_plane(const ReplayArgs P, int fa, int splits) {
+    extern __shared__ double2 sh_z[];                                   // [Ns*Ns] Z(p,q), q fastest
+    const Geom& g = P.g;
+    const int Ns = g.Ns, N2 = Ns * Ns;
+    double* sh_o = reinterpret_cast<double*>(sh_z + N2);                // [12][Ns*Ns] O^T (fp64 copies: no conversion in the loop): index (q*Ns + p)
+    const int r = blockIdx.y + 1;
+    const int mu = blockIdx.z / splits + 1, split = blockIdx.z - (mu - 1) * splits;
+    const int nu = 1 + (mu % 3), rho = 1 + ((mu + 1) % 3);
+    const int stride[4] = {0, 1, Ns, Ns * Ns};
+    const long long n = (long long)P.n_slab * g.Vs;
+    const int out = blockIdx.x * blockDim.x + threadIdx.x;              // fp = b + Ns c
+    const int b = out % Ns, c = out / Ns;
+    const double2* Wm = P.W + ((long long)(mu - 1) * P.r_max + (r - 1)) * n;
+    int o_of[6];
+    float s_of[6];
+#pragma unroll
+    for (int comp = 0; comp < 6; ++comp) {
+        int pa, pb;
+        comp_dirs(mu, comp, pa, pb);
+        orient_of(pa, pb, o_of[comp], s_of[comp]);
+    }
+    double acc[24];
+#pragma unroll
+    for (int i = 0; i < 24; ++i) acc[i] = 0.0;
+    const int n_planes = P.n_slab * Ns;
+    for (int pl = split; pl < n_planes; pl += splits) {
+        const int s = pl / Ns, xm = pl - s * Ns;
+        const int xo = modc(xm + r / 2 + fa, Ns);                       // plane of the plaquettes (anchor, DESIGN R10)
+        const int ym = wrapc(xm + r, Ns);
+        __syncthreads();
+        for (int e = threadIdx.x; e < N2; e += blockDim.x) {            // e = p*Ns + q  (p along nu, q along rho)
+            const int p = e / Ns, q = e - p * Ns;
+            const int xs = xm * stride[mu] + p * stride[nu] + q * stride[rho];
+            const int ys = ym * stride[mu] + p * stride[nu] + q * stride[rho];
+            const long long j = (long long)s * g.Vs + xs;
+            const double2 u = P.U[j], v = P.U[(long long)s * g.Vs + ys];
+            const double2 T = make_double2(fma(v.x, u.x, v.y * u.y), fma(v.y, u.x, -(v.x * u.y)));
+            sh_z[e] = cmul(Wm[j], T);
+            const long long zs = (long long)s * g.Vs + xo * stride[mu] + p * stride[nu] + q * stride[rho];
+#pragma unroll
+            for (int comp = 0; comp < 6; ++comp) {
+                sh_o[(2 * comp) * N2 + q * Ns + p] = (double)P.Ot[(long long)(2 * o_of[comp]) * n + zs];
+                sh_o[(2 * comp + 1) * N2 + q * Ns + p] = (double)(s_of[comp] * P.Ot[(long long)(2 * o_of[comp] + 1) * n + zs]);
+            }
+        }
+        __syncthreads();
+        if (out < N2) {
+            for (int q = 0; q < Ns; ++q) {
+                const int qc = wrapc(q + c, Ns) * Ns;
+                for (int p = 0; p < Ns; ++p) {
+                    const double2 z = sh_z[p * Ns + q];
+                    const int io = qc + wrapc(p + b, Ns);
+#pragma unroll
+                    for (int ch = 0; ch < 12; ++ch) {
+                        const double o = sh_o[ch * N2 + io];
+                        acc[2 * ch] = fma(z.x, o, acc[2 * ch]);
+                        acc[2 * ch + 1] = fma(z.y, o, acc[2 * ch + 1]);
+                    }
+                }
+            }
+        }
+    }
+    if (out < N2) {
+        const long long o0 = P.r_max + ((long long)(r - 1) * P.n_fp + out) * 12;
+        const int nbk = 3 * splits, bk = (mu - 1) * splits + split;
+#pragma unroll
+        for (int i = 0; i < 24; ++i) P.partial[(2 * (o0 + i / 2) + (i & 1)) * nbk + bk] = acc[i];
+    }
+}
+
 // vacuum[ch] = (1/(3 V n_acc)) sum_mu sgn * colsum[orient(mu, comp)][kind]
 __global__ void k_vacuum(const double* __restrict__ colsum /*[12]*/, double scale, double* __restrict__ vac /*[12]*/) {
     const int ch = threadIdx.x;
