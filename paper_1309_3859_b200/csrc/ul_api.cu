@@ -267,6 +267,11 @@ int compound(ul_ctx* c, int n_hb, int n_or, int slab_d) {
             return compound_direct(c, n_hb, n_or, slab_d);
         }
         cudaGraphDestroy(graph);
+        if (c->graphs.size() >= 16) {                 // e.g. a scan in beta: keep the cache bounded, drop the oldest recipe
+            cudaStreamSynchronize(c->stream);
+            cudaGraphExecDestroy(c->graphs.front().exec);
+            c->graphs.erase(c->graphs.begin());
+        }
         c->graphs.push_back(ng);
         g = &c->graphs.back();
     }

@@ -1017,3 +1017,22 @@ def test_config4_full_mid_plane_field_map_by_replay(ul):
     assert np.all(np.isfinite(fmap))
     ref = out["sampled"][1]
     assert np.abs(fmap[:, idx] - ref).max() <= 1e-11 * np.abs(ref).max()
+
+
+def test_graph_cache_stays_bounded_over_a_beta_scan(ul):
+    """Every new recipe (here: 40 values of beta) captures a new graph; the cache keeps the last 16.  The scan must
+    give the same links as the same scan issued sub-step by sub-step."""
+    a = ul.Lattice(8, 4, 0.5, 3)
+    b = ul.Lattice(8, 4, 0.5, 3)
+    for i in range(40):
+        beta = 0.5 + 0.02 * i
+        a.set_beta(beta)
+        b.set_beta(beta)
+        a.sweep(1, 1)
+        for kind in (0, 1):
+            for parity in range(2):
+                for mu in range(4):
+                    b.substep(kind, parity, mu, 0)
+            if kind == 0:
+                b.set_counter(b.get_counter() + 1)
+    assert np.array_equal(a.get_links_raw(), b.get_links_raw()) and a.get_counter() == b.get_counter() == 40
