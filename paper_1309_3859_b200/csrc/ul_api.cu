@@ -663,9 +663,15 @@ int reduce_fields(ul_ctx* c, const ulk::ReplayArgs& ra, bool plane, int plane_a,
     const long long n = (long long)c->n_slab * c->Vs;
     int nb;
     if (plane) {
-        const int N2 = c->Ns * c->Ns, tiles = (N2 + 255) / 256, n_planes = c->n_slab * c->Ns;
-        int splits = NBLK / (tiles * ra.r_max * 3) + 1;
-        splits = splits > 4 ? 4 : splits;
+        const int N2 = c->Ns * c->Ns, tiles = (N2 / 2 + 255) / 256, n_planes = c->n_slab * c->Ns;   // two outputs per thread
+        // one block per SM (214 registers): the number of blocks closest below a whole number of waves of 148, <= 4 splits
+        const int base = tiles * ra.r_max * 3;
+        int splits = 1;
+        double best = 0.0;
+        for (int sp = 1; sp <= 4; ++sp) {
+            const double waves = (double)(base * sp) / 148.0, eff = waves / (double)(long long)(waves + 0.999999);
+            if (eff > best + 1e-9 || (eff > best - 0.02 && sp > splits && base * splits < 148)) { best = eff; splits = sp; }
+        }
         splits = splits > n_planes ? n_planes : splits;
         const size_t smem = (size_t)N2 * (sizeof(double2) + 12 * sizeof(double));
         static bool attr_set = false;

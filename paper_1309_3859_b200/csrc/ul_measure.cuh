@@ -773,11 +773,11 @@ __global__ void __launch_bounds__(256) k_replay_reduce(const ReplayArgs P) {
 // (BJ config 4's "full mid-plane maps"): for every plane (s, x_mu) of the lattice the map is the 2-d cross-correlation
 //   G(b,c) += sum_{p,q} Z(p,q) O(p + b, q + c),   Z = W T on the plane x_mu, O on the plane x_mu + floor(r/2) + a,
 // a dense contraction.  A block owns 256 outputs (b,c) of one (mu, r) for all 12 channels (24 fp64 accumulators per
-// thread), stages Z (fp64 complex) and the 12 O planes (as fp64, transposed so that the lanes of a warp read consecutive
+// thread; two outputs per thread share every O load), stages Z (fp64 complex) and the 12 O planes (as fp64, transposed so that the lanes of a warp read consecutive
 // words) in shared memory, and walks over its share of the planes: ~1.5 instructions per DFMA instead of ~4 for
-// k_replay_reduce.  Ns <= 32 (shared memory); gridDim = (Ns^2/256, r_max, 3 * splits).
+// k_replay_reduce.  Ns <= 32 (shared memory); gridDim = (Ns^2/512, r_max, 3 * splits).
 constexpr int PLANE_MAX_NS = 32;
-__global__ void __launch_bounds__(256) k_replay_reduce_plane(const ReplayArgs P, int fa, int splits) {
+__global__ void __launch_bounds__(256, 1) k_replay_reduce_plane(const ReplayArgs P, int fa, int splits) {
     extern __shared__ double2 sh_z[];                                   // [Ns*Ns] Z(p,q), q fastest
     const Geom& g = P.g;
     const int Ns = g.Ns, N2 = Ns * Ns;
@@ -787,8 +787,9 @@ __global__ void __launch_bounds__(256) k_replay_reduce_plane(const ReplayArgs P,
     const int nu = 1 + (mu % 3), rho = 1 + ((mu + 1) % 3);
     const int stride[4] = {0, 1, Ns, Ns * Ns};
     const long long n = (long long)P.n_slab * g.Vs;
-    const int out = blockIdx.x * blockDim.x + threadIdx.x;              // fp = b + Ns c
-    const int b = out % Ns, c = out / Ns;
+    const int pair = blockIdx.x * blockDim.x + threadIdx.x;             // a thread owns the outputs (b, c0) and (b, c0 + 1):
+    const int b = pair % Ns, c0 = 2 * (pair / Ns);                      // O(q + c0 + 1) of one step is O(q' + c0) of the next
+    const bool live = c0 < Ns;
     const double2* Wm = P.W + ((long long)(mu - 1) * P.r_max + (r - 1)) * n;
     int o_of[6];
     float s_of[6];
@@ -798,9 +799,9 @@ __global__ void __launch_bounds__(256) k_replay_reduce_plane(const ReplayArgs P,
         comp_dirs(mu, comp, pa, pb);
         orient_of(pa, pb, o_of[comp], s_of[comp]);
     }
-    double acc[24];
+    double acc[48];                                                     // [output 0 / 1][ch][re, im]
 #pragma unroll
-    for (int i = 0; i < 24; ++i) acc[i] = 0.0;
+    for (int i = 0; i < 48; ++i) acc[i] = 0.0;
     const int n_planes = P.n_slab * Ns;
     for (int pl = split; pl < n_planes; pl += splits) {
         const int s = pl / Ns, xm = pl - s * Ns;
@@ -823,27 +824,36 @@ __global__ void __launch_bounds__(256) k_replay_reduce_plane(const ReplayArgs P,
             }
         }
         __syncthreads();
-        if (out < N2) {
-            for (int q = 0; q < Ns; ++q) {
-                const int qc = wrapc(q + c, Ns) * Ns;
-                for (int p = 0; p < Ns; ++p) {
+        if (live) {
+            for (int p = 0; p < Ns; ++p) {
+                const int pb = wrapc(p + b, Ns);
+                double o_cur[12];
+#pragma unroll
+                for (int ch = 0; ch < 12; ++ch) o_cur[ch] = sh_o[ch * N2 + c0 * Ns + pb];
+                for (int q = 0; q < Ns; ++q) {
                     const double2 z = sh_z[p * Ns + q];
-                    const int io = qc + wrapc(p + b, Ns);
+                    const int io = wrapc(q + c0 + 1, Ns) * Ns + pb;
 #pragma unroll
                     for (int ch = 0; ch < 12; ++ch) {
-                        const double o = sh_o[ch * N2 + io];
-                        acc[2 * ch] = fma(z.x, o, acc[2 * ch]);
-                        acc[2 * ch + 1] = fma(z.y, o, acc[2 * ch + 1]);
+                        const double o_nxt = sh_o[ch * N2 + io];
+                        acc[2 * ch] = fma(z.x, o_cur[ch], acc[2 * ch]);
+                        acc[2 * ch + 1] = fma(z.y, o_cur[ch], acc[2 * ch + 1]);
+                        acc[24 + 2 * ch] = fma(z.x, o_nxt, acc[24 + 2 * ch]);
+                        acc[24 + 2 * ch + 1] = fma(z.y, o_nxt, acc[24 + 2 * ch + 1]);
+                        o_cur[ch] = o_nxt;
                     }
                 }
             }
         }
     }
-    if (out < N2) {
-        const long long o0 = P.r_max + ((long long)(r - 1) * P.n_fp + out) * 12;
+    if (live) {
         const int nbk = 3 * splits, bk = (mu - 1) * splits + split;
 #pragma unroll
-        for (int i = 0; i < 24; ++i) P.partial[(2 * (o0 + i / 2) + (i & 1)) * nbk + bk] = acc[i];
+        for (int w = 0; w < 2; ++w) {
+            const long long o0 = P.r_max + ((long long)(r - 1) * P.n_fp + (b + Ns * (c0 + w))) * 12;
+#pragma unroll
+            for (int i = 0; i < 24; ++i) P.partial[(2 * (o0 + i / 2) + (i & 1)) * nbk + bk] = acc[24 * w + i];
+        }
     }
 }
 
