@@ -194,12 +194,13 @@ int ul_polyakov(ul_ctx* h, int multihit, double* mean_P);
  * a shard is a lattice of Nt_loc + d time layers whose last slab is a ghost (its first layer holds a copy
  * of the next shard's frozen spatial links; nothing a shard owns depends on the rest of the ghost slab).
  * ul_set_site_offset makes the Philox counters those of the global lattice (offset = t0 * Ns^3 added to
- * the local site index; offset + local volume <= 2^29), so a sharded run reproduces the unsharded one bit
+ * the local site index; it may be negative, down to -V, when ghost layers sit below the shard's first own layer;
+ * offset + local volume <= 2^29), so a sharded run reproduces the unsharded one bit
  * for bit.  ul_slab_partial_product writes prod_{s_begin <= s < s_end} [T](x,s) of the last measurement
  * to a DEVICE buffer double[3][r_max][Ns^3][2] (caller-owned, e.g. a torch tensor): the one array the
  * shards exchange (all-gather) before the slab product of row a10.  paper_1309_3859_b200/sharded.py holds
  * the partition arithmetic and the exchange over torch.distributed. */
-int ul_set_site_offset(ul_ctx* h, uint64_t offset);
+int ul_set_site_offset(ul_ctx* h, int64_t offset);
 int ul_slab_partial_product(ul_ctx* h, int s_begin, int s_end, void* dev_out);
 
 /* Results of the last measurement, HOST buffers (any may be NULL):

@@ -927,9 +927,10 @@ int ul_read_slab_averages(ul_ctx* c, double* out) {
     for (size_t i = 0; i < n; ++i) out[i] *= c->res_inv;
     return UL_OK;
 }
-int ul_set_site_offset(ul_ctx* c, uint64_t offset) {
-    if (!c || offset + (uint64_t)c->V > ((uint64_t)1 << 29)) return fail(c, UL_EINVAL, "site offset + local volume must be <= 2^29");
-    c->site_offset = (uint32_t)offset;
+int ul_set_site_offset(ul_ctx* c, int64_t offset) {
+    if (!c || offset < -(int64_t)c->V || offset + (int64_t)c->V > ((int64_t)1 << 29))
+        return fail(c, UL_EINVAL, "need -V <= site offset and site offset + local volume <= 2^29");
+    c->site_offset = (uint32_t)(uint64_t)offset;      // mod 2^32: a negative offset (ghost layers below t0) wraps back for the own layers
     return UL_OK;
 }
 int ul_slab_partial_product(ul_ctx* c, int s_begin, int s_end, void* dev_out) {

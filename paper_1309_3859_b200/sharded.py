@@ -161,3 +161,90 @@ def main():
 
 if __name__ == "__main__":
     main()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Full (unmasked) sweeps of a t-sharded lattice: SURVEY 8(e)(2).  Nothing is frozen, so a shard's boundary links depend
+# on its neighbours' and one halo layer of the array a sub-step (parity, mu) has just written goes each way after every
+# sub-step (8 exchanges per sweep).  A shard carries GL = 2 ghost layers on each side (two, so that the checkerboard
+# parity of the local lattice is the global one); the kernels also "update" the ghost layers of the array they write,
+# from stale data, and the exchange overwrites them before anything reads them (a sub-step never reads the array it
+# writes, except a link's own old value).
+GL = 2
+
+
+def shard_links_halo(links, t0, nt_loc):
+    """Canonical global links -> the shard's [4][GL + nt_loc + GL][...]: GL layers below, the own layers, GL above."""
+    Nt = links.shape[1]
+    t = (t0 - GL + np.arange(nt_loc + 2 * GL)) % Nt
+    return np.ascontiguousarray(links[:, t])
+
+
+def halo_ranges(nt_loc):
+    """Local time-layer ranges (send_down, send_up, recv_from_below, recv_from_above)."""
+    if nt_loc < GL:
+        raise ValueError("a shard needs at least GL own layers")
+    return (GL, 2 * GL), (nt_loc, nt_loc + GL), (0, GL), (GL + nt_loc, 2 * GL + nt_loc)
+
+
+def internal_view(lat):
+    """The lattice's link tensor as int32 [8 = 2 mu + parity][Nt_ext][Ns^2 Ns/2]: a time layer of one array is contiguous."""
+    import torch
+    return lat.links.view(torch.int32).view(8, lat.Nt, -1)
+
+
+def exchange_halos(view, arr, nt_loc, dist, rank, world):
+    """After a sub-step wrote array `arr`: send the first / last GL own layers down / up, receive the neighbours'."""
+    send_dn, send_up, recv_lo, recv_hi = halo_ranges(nt_loc)
+    dn, up = (rank - 1) % world, (rank + 1) % world
+    ops = [dist.P2POp(dist.isend, view[arr, send_dn[0]:send_dn[1]], dn), dist.P2POp(dist.isend, view[arr, send_up[0]:send_up[1]], up),
+           dist.P2POp(dist.irecv, view[arr, recv_hi[0]:recv_hi[1]], up), dist.P2POp(dist.irecv, view[arr, recv_lo[0]:recv_lo[1]], dn)]
+    for req in dist.batch_isend_irecv(ops):
+        req.wait()
+
+
+class ShardedSweeper:
+    """Full sweeps of one lattice cut in t.  `group`: None under torch.distributed (one shard per process), or the list
+    of all shards when they live in one process (shard-after-shard emulation on one GPU: the exchange is then a copy)."""
+
+    def __init__(self, Ns, Nt, beta, seed, rank, world, links, counter=0, device="cuda:0"):
+        from . import ul
+        if Nt % world or (Nt // world) % 2:
+            raise ValueError("Nt / world must be an even number of layers")
+        self.nt_loc, self.rank, self.world = Nt // world, rank, world
+        self.t0 = rank * self.nt_loc
+        self.lat = ul.Lattice(Ns, self.nt_loc + 2 * GL, beta, seed, device=device)
+        self.lat.set_site_offset((self.t0 - GL) * Ns ** 3)
+        self.lat.set_links(shard_links_halo(links, self.t0, self.nt_loc))
+        self.lat.set_counter(counter)
+        self.view = internal_view(self.lat)
+        self.alg = 0
+
+    def own_links_raw(self):
+        return self.lat.get_links_raw()[:, GL:GL + self.nt_loc]
+
+
+def sharded_sweep(shards, n_hb, n_or, dist=None):
+    """n_hb stochastic sweeps then n_or overrelaxation sweeps (the order of ul_sweep) on `shards`: the list of all
+    shards in one process (emulation) or [this rank's shard] under torch.distributed."""
+    for kind, count in ((2 if shards[0].alg == 1 else 0, n_hb), (1, n_or)):
+        for _ in range(count):
+            for parity in range(2):
+                for mu in range(4):
+                    for sh in shards:
+                        sh.lat.substep(kind, parity, mu, 0)
+                    arr = 2 * mu + parity
+                    if dist is not None:
+                        sh = shards[0]
+                        sh.lat.sync()
+                        exchange_halos(sh.view, arr, sh.nt_loc, dist, sh.rank, sh.world)
+                    else:
+                        n = shards[0].nt_loc
+                        send_dn, send_up, recv_lo, recv_hi = halo_ranges(n)
+                        for sh in shards:                             # all copies are enqueued after all kernels of this sub-step
+                            up, dn = shards[(sh.rank + 1) % len(shards)], shards[(sh.rank - 1) % len(shards)]
+                            up.view[arr, recv_lo[0]:recv_lo[1]].copy_(sh.view[arr, send_up[0]:send_up[1]])
+                            dn.view[arr, recv_hi[0]:recv_hi[1]].copy_(sh.view[arr, send_dn[0]:send_dn[1]])
+            if kind != 1:
+                for sh in shards:
+                    sh.lat.set_counter(sh.lat.get_counter() + 1)

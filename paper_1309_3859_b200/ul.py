@@ -71,7 +71,7 @@ def lib():
         L.ul_set_accum_batch.argtypes = [P, C.c_int]
         L.ul_set_multihit.argtypes = [P, C.c_int]
         L.ul_polyakov.argtypes = [P, C.c_int, P]
-        L.ul_set_site_offset.argtypes = [P, C.c_uint64]
+        L.ul_set_site_offset.argtypes = [P, C.c_int64]
         L.ul_slab_partial_product.argtypes = [P, C.c_int, C.c_int, P]
         L.ul_accumulate.argtypes = [P]
         L.ul_measure_end.argtypes = [P]

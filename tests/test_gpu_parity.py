@@ -1036,3 +1036,27 @@ def test_graph_cache_stays_bounded_over_a_beta_scan(ul):
             if kind == 0:
                 b.set_counter(b.get_counter() + 1)
     assert np.array_equal(a.get_links_raw(), b.get_links_raw()) and a.get_counter() == b.get_counter() == 40
+
+
+@pytest.mark.parametrize("world", [2, 4])
+@pytest.mark.parametrize("alg", [0, 1])
+def test_sharded_full_sweeps_reproduce_the_unsharded_run(ul, world, alg):
+    """Full (unmasked) sweeps of a t-sharded lattice with one halo exchange per sub-step, the shards run one after
+    the other on this GPU and the exchange done as copies: bit-identical to ul_sweep on the whole lattice."""
+    from paper_1309_3859_b200 import sharded
+    Ns, Nt, beta, seed = 8, 16, 0.99, 91
+    full = ul.Lattice(Ns, Nt, beta, seed)
+    full.set_update_algorithm(alg, 1.2)
+    full.sweep(2, 1)
+    links0, ctr0 = full.get_links(), full.get_counter()
+    full.set_links(links0)
+    full.sweep(2, 2)
+    want = full.get_links_raw()
+    shards = [sharded.ShardedSweeper(Ns, Nt, beta, seed, r, world, links0, ctr0) for r in range(world)]
+    for sh in shards:
+        sh.alg = alg
+        sh.lat.set_update_algorithm(alg, 1.2)
+    sharded.sharded_sweep(shards, 2, 2)
+    got = np.concatenate([sh.own_links_raw() for sh in shards], axis=1)
+    assert np.array_equal(got, want)
+    assert all(sh.lat.get_counter() == full.get_counter() for sh in shards)

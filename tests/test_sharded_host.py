@@ -73,3 +73,55 @@ def test_exchange_world_size_2_gloo(tmp_path):
     for r in range(2):
         line = [l for l in outs[r][0].splitlines() if l.startswith("RESULT")][0]
         assert line == f"RESULT {r} True (4,)", line
+
+
+def test_halo_ranges_and_shard_with_halo():
+    from paper_1309_3859_b200 import sharded
+    assert sharded.halo_ranges(8) == ((2, 4), (8, 10), (0, 2), (10, 12))
+    with pytest.raises(ValueError):
+        sharded.halo_ranges(1)
+    Ns, Nt = 4, 12
+    links = np.arange(4 * Nt * Ns ** 3, dtype=np.float32).reshape(4, Nt, Ns, Ns, Ns)
+    s = sharded.shard_links_halo(links, 4, 4)
+    assert s.shape[1] == 8 and np.array_equal(s[:, 2:6], links[:, 4:8])
+    assert np.array_equal(s[:, :2], links[:, 2:4]) and np.array_equal(s[:, 6:], links[:, 8:10])
+    s0 = sharded.shard_links_halo(links, 0, 4)
+    assert np.array_equal(s0[:, :2], links[:, 10:12])                                  # periodic in t
+
+
+HALO_WORKER = r"""
+import os, sys
+sys.path.insert(0, {root!r})
+import torch, torch.distributed as dist
+from paper_1309_3859_b200 import sharded
+dist.init_process_group("gloo", rank=int(os.environ["RANK"]), world_size=2)
+r, nt_loc, GL = dist.get_rank(), 6, sharded.GL
+# stand-in for the internal link view: [8 arrays][GL + nt_loc + GL layers][16 words]; own layers hold 1000 r + 10 arr + t
+view = torch.full((8, nt_loc + 2 * GL, 16), -1, dtype=torch.int32)
+for arr in range(8):
+    for t in range(nt_loc):
+        view[arr, GL + t] = 1000 * r + 10 * arr + t
+sharded.exchange_halos(view, 5, nt_loc, dist, r, 2)
+o = 1 - r
+ok = all(int(view[5, t, 0]) == 1000 * o + 50 + (nt_loc - GL + t) for t in range(GL))                   # from below: the other rank's last layers
+ok = ok and all(int(view[5, GL + nt_loc + t, 0]) == 1000 * o + 50 + t for t in range(GL))              # from above: its first layers
+ok = ok and int(view[4, 0, 0]) == -1 and int(view[5, GL, 0]) == 1000 * r + 50                         # nothing else touched
+dist.barrier()
+print("RESULT", r, bool(ok))
+dist.destroy_process_group()
+"""
+
+
+def test_halo_exchange_world_size_2_gloo(tmp_path):
+    script = tmp_path / "halo_worker.py"
+    script.write_text(HALO_WORKER.format(root=ROOT))
+    port = 33500 + os.getpid() % 2000
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True))
+    outs = [p.communicate(timeout=240) for p in procs]
+    assert all(p.returncode == 0 for p in procs), outs
+    for r in range(2):
+        line = [l for l in outs[r][0].splitlines() if l.startswith("RESULT")][0]
+        assert line == f"RESULT {r} True", line
