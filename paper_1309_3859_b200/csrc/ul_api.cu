@@ -130,6 +130,11 @@ struct ul_ctx {
     bool multihit = false;   // ul_set_multihit: sums of T at r >= 2 from multihit temporal links
     bool skip_colsum = false; // replayed configurations: their plaquette column sums are already in the vacuum sums
     float* staging2 = nullptr; // second configuration copy (two-level replay)
+    char* plane_buf = nullptr; // full-plane maps through the transverse DFT: Ohat, group partials, Ghat (library-owned)
+    size_t plane_bytes = 0;
+    bool plane_fresh = true;   // Ghat holds nothing yet
+    double plane_scale = 0.0;
+    int plane_r_max = 0;
     bool replay = false;     // ul_multilevel_replay in progress: no TO sums, fields reduced on the fly in pass 2
     bool acc_fresh = true;   // the inner sums A2, B2 hold nothing yet: the next pass writes instead of adding
     Workspace ws;
@@ -311,6 +316,7 @@ int open_measurement(ul_ctx* c, int d_in, int d_out, int r_max, const int* fps, 
     c->n_acc = 0;
     c->n_pending = 0;
     c->acc_fresh = true;
+    c->plane_fresh = true;
     c->have = false;
     if (n_fp > 0) UL_CUDA(c, cudaMemcpyAsync(c->work + w.fps, fps, sizeof(int) * 3 * (size_t)n_fp, cudaMemcpyHostToDevice, c->stream));
     if (w.partial > w.A4) UL_CUDA(c, cudaMemsetAsync(c->work + w.A4, 0, w.partial - w.A4, c->stream));   // A4, B4 (A2, B2: first pass writes)
@@ -512,6 +518,7 @@ int ul_destroy(ul_ctx* c) {
     if (c->own_work && c->work) cudaFree(c->work);
     if (c->staging) cudaFree(c->staging);
     if (c->staging2) cudaFree(c->staging2);
+    if (c->plane_buf) cudaFree(c->plane_buf);
     if (c->scratch) cudaFree(c->scratch);
     if (c->hb_queue) cudaFree(c->hb_queue);
     for (auto& e : c->graphs) if (e.exec) cudaGraphExecDestroy(e.exec);
@@ -663,21 +670,43 @@ int reduce_fields(ul_ctx* c, const ulk::ReplayArgs& ra, bool plane, int plane_a,
     const long long n = (long long)c->n_slab * c->Vs;
     int nb;
     if (plane) {
-        const int N2 = c->Ns * c->Ns, tiles = (N2 / 2 + 255) / 256, n_planes = c->n_slab * c->Ns;   // two outputs per thread
-        // one block per SM (214 registers): the number of blocks closest below a whole number of waves of 148, <= 4 splits
-        const int base = tiles * ra.r_max * 3;
-        int splits = 1;
-        double best = 0.0;
-        for (int sp = 1; sp <= 4; ++sp) {
-            const double waves = (double)(base * sp) / 148.0, eff = waves / (double)(long long)(waves + 0.999999);
-            if (eff > best + 1e-9 || (eff > best - 0.02 && sp > splits && base * splits < 148)) { best = eff; splits = sp; }
+        // full transverse plane: DFT route (k_plane_*), results go to Ghat and are transformed back once per measurement
+        const int N2 = c->Ns * c->Ns, R = ra.r_max, n_planes = c->n_slab * c->Ns;
+        int groups = (148 + R - 1) / R;
+        groups = groups > n_planes ? n_planes : groups;
+        const size_t oh_b = (size_t)12 * n_planes * N2 * 16, ghp_b = (size_t)groups * R * 12 * N2 * 16, gh_b = (size_t)R * 12 * N2 * 16;
+        const size_t need = align_up(oh_b) + align_up(ghp_b) + align_up(gh_b);
+        if (need > c->plane_bytes) {
+            UL_CUDA(c, cudaStreamSynchronize(c->stream));
+            if (c->plane_buf) cudaFree(c->plane_buf);
+            c->plane_buf = nullptr; c->plane_bytes = 0;
+            void* pb = nullptr;
+            UL_CUDA(c, cudaMalloc(&pb, need));
+            c->plane_buf = (char*)pb; c->plane_bytes = need;
+            c->plane_fresh = true;
         }
-        splits = splits > n_planes ? n_planes : splits;
-        const size_t smem = (size_t)N2 * (sizeof(double2) + 12 * sizeof(double));
+        double2* Oh = (double2*)c->plane_buf;
+        double2* Ghp = (double2*)(c->plane_buf + align_up(oh_b));
+        double2* Gh = (double2*)(c->plane_buf + align_up(oh_b) + align_up(ghp_b));
+        if (c->plane_fresh) { UL_CUDA(c, cudaMemsetAsync(Gh, 0, gh_b, c->stream)); c->plane_fresh = false; }
+        c->plane_scale = scale; c->plane_r_max = R;
+        const size_t smem = (size_t)3 * N2 * sizeof(double2);
         static bool attr_set = false;
-        if (!attr_set) { cudaFuncSetAttribute(ulk::k_replay_reduce_plane, cudaFuncAttributeMaxDynamicSharedMemorySize, ulk::PLANE_MAX_NS * ulk::PLANE_MAX_NS * 112); attr_set = true; }
-        ulk::k_replay_reduce_plane<<<dim3(tiles, ra.r_max, 3 * splits), 256, smem, c->stream>>>(ra, plane_a, splits);
-        nb = 3 * splits;
+        if (!attr_set) {
+            const int cap = 3 * ulk::PLANE_MAX_NS * ulk::PLANE_MAX_NS * (int)sizeof(double2);
+            cudaFuncSetAttribute(ulk::k_plane_dft_o, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+            cudaFuncSetAttribute(ulk::k_plane_spectral, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+            cudaFuncSetAttribute(ulk::k_plane_idft, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+            attr_set = true;
+        }
+        const long long ne = (long long)R * 12 * N2;
+        for (int mu = 1; mu <= 3; ++mu) {
+            ulk::k_plane_dft_o<<<dim3(n_planes, 12), N2, smem, c->stream>>>(ra, mu, Oh);
+            ulk::k_plane_spectral<<<dim3(R, groups, 2), N2, smem, c->stream>>>(ra, mu, plane_a, Oh, Ghp);
+            ulk::k_plane_gh_accum<<<(unsigned)((ne + 255) / 256), 256, 0, c->stream>>>(Ghp, groups, ne, Gh);
+        }
+        c->launches += 9;
+        return cudaGetLastError() == cudaSuccess ? UL_OK : fail(c, UL_ECUDA, "plane reduction launch");
     } else {
         nb = replay_blocks(n);
         ulk::k_replay_reduce<<<dim3(nb, ra.r_max * ra.n_fp), 256, 0, c->stream>>>(ra);
@@ -685,6 +714,20 @@ int reduce_fields(ul_ctx* c, const ulk::ReplayArgs& ra, bool plane, int plane_a,
     ulk::k_sum_partials<<<2 * (n_entries - ra.r_max), 256, 0, c->stream>>>(ra.partial + (size_t)2 * ra.r_max * nb, nb, res + 2 * ra.r_max, scale, 1);
     c->launches += 2;
     return cudaGetLastError() == cudaSuccess ? UL_OK : fail(c, UL_ECUDA, "field reduction launch");
+}
+
+// Ghat -> the field map in the result buffer (once per measurement, before finish())
+int plane_finish(ul_ctx* c, int r_max) {
+    const int N2 = c->Ns * c->Ns, n_planes = c->n_slab * c->Ns;
+    int groups = (148 + r_max - 1) / r_max;
+    groups = groups > n_planes ? n_planes : groups;
+    const size_t oh_b = (size_t)12 * n_planes * N2 * 16, ghp_b = (size_t)groups * r_max * 12 * N2 * 16;
+    const double2* Gh = (const double2*)(c->plane_buf + align_up(oh_b) + align_up(ghp_b));
+    double2* field = (double2*)(wsp<double>(c, c->ws.result) + 2 * r_max);
+    ulk::k_plane_idft<<<dim3(r_max, 12), N2, (size_t)3 * N2 * sizeof(double2), c->stream>>>(Gh, c->Ns, c->plane_scale, field);
+    c->launches += 1;
+    c->plane_fresh = true;
+    return cudaGetLastError() == cudaSuccess ? UL_OK : fail(c, UL_ECUDA, "k_plane_idft launch");
 }
 
 // Single-level measurement by replay: the same estimator, trajectory and results as
@@ -750,6 +793,7 @@ int ul_multilevel_replay(ul_ctx* c, int d, int n_sub, int r_max, const int* fps,
         rc = reduce_fields(c, ra, plane, plane_a, n_entries, scale);
         if (rc) return bail(rc);
     }
+    if (plane) { rc = plane_finish(c, r_max); if (rc) return bail(rc); }
     rc = finish(c, wsp<double2>(c, c->ws.A2), nullptr, c->n_slab, inv, inv);
     c->replay = false;
     return rc;
@@ -879,6 +923,7 @@ int ul_multilevel2_replay(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, i
         if (cudaGetLastError() != cudaSuccess) return bail(fail(c, UL_ECUDA, "two-level replay, pass 2"));
     }
     c->skip_colsum = false;
+    if (plane) { rc = plane_finish(c, r_max); if (rc) return bail(rc); }
     rc = finish(c, ca.A4, nullptr, c->n_outer, 1.0 / (double)n_out, 1.0 / ((double)n_in * (double)n_out));
     c->replay = false;
     return rc;

@@ -769,92 +769,134 @@ __global__ void __launch_bounds__(256) k_replay_reduce(const ReplayArgs P) {
     }
 }
 
-// The same reduction when the field points are a FULL transverse plane, fp = b + Ns c <-> offset (a, b, c) with one a
-// (BJ config 4's "full mid-plane maps"): for every plane (s, x_mu) of the lattice the map is the 2-d cross-correlation
-//   G(b,c) += sum_{p,q} Z(p,q) O(p + b, q + c),   Z = W T on the plane x_mu, O on the plane x_mu + floor(r/2) + a,
-// a dense contraction.  A block owns 256 outputs (b,c) of one (mu, r) for all 12 channels (24 fp64 accumulators per
-// thread; two outputs per thread share every O load), stages Z (fp64 complex) and the 12 O planes (as fp64, transposed so that the lanes of a warp read consecutive
-// words) in shared memory, and walks over its share of the planes: ~1.5 instructions per DFMA instead of ~4 for
-// k_replay_reduce.  Ns <= 32 (shared memory); gridDim = (Ns^2/512, r_max, 3 * splits).
-constexpr int PLANE_MAX_NS = 32;
-__global__ void __launch_bounds__(256, 1) k_replay_reduce_plane(const ReplayArgs P, int fa, int splits) {
-    extern __shared__ double2 sh_z[];                                   // [Ns*Ns] Z(p,q), q fastest
+constexpr int PLANE_MAX_NS = 32;   // the DFT route runs one block of Ns^2 threads per plane
+
+// ---------------------------------------------------------------- full-plane maps through the transverse DFT
+// When the field points are a FULL transverse plane, fp = b + Ns c <-> offset (a, b, c) with one a (BJ config 4's "full
+// mid-plane maps"), the map of one lattice plane (s, x_mu) is a 2-d cross-correlation, Z = W T on the plane x_mu, O on the
+// plane x_mu + floor(r/2) + a:
+// G(b,c) = sum_{p,q} Z(p,q) O(p+b, q+c)  <=>  Ghat(k,l) = Zhat(-k,-l) Ohat(k,l)  with the 2-d DFT over the transverse plane:
+// 2 Ns^3 complex MACs per plane for the transforms instead of Ns^4 per plane and channel for the direct sum.  The DFT is
+// done as two small dense matrix products with the Ns x Ns matrix W[j][k] = e^{-2 pi i jk/Ns} (any Ns, no radix
+// restriction), in fp64, one block of Ns^2 threads per plane (Ns <= 32).  Ohat of the 12 channels of one direction mu is
+// tabulated first (k_plane_dft_o); k_plane_spectral transforms Z = W T of every plane of its group, multiplies with the
+// 12 Ohat planes and keeps 12 complex sums per (k,l) in registers; k_plane_gh_accum adds the groups' partial sums to
+// Ghat; k_plane_idft turns Ghat into the map once per measurement.  Everything is owned by one thread per entry and
+// summed in a fixed order: bitwise reproducible.
+__device__ __forceinline__ void dft_matrix_to_smem(double2* Wm, int Ns, bool conjugate) {
+    for (int e = threadIdx.x; e < Ns * Ns; e += blockDim.x) {
+        const int j = e / Ns, k = e - j * Ns;
+        double sn, cs;
+        sincospi(2.0 * (double)((j * k) % Ns) / (double)Ns, &sn, &cs);
+        Wm[e] = make_double2(cs, conjugate ? sn : -sn);
+    }
+}
+// Ahat = M A M for the plane in A (thread e = k*Ns + l); M symmetric; T is scratch.  Returns the thread's own entry.
+__device__ __forceinline__ double2 dft2_entry(const double2* A, double2* T, const double2* M, int Ns) {
+    const int e = threadIdx.x, k = e / Ns, l = e - k * Ns;
+    double2 t = make_double2(0.0, 0.0);
+    for (int p = 0; p < Ns; ++p) {                                       // T[k][l] = sum_p M[k][p] A[p][l]
+        const double2 m = M[k * Ns + p], a = A[p * Ns + l];
+        t.x = fma(m.x, a.x, fma(-m.y, a.y, t.x));
+        t.y = fma(m.x, a.y, fma(m.y, a.x, t.y));
+    }
+    T[e] = t;
+    __syncthreads();
+    double2 r = make_double2(0.0, 0.0);
+    for (int q = 0; q < Ns; ++q) {                                       // R[k][l] = sum_q T[k][q] M[q][l]
+        const double2 a = T[k * Ns + q], m = M[q * Ns + l];
+        r.x = fma(a.x, m.x, fma(-a.y, m.y, r.x));
+        r.y = fma(a.x, m.y, fma(a.y, m.x, r.y));
+    }
+    __syncthreads();
+    return r;
+}
+
+// Ohat[ch][plane][k*Ns + l] for direction mu; grid (n_planes, 12), block Ns^2, dynamic smem 3 Ns^2 double2
+__global__ void __launch_bounds__(1024, 1) k_plane_dft_o(const ReplayArgs P, int mu, double2* __restrict__ Oh) {
+    extern __shared__ double2 sh[];
     const Geom& g = P.g;
     const int Ns = g.Ns, N2 = Ns * Ns;
-    double* sh_o = reinterpret_cast<double*>(sh_z + N2);                // [12][Ns*Ns] O^T (fp64 copies: no conversion in the loop): index (q*Ns + p)
-    const int r = blockIdx.y + 1;
-    const int mu = blockIdx.z / splits + 1, split = blockIdx.z - (mu - 1) * splits;
+    double2 *Wm = sh, *A = sh + N2, *T = sh + 2 * N2;
     const int nu = 1 + (mu % 3), rho = 1 + ((mu + 1) % 3);
     const int stride[4] = {0, 1, Ns, Ns * Ns};
     const long long n = (long long)P.n_slab * g.Vs;
-    const int pair = blockIdx.x * blockDim.x + threadIdx.x;             // a thread owns the outputs (b, c0) and (b, c0 + 1):
-    const int b = pair % Ns, c0 = 2 * (pair / Ns);                      // O(q + c0 + 1) of one step is O(q' + c0) of the next
-    const bool live = c0 < Ns;
+    const int pl = blockIdx.x, s = pl / Ns, xm = pl - s * Ns, ch = blockIdx.y;
+    int pa, pb, o;
+    float sgn;
+    comp_dirs(mu, ch >> 1, pa, pb);
+    orient_of(pa, pb, o, sgn);
+    dft_matrix_to_smem(Wm, Ns, false);
+    const int e = threadIdx.x, p = e / Ns, q = e - p * Ns;
+    const long long zs = (long long)s * g.Vs + xm * stride[mu] + p * stride[nu] + q * stride[rho];
+    const float v = P.Ot[(long long)(2 * o + (ch & 1)) * n + zs];
+    A[e] = make_double2((double)((ch & 1) ? sgn * v : v), 0.0);
+    __syncthreads();
+    Oh[((long long)ch * gridDim.x + pl) * N2 + e] = dft2_entry(A, T, Wm, Ns);
+}
+
+// partial[(group*r_max + r-1)*12 + ch][k*Ns + l] = sum over the planes of the group of Zhat(-k,-l) Ohat_ch(k,l);
+// grid (r_max, groups, 2 channel halves), block Ns^2 (<= 1024 threads: 64 registers each, hence 6 channels per block)
+__global__ void __launch_bounds__(1024, 1) k_plane_spectral(const ReplayArgs P, int mu, int fa, const double2* __restrict__ Oh, double2* __restrict__ Ghp) {
+    extern __shared__ double2 sh[];
+    const Geom& g = P.g;
+    const int Ns = g.Ns, N2 = Ns * Ns;
+    double2 *Wc = sh, *A = sh + N2, *T = sh + 2 * N2;
+    const int nu = 1 + (mu % 3), rho = 1 + ((mu + 1) % 3);
+    const int stride[4] = {0, 1, Ns, Ns * Ns};
+    const long long n = (long long)P.n_slab * g.Vs;
+    const int r = blockIdx.x + 1, n_planes = P.n_slab * Ns;
     const double2* Wm = P.W + ((long long)(mu - 1) * P.r_max + (r - 1)) * n;
-    int o_of[6];
-    float s_of[6];
+    dft_matrix_to_smem(Wc, Ns, true);                                    // conj(W): Zhat(-k,-l)
+    const int e = threadIdx.x, p = e / Ns, q = e - p * Ns;
+    const int ch0 = 6 * blockIdx.z;
+    double2 acc[6];
 #pragma unroll
-    for (int comp = 0; comp < 6; ++comp) {
-        int pa, pb;
-        comp_dirs(mu, comp, pa, pb);
-        orient_of(pa, pb, o_of[comp], s_of[comp]);
-    }
-    double acc[48];                                                     // [output 0 / 1][ch][re, im]
-#pragma unroll
-    for (int i = 0; i < 48; ++i) acc[i] = 0.0;
-    const int n_planes = P.n_slab * Ns;
-    for (int pl = split; pl < n_planes; pl += splits) {
+    for (int ch = 0; ch < 6; ++ch) acc[ch] = make_double2(0.0, 0.0);
+    for (int pl = blockIdx.y; pl < n_planes; pl += gridDim.y) {
         const int s = pl / Ns, xm = pl - s * Ns;
-        const int xo = modc(xm + r / 2 + fa, Ns);                       // plane of the plaquettes (anchor, DESIGN R10)
-        const int ym = wrapc(xm + r, Ns);
+        const int xs = xm * stride[mu] + p * stride[nu] + q * stride[rho];
+        const int ys = wrapc(xm + r, Ns) * stride[mu] + p * stride[nu] + q * stride[rho];
+        const long long j = (long long)s * g.Vs + xs;
+        const double2 u = P.U[j], v = P.U[(long long)s * g.Vs + ys];
+        const double2 Tj = make_double2(fma(v.x, u.x, v.y * u.y), fma(v.y, u.x, -(v.x * u.y)));
+        A[e] = cmul(Wm[j], Tj);
         __syncthreads();
-        for (int e = threadIdx.x; e < N2; e += blockDim.x) {            // e = p*Ns + q  (p along nu, q along rho)
-            const int p = e / Ns, q = e - p * Ns;
-            const int xs = xm * stride[mu] + p * stride[nu] + q * stride[rho];
-            const int ys = ym * stride[mu] + p * stride[nu] + q * stride[rho];
-            const long long j = (long long)s * g.Vs + xs;
-            const double2 u = P.U[j], v = P.U[(long long)s * g.Vs + ys];
-            const double2 T = make_double2(fma(v.x, u.x, v.y * u.y), fma(v.y, u.x, -(v.x * u.y)));
-            sh_z[e] = cmul(Wm[j], T);
-            const long long zs = (long long)s * g.Vs + xo * stride[mu] + p * stride[nu] + q * stride[rho];
+        const double2 zh = dft2_entry(A, T, Wc, Ns);
+        const int plo = s * Ns + modc(xm + r / 2 + fa, Ns);              // plane of the plaquettes (anchor, DESIGN R10)
 #pragma unroll
-            for (int comp = 0; comp < 6; ++comp) {
-                sh_o[(2 * comp) * N2 + q * Ns + p] = (double)P.Ot[(long long)(2 * o_of[comp]) * n + zs];
-                sh_o[(2 * comp + 1) * N2 + q * Ns + p] = (double)(s_of[comp] * P.Ot[(long long)(2 * o_of[comp] + 1) * n + zs]);
-            }
-        }
-        __syncthreads();
-        if (live) {
-            for (int p = 0; p < Ns; ++p) {
-                const int pb = wrapc(p + b, Ns);
-                double o_cur[12];
-#pragma unroll
-                for (int ch = 0; ch < 12; ++ch) o_cur[ch] = sh_o[ch * N2 + c0 * Ns + pb];
-                for (int q = 0; q < Ns; ++q) {
-                    const double2 z = sh_z[p * Ns + q];
-                    const int io = wrapc(q + c0 + 1, Ns) * Ns + pb;
-#pragma unroll
-                    for (int ch = 0; ch < 12; ++ch) {
-                        const double o_nxt = sh_o[ch * N2 + io];
-                        acc[2 * ch] = fma(z.x, o_cur[ch], acc[2 * ch]);
-                        acc[2 * ch + 1] = fma(z.y, o_cur[ch], acc[2 * ch + 1]);
-                        acc[24 + 2 * ch] = fma(z.x, o_nxt, acc[24 + 2 * ch]);
-                        acc[24 + 2 * ch + 1] = fma(z.y, o_nxt, acc[24 + 2 * ch + 1]);
-                        o_cur[ch] = o_nxt;
-                    }
-                }
-            }
+        for (int ch = 0; ch < 6; ++ch) {
+            const double2 oh = Oh[((long long)(ch0 + ch) * n_planes + plo) * N2 + e];
+            acc[ch].x = fma(zh.x, oh.x, fma(-zh.y, oh.y, acc[ch].x));
+            acc[ch].y = fma(zh.x, oh.y, fma(zh.y, oh.x, acc[ch].y));
         }
     }
-    if (live) {
-        const int nbk = 3 * splits, bk = (mu - 1) * splits + split;
 #pragma unroll
-        for (int w = 0; w < 2; ++w) {
-            const long long o0 = P.r_max + ((long long)(r - 1) * P.n_fp + (b + Ns * (c0 + w))) * 12;
-#pragma unroll
-            for (int i = 0; i < 24; ++i) P.partial[(2 * (o0 + i / 2) + (i & 1)) * nbk + bk] = acc[24 * w + i];
-        }
-    }
+    for (int ch = 0; ch < 6; ++ch) Ghp[(((long long)blockIdx.y * P.r_max + (r - 1)) * 12 + ch0 + ch) * N2 + e] = acc[ch];
+}
+
+// Gh[(r-1)*12 + ch][kl] += sum_groups Ghp[group][...]; one thread per entry
+__global__ void __launch_bounds__(256) k_plane_gh_accum(const double2* __restrict__ Ghp, int groups, long long n_entries, double2* __restrict__ Gh) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_entries) return;
+    double2 a = Gh[i];
+    for (int gidx = 0; gidx < groups; ++gidx) { const double2 v = Ghp[(long long)gidx * n_entries + i]; a.x += v.x; a.y += v.y; }
+    Gh[i] = a;
+}
+
+// field[((r-1)*Ns^2 + (b + Ns c))*12 + ch] = scale/Ns^2 * sum_{k,l} Gh(k,l) e^{+2 pi i (kb + lc)/Ns}; grid (r_max, 12), block Ns^2
+__global__ void __launch_bounds__(1024, 1) k_plane_idft(const double2* __restrict__ Gh, int Ns, double scale, double2* __restrict__ field) {
+    extern __shared__ double2 sh[];
+    const int N2 = Ns * Ns;
+    double2 *Wc = sh, *A = sh + N2, *T = sh + 2 * N2;
+    const int r1 = blockIdx.x, ch = blockIdx.y, e = threadIdx.x;
+    dft_matrix_to_smem(Wc, Ns, true);
+    A[e] = Gh[((long long)r1 * 12 + ch) * N2 + e];
+    __syncthreads();
+    const double2 v = dft2_entry(A, T, Wc, Ns);                          // entry e = b*Ns + c
+    const int b = e / Ns, c = e - b * Ns;
+    const double f = scale / (double)N2;
+    field[((long long)r1 * N2 + (b + Ns * c)) * 12 + ch] = make_double2(v.x * f, v.y * f);
 }
 
 // vacuum[ch] = (1/(3 V n_acc)) sum_mu sgn * colsum[orient(mu, comp)][kind]
