@@ -1060,3 +1060,51 @@ def test_sharded_full_sweeps_reproduce_the_unsharded_run(ul, world, alg):
     got = np.concatenate([sh.own_links_raw() for sh in shards], axis=1)
     assert np.array_equal(got, want)
     assert all(sh.lat.get_counter() == full.get_counter() for sh in shards)
+
+
+# ----------------------------------------------------------------------------- degenerate and extreme shapes
+@pytest.mark.parametrize("Ns,Nt,d", [(2, 2, 2), (2, 4, 1), (4, 2, 2), (6, 6, 6), (4, 8, 8), (10, 4, 2)])
+def test_degenerate_shapes_against_oracle(ul, ulo, Ns, Nt, d):
+    """Smallest lattice (2^4 sites wrap onto themselves), a single slab (d = Nt), thickness 1 (every spatial link
+    frozen), r_max = Ns/2 (the largest separation), rows that are not a multiple of the vector width (Ns = 6, 10):
+    one heatbath and one overrelaxation sweep link by link, then the frozen-configuration estimator, stored and replay."""
+    beta, R = 0.9, Ns // 2
+    o = ulo.Oracle(Ns, Nt, beta, 8)
+    ob = ulo.Oracle(Ns, Nt, beta, 8)
+    g = ul.Lattice(Ns, Nt, beta, 8)
+    assert same_links(g.get_links(), o.get_links())
+    for kind in (0, 1):
+        for slab in (0, d):
+            for parity in range(2):
+                for mu in range(4):
+                    before = o.get_links()
+                    ob.set_links(before)
+                    g.set_links(before)
+                    g.set_counter(o.get_counter())
+                    o.substep(kind, parity, mu, slab)
+                    g.substep(kind, parity, mu, slab)
+                    check_links(g.get_links(), o.get_links(), before, ob, (kind, slab, parity, mu), allow_frac=1e-3)
+    fps = [(0, 0, 0), (0, 1, 0), (-1, 0, 1)]
+    g.set_links(o.get_links())
+    o.multilevel(d, 0, R, fps)
+    co, fo, vo = o.read_correlators()
+    Vs = Ns ** 3
+    for call in (g.multilevel, g.multilevel_replay):
+        call(d, 0, R, fps)
+        cg, fg, vg = g.read_correlators()
+        assert np.abs(g.read_slab_averages() - o.read_slab_averages()).max() < 1e-5
+        for got, want, n in ((cg, co, 3 * Vs), (fg, fo, 3 * Vs * Nt), (vg, vo, 3 * Vs * Nt)):
+            ok, worst = rel_ok(got, want, n)
+            assert ok, worst
+    g.multilevel(d, 3, R, fps)                                      # and the sub-update loop runs (d = 1: nothing spatial moves)
+    assert np.all(np.isfinite(g.read_correlators()[0]))
+
+
+def test_beta_zero_heatbath_is_uniform_on_device(ul):
+    from scipy import stats
+    g = ul.Lattice(16, 4, 0.0, 5)
+    g.init(0)
+    g.sweep(1, 0)
+    th = g.get_links().astype(np.float64).ravel()
+    _, p = stats.kstest(th, lambda x: (x + np.pi) / (2 * np.pi))
+    assert p > 1e-3 and abs(g.plaquette()[0]) < 0.01
