@@ -43,6 +43,13 @@ struct ulo_ctx {
     int res_r_max = 0, res_n_fp = 0, res_n_slab = 0;
     std::vector<double> corr, field, vacuum;
     std::vector<cplx> slab_avg;    // [3][r_max][n_slab][Vs]
+    std::vector<cplx> slab_field_avg;  // [3][r_max][n_slab][n_fp][12][Vs]
+    // open two-level measurement (S8(c)-O7): outer sums and the number of outer iterations combined so far
+    bool open2 = false;
+    int d_out = 0, n_outer = 0;
+    long n_comb = 0;
+    std::vector<cplx> A4, B4;      // [3][r_max][n_outer][Vs], [3][r_max][n_outer][n_fp][12][Vs]
+    std::vector<double> vac4;      // [12]
     std::string err;
 };
 
@@ -357,6 +364,7 @@ static void reduce_result(ulo_ctx* c, const std::vector<cplx>& avT, const std::v
     }
     c->vacuum = vac;
     c->slab_avg = avT;
+    c->slab_field_avg = avTO;
     c->res_r_max = R; c->res_n_fp = F; c->res_n_slab = n_slab;
     c->have = true;
 }
@@ -464,7 +472,7 @@ int ulo_accumulate(ulo_ctx* c) {
 }
 int ulo_measure_end(ulo_ctx* c) {
     if (!c) return ULO_EINVAL;
-    if (!c->open || c->n_acc == 0) { c->err = "nothing accumulated"; return ULO_ESTATE; }
+    if (!c->open || c->open2 || c->n_acc == 0) { c->err = "nothing accumulated (or a two-level measurement is open)"; return ULO_ESTATE; }
     close_measurement(c);
     return ULO_OK;
 }
@@ -484,57 +492,95 @@ int ulo_multilevel(ulo_ctx* c, int d, int n_sub, int r_max, const int* fps, int 
     return ULO_OK;
 }
 
-// two levels, S8(c)-O7 (Eq. 27, Eqs. 32-33 P:343-347 with the t+2 reading DESIGN R7, Alg. 1)
-int ulo_multilevel2(ulo_ctx* c, int d_in, int n_in, int d_out, int n_out, int r_max, const int* fps, int n_fp) {
-    if (!c || n_in < 1 || n_out < 1) return ULO_EINVAL;
+// two levels, S8(c)-O7 (Eq. 27, Eqs. 32-33 P:343-347 with the t+2 reading DESIGN R7, Alg. 1).
+// The three steps below are Alg. 1 lines 5 (open the outer sums), 16 (combine the inner averages of one outer
+// iteration into T^(4), TO^(4) and add them to the outer sums) and 18 (outer averages, slab product); they are also
+// exported as test hooks so that a harness can feed configurations one by one (ulo_accumulate in between).
+static int begin2(ulo_ctx* c, int d_in, int d_out, int r_max, const int* fps, int n_fp) {
     int rc = check_meas_args(c, d_in, r_max, fps, n_fp);
     if (rc) return rc;
     if (d_out < d_in || d_out % d_in != 0 || c->Nt % d_out != 0) { c->err = "need d_in | d_out | Nt"; return ULO_EINVAL; }
-    const int m = d_out / d_in, n_outer = c->Nt / d_out, R = r_max, F = n_fp;
-    std::vector<cplx> A4, B4;
-    std::vector<double> vac4(12, 0.0);
+    c->d_out = d_out; c->n_outer = c->Nt / d_out; c->n_comb = 0;
     try {
-        A4.assign((size_t)3 * R * n_outer * c->Vs, cplx(0, 0));
-        B4.assign((size_t)3 * R * n_outer * F * 12 * c->Vs, cplx(0, 0));
+        c->A4.assign((size_t)3 * r_max * c->n_outer * c->Vs, cplx(0, 0));
+        c->B4.assign((size_t)3 * r_max * c->n_outer * n_fp * 12 * c->Vs, cplx(0, 0));
+        open_measurement(c, d_in, r_max, fps, n_fp);                         // A2, B2 <- 0
     } catch (...) { c->err = "accumulators do not fit"; return ULO_ENOMEM; }
+    c->vac4.assign(12, 0.0);
+    c->open2 = true;
+    return ULO_OK;
+}
+static void combine2(ulo_ctx* c) {
+    const int m = c->d_out / c->d, n_outer = c->n_outer, R = c->r_max, F = c->n_fp;
+    const double inv = 1.0 / (double)c->n_acc;                               // [.] = inner sum / n_in
+    for (long xs = 0; xs < c->Vs; ++xs)
+        for (int mu = 1; mu <= 3; ++mu)
+            for (int r = 1; r <= R; ++r)
+                for (int S = 0; S < n_outer; ++S) {
+                    cplx t4(1, 0);
+                    for (int i = 0; i < m; ++i) t4 *= c->A[A_idx(c, mu, r, S * m + i, xs)] * inv;          // Eq. 32
+                    c->A4[((((size_t)(mu - 1) * R + (r - 1)) * n_outer + S) * c->Vs) + xs] += t4;
+                    for (int fp = 0; fp < F; ++fp)
+                        for (int ch = 0; ch < 12; ++ch) {
+                            cplx to4(0, 0);
+                            for (int i = 0; i < m; ++i) {                                                   // Eq. 33
+                                cplx term = c->B[B_idx(c, mu, r, S * m + i, fp, ch, xs)] * inv;
+                                for (int i2 = 0; i2 < m; ++i2)
+                                    if (i2 != i) term *= c->A[A_idx(c, mu, r, S * m + i2, xs)] * inv;
+                                to4 += term;
+                            }
+                            c->B4[((((((size_t)(mu - 1) * R + (r - 1)) * n_outer + S) * F + fp) * 12 + ch) * c->Vs) + xs] += to4;
+                        }
+                }
+    for (int ch = 0; ch < 12; ++ch) c->vac4[ch] += c->vac_sum[ch] * inv;
+    c->n_comb += 1;
+    // the next outer iteration starts its inner sums from zero
+    std::fill(c->A.begin(), c->A.end(), cplx(0, 0));
+    std::fill(c->B.begin(), c->B.end(), cplx(0, 0));
+    std::fill(c->vac_sum.begin(), c->vac_sum.end(), 0.0);
+    c->n_acc = 0;
+}
+static void end2(ulo_ctx* c) {
+    const double invo = 1.0 / (double)c->n_comb;                             // [.] = outer sum / n_out
+    for (auto& z : c->A4) z *= invo;
+    for (auto& z : c->B4) z *= invo;
+    for (auto& v : c->vac4) v *= invo;
+    reduce_result(c, c->A4, c->B4, c->n_outer, c->vac4);
+    c->open = false; c->open2 = false;
+    c->A.clear(); c->A.shrink_to_fit();
+    c->B.clear(); c->B.shrink_to_fit();
+    c->A4.clear(); c->A4.shrink_to_fit();
+    c->B4.clear(); c->B4.shrink_to_fit();
+}
+int ulo_multilevel2(ulo_ctx* c, int d_in, int n_in, int d_out, int n_out, int r_max, const int* fps, int n_fp) {
+    if (!c || n_in < 1 || n_out < 1) return ULO_EINVAL;
+    int rc = begin2(c, d_in, d_out, r_max, fps, n_fp);
+    if (rc) return rc;
     for (int J = 0; J < n_out; ++J) {
         for (int k = 0; k < c->sub_k; ++k) compound(c, c->sub_hb, c->sub_or, d_out);
-        try { open_measurement(c, d_in, r_max, fps, n_fp); } catch (...) { c->err = "accumulators do not fit"; return ULO_ENOMEM; }
         for (int j = 0; j < n_in; ++j) {
             for (int k = 0; k < c->sub_k; ++k) compound(c, c->sub_hb, c->sub_or, d_in);
             accumulate(c);
         }
-        const double inv = 1.0 / (double)n_in;
-        const int n_inner = c->n_slab;
-        for (long xs = 0; xs < c->Vs; ++xs)
-            for (int mu = 1; mu <= 3; ++mu)
-                for (int r = 1; r <= R; ++r)
-                    for (int S = 0; S < n_outer; ++S) {
-                        cplx t4(1, 0);
-                        for (int i = 0; i < m; ++i) t4 *= c->A[A_idx(c, mu, r, S * m + i, xs)] * inv;          // Eq. 32
-                        A4[((((size_t)(mu - 1) * R + (r - 1)) * n_outer + S) * c->Vs) + xs] += t4;
-                        for (int fp = 0; fp < F; ++fp)
-                            for (int ch = 0; ch < 12; ++ch) {
-                                cplx to4(0, 0);
-                                for (int i = 0; i < m; ++i) {                                                   // Eq. 33
-                                    cplx term = c->B[B_idx(c, mu, r, S * m + i, fp, ch, xs)] * inv;
-                                    for (int i2 = 0; i2 < m; ++i2)
-                                        if (i2 != i) term *= c->A[A_idx(c, mu, r, S * m + i2, xs)] * inv;
-                                    to4 += term;
-                                }
-                                B4[((((((size_t)(mu - 1) * R + (r - 1)) * n_outer + S) * F + fp) * 12 + ch) * c->Vs) + xs] += to4;
-                            }
-                    }
-        (void)n_inner;
-        for (int ch = 0; ch < 12; ++ch) vac4[ch] += c->vac_sum[ch] * inv;
-        c->open = false;
+        combine2(c);
     }
-    const double invo = 1.0 / (double)n_out;
-    for (auto& z : A4) z *= invo;
-    for (auto& z : B4) z *= invo;
-    for (auto& v : vac4) v *= invo;
-    c->A.clear(); c->B.clear();
-    reduce_result(c, A4, B4, n_outer, vac4);
+    end2(c);
+    return ULO_OK;
+}
+int ulo_measure2_begin(ulo_ctx* c, int d_in, int d_out, int r_max, const int* fps, int n_fp) {
+    if (!c) return ULO_EINVAL;
+    return begin2(c, d_in, d_out, r_max, fps, n_fp);
+}
+int ulo_combine(ulo_ctx* c) {
+    if (!c) return ULO_EINVAL;
+    if (!c->open2 || c->n_acc == 0) { c->err = "no open two-level measurement with accumulated configurations"; return ULO_ESTATE; }
+    combine2(c);
+    return ULO_OK;
+}
+int ulo_measure2_end(ulo_ctx* c) {
+    if (!c) return ULO_EINVAL;
+    if (!c->open2 || c->n_comb == 0 || c->n_acc != 0) { c->err = "nothing combined, or configurations accumulated since the last combine"; return ULO_ESTATE; }
+    end2(c);
     return ULO_OK;
 }
 
@@ -564,6 +610,12 @@ int ulo_read_slab_averages(ulo_ctx* c, double* out) {
     if (!c || !out) return ULO_EINVAL;
     if (!c->have) { c->err = "no measurement yet"; return ULO_ESTATE; }
     for (size_t i = 0; i < c->slab_avg.size(); ++i) { out[2 * i] = c->slab_avg[i].real(); out[2 * i + 1] = c->slab_avg[i].imag(); }
+    return ULO_OK;
+}
+int ulo_read_slab_field_averages(ulo_ctx* c, double* out) {
+    if (!c || !out) return ULO_EINVAL;
+    if (!c->have) { c->err = "no measurement yet"; return ULO_ESTATE; }
+    for (size_t i = 0; i < c->slab_field_avg.size(); ++i) { out[2 * i] = c->slab_field_avg[i].real(); out[2 * i + 1] = c->slab_field_avg[i].imag(); }
     return ULO_OK;
 }
 const char* ulo_last_error(ulo_ctx* c) { return c ? c->err.c_str() : "null handle"; }

@@ -59,6 +59,12 @@ int ulo_multilevel2(ulo_ctx* h, int d_in, int n_in, int d_out, int n_out, int r_
 int ulo_measure_begin(ulo_ctx* h, int slab_thickness, int r_max, const int* field_points, int n_fp);
 int ulo_accumulate(ulo_ctx* h);
 int ulo_measure_end(ulo_ctx* h);
+/* the same for two levels (S8(c)-O7; Alg. 1 lines 5, 16, 18): begin, then per outer iteration {ulo_accumulate of every
+ * inner configuration, ulo_combine (Eqs. 32-33 on the inner averages, added to the outer sums)}, then end (outer
+ * averages, slab product).  ulo_multilevel2 is exactly this sequence with its own sweeps in between. */
+int ulo_measure2_begin(ulo_ctx* h, int d_in, int d_out, int r_max, const int* field_points, int n_fp);
+int ulo_combine(ulo_ctx* h);
+int ulo_measure2_end(ulo_ctx* h);
 
 int ulo_plaquette(ulo_ctx* h, double* mean_cos /*[3]: all, time-like, space-like*/);
 /* Polyakov-loop average <P> (Eqs. 15-16), out[2] = (Re, Im); multihit = 1: analytic multihit on every
@@ -69,6 +75,9 @@ int ulo_read_correlators(ulo_ctx* h, double* corr /*[r_max][2]*/,
 /* slab averages [T] of the last measurement (outer level for two-level):
  * out[((mu-1)*r_max + (r-1))*n_slab + s][xs][2], xs = x1 + Ns*(x2 + Ns*x3) */
 int ulo_read_slab_averages(ulo_ctx* h, double* out);
+/* slab averages [TO] of the last measurement (outer level for two-level):
+ * out[(((mu-1)*r_max + (r-1))*n_slab + s)*n_fp + fp][ch][xs][2] */
+int ulo_read_slab_field_averages(ulo_ctx* h, double* out);
 const char* ulo_last_error(ulo_ctx* h);
 
 /* ---- extra oracle-only entry points used by the pins in tests/ ---- */

@@ -52,6 +52,10 @@ def lib():
         L.ulo_measure_begin.argtypes = [P, C.c_int, C.c_int, P, C.c_int]
         L.ulo_accumulate.argtypes = [P]
         L.ulo_measure_end.argtypes = [P]
+        L.ulo_measure2_begin.argtypes = [P, C.c_int, C.c_int, C.c_int, P, C.c_int]
+        L.ulo_combine.argtypes = [P]
+        L.ulo_measure2_end.argtypes = [P]
+        L.ulo_read_slab_field_averages.argtypes = [P, P]
         L.ulo_plaquette.argtypes = [P, P]
         L.ulo_read_correlators.argtypes = [P, P, P, P]
         L.ulo_read_slab_averages.argtypes = [P, P]
@@ -169,6 +173,23 @@ class Oracle:
 
     def measure_end(self):
         self._ck(lib().ulo_measure_end(self._h))
+
+    def measure2_begin(self, d_in, d_out, r_max, field_points=None):
+        fp, n = _fps(field_points)
+        self._ck(lib().ulo_measure2_begin(self._h, int(d_in), int(d_out), int(r_max), _ptr(fp), n))
+        self._meas = (int(r_max), n, self.Nt // int(d_out))
+
+    def combine(self):
+        self._ck(lib().ulo_combine(self._h))
+
+    def measure2_end(self):
+        self._ck(lib().ulo_measure2_end(self._h))
+
+    def read_slab_field_averages(self):
+        R, F, S = self._meas
+        out = np.zeros((3, R, S, F, 12, self.Ns ** 3, 2))
+        self._ck(lib().ulo_read_slab_field_averages(self._h, _ptr(out)))
+        return out[..., 0] + 1j * out[..., 1]
 
     def plaquette(self):
         out = np.zeros(3)

@@ -266,6 +266,135 @@ def test_two_level_combine_against_numpy(ulo):
     assert np.allclose(corr2, C, atol=1e-14)
 
 
+def eq34_from_slab_averages(avT, avTO, Nt):
+    """C(r), G(r,fp,ch) from slab averages, straight from Eqs. 26 and 34:
+    avT [3][R][S][Vs], avTO [3][R][S][F][12][Vs]."""
+    Vs = avT.shape[-1]
+    S = avT.shape[2]
+    C = avT.prod(axis=2).sum(axis=(0, 2)) / (3 * Vs)
+    G = 0
+    for s in range(S):
+        others = np.delete(avT, s, axis=2).prod(axis=2)                    # prod_{s' != s} [T](s'), [3][R][Vs]
+        G = G + (avTO[:, :, s] * others[:, :, None, None, :]).sum(axis=(0, 4))
+    return C, G / (3 * Vs * Nt)
+
+
+def outer_masked_compound_sweep(o, d_out, n_or=3):
+    """The d_out-masked compound sweep (1 heatbath + 3 overrelaxation, the default sub-update) by sub-steps."""
+    for parity in (0, 1):
+        for mu in range(4):
+            o.substep(0, parity, mu, d_out)
+    o.set_counter(o.get_counter() + 1)
+    for _ in range(n_or):
+        for parity in (0, 1):
+            for mu in range(4):
+                o.substep(1, parity, mu, d_out)
+
+
+@pytest.mark.parametrize("Nt,d_in,d_out,n_in", [(8, 2, 4, 2), (12, 2, 6, 2), (8, 1, 4, 3)])
+def test_two_level_field_combine_against_numpy(ulo, Nt, d_in, d_out, n_in):
+    # Eq. 33 (P:345-347) with the t+2 reading R7, for m = d_out/d_in = 2 (the paper's case), 3 and 4 inner slabs per
+    # outer slab: TO^(d_out)(S) = sum_i [TO](s_i) prod_{i' != i} [T](s_i'), rebuilt in numpy from the single-level
+    # slab averages of the same trajectory; then Eq. 34 on the outer averages; then the vacuum.
+    Ns, R = 4, 2
+    fps = FPS[:3]
+    m = d_out // d_in
+    a = ulo.Oracle(Ns, Nt, 0.9, 7)
+    a.multilevel2(d_in, n_in, d_out, 1, R, fps)
+    corr2, field2, vac2 = a.read_correlators()
+    T4, TO4 = a.read_slab_averages(), a.read_slab_field_averages()
+    b = ulo.Oracle(Ns, Nt, 0.9, 7)
+    outer_masked_compound_sweep(b, d_out)
+    b.multilevel(d_in, n_in, R, fps)
+    T2, TO2 = b.read_slab_averages(), b.read_slab_field_averages()       # [3][R][Nt/d_in][Vs], [3][R][Nt/d_in][F][12][Vs]
+    _, _, vac1 = b.read_correlators()
+    assert np.array_equal(a.get_links(), b.get_links())
+    n_outer = Nt // d_out
+    T2g = T2.reshape(3, R, n_outer, m, -1)
+    TO2g = TO2.reshape(3, R, n_outer, m, len(fps), 12, -1)
+    wantT = T2g.prod(axis=3)                                               # Eq. 32
+    wantTO = 0
+    for i in range(m):                                                     # Eq. 33
+        others = np.delete(T2g, i, axis=3).prod(axis=3)
+        wantTO = wantTO + TO2g[:, :, :, i] * others[:, :, :, None, None, :]
+    assert np.abs(TO2).max() > 0.1                                         # the comparison is not vacuous
+    assert np.allclose(T4, wantT, atol=1e-14)
+    assert np.allclose(TO4, wantTO, atol=1e-14)
+    C, G = eq34_from_slab_averages(wantT, wantTO, Nt)
+    assert np.allclose(corr2, C, atol=1e-15) and np.allclose(field2, G, atol=1e-15)
+    assert np.allclose(vac2, vac1, atol=1e-15)
+
+
+@pytest.mark.parametrize("Nt,d_in,d_out", [(8, 2, 4), (12, 2, 6)])
+def test_two_level_on_one_configuration_equals_brute_force(ulo, Nt, d_in, d_out):
+    # n_in = n_out = 1: every average is over ONE configuration, so Eqs. 32-34 must give the plain single-configuration
+    # C and G of the final links (np.roll restatement of Eqs. 22-34, no slab structure at all): pins the cross terms
+    # of Eq. 33 and every 1/n factor without reading any intermediate of the oracle
+    Ns, R = 4, 2
+    a = ulo.Oracle(Ns, Nt, 0.9, 21)
+    a.multilevel2(d_in, 1, d_out, 1, R, FPS)
+    corr, field, vac = a.read_correlators()
+    C, G = brute_force_single_config(a.get_links(), d_out, R, FPS)
+    assert np.allclose(corr, C, atol=1e-13)
+    assert np.allclose(field, G, atol=1e-13)
+    assert np.abs(G).max() > 1e-3
+
+
+def test_two_level_outer_average_is_mean_of_chained_runs(ulo):
+    # Alg. 1 lines 5-17 (P:228-266), Eq. 27 (P:308-311): [T4], [TO4] and the vacuum over n_out outer iterations are
+    # the means of the single-iteration values along the same trajectory; C and G follow from the means by Eq. 34
+    Ns, Nt, R, n_in, n_out = 4, 8, 2, 2, 3
+    fps = FPS[:2]
+    a = ulo.Oracle(Ns, Nt, 0.95, 9)
+    a.multilevel2(2, n_in, 4, n_out, R, fps)
+    b = ulo.Oracle(Ns, Nt, 0.95, 9)
+    T4, TO4, vac = 0, 0, 0
+    for _ in range(n_out):
+        b.multilevel2(2, n_in, 4, 1, R, fps)                               # chained from b's own state
+        T4 = T4 + b.read_slab_averages()
+        TO4 = TO4 + b.read_slab_field_averages()
+        vac = vac + b.read_correlators()[2]
+    assert np.array_equal(a.get_links(), b.get_links()) and a.get_counter() == b.get_counter()
+    assert np.allclose(a.read_slab_averages(), T4 / n_out, atol=1e-15)
+    assert np.allclose(a.read_slab_field_averages(), TO4 / n_out, atol=1e-15)
+    corr, field, vac_a = a.read_correlators()
+    C, G = eq34_from_slab_averages(T4 / n_out, TO4 / n_out, Nt)
+    assert np.allclose(corr, C, atol=1e-15) and np.allclose(field, G, atol=1e-15)
+    assert np.allclose(vac_a, vac / n_out, atol=1e-15)
+    # and the mean is not the single-iteration value
+    assert not np.allclose(a.read_slab_averages(), b.read_slab_averages(), atol=1e-3)
+
+
+def test_two_level_hooks_equal_multilevel2(ulo):
+    # measure2_begin / accumulate / combine / measure2_end with the sweeps done by hand reproduce ulo_multilevel2
+    Ns, Nt, R, n_in, n_out = 4, 8, 2, 3, 2
+    fps = FPS[:2]
+    a = ulo.Oracle(Ns, Nt, 0.95, 3)
+    b = ulo.Oracle(Ns, Nt, 0.95, 3)
+    a.multilevel2(2, n_in, 4, n_out, R, fps)
+    b.measure2_begin(2, 4, R, fps)
+    for _ in range(n_out):
+        outer_masked_compound_sweep(b, 4)
+        for _ in range(n_in):
+            outer_masked_compound_sweep(b, 2)
+            b.accumulate()
+        b.combine()
+    b.measure2_end()
+    for x, y in zip(a.read_correlators(), b.read_correlators()):
+        assert np.array_equal(x, y)
+    assert np.array_equal(a.read_slab_field_averages(), b.read_slab_field_averages())
+    assert np.array_equal(a.get_links(), b.get_links())
+    # state errors: end with configurations pending, combine with nothing accumulated
+    b.measure2_begin(2, 4, R, fps)
+    with pytest.raises(ulo.OracleError):
+        b.combine()
+    b.accumulate()
+    with pytest.raises(ulo.OracleError):
+        b.measure2_end()
+    with pytest.raises(ulo.OracleError):
+        b.measure_end()
+
+
 # ----------------------------------------------------------------------------- theory (statistical)
 def _series_mean_err(x, nbins=10):
     x = np.asarray(x, dtype=float)
