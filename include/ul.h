@@ -159,6 +159,29 @@ int ul_multilevel2(ul_ctx* h, int d_in, int n_in, int d_out, int n_out, int r_ma
 int ul_measure_begin(ul_ctx* h, int slab_thickness, int r_max, const int* field_points, int n_fp);
 int ul_accumulate(ul_ctx* h);
 int ul_measure_end(ul_ctx* h);
+/* The same for two levels (Alg. 1 lines 5, 16, 18; Eqs. 32-33 P:343-347 with DESIGN R7): begin; per outer
+ * iteration { ul_accumulate for every inner configuration; ul_combine: inner averages = inner sums / number of
+ * configurations accumulated since the last combine, T^(d_out) and TO^(d_out) of every outer slab added to the outer
+ * sums, inner sums restarted }; end: outer averages = outer sums / number of combines, slab product, reduction
+ * (row a10).  ul_multilevel2 is this sequence with its own sub-updates in between.  UL_ESTATE: no two-level
+ * measurement open, nothing accumulated since the last combine, a different number of configurations than in
+ * the previous outer iteration, configurations pending at end; ul_measure_end refuses a two-level measurement. */
+int ul_measure2_begin(ul_ctx* h, int d_in, int d_out, int r_max, const int* field_points, int n_fp);
+int ul_combine(ul_ctx* h);
+int ul_measure2_end(ul_ctx* h);
+
+/* Slab-group-major order of the sub-update loop ("hold their spatial links constant [and] isolate the dynamics
+ * of the sublattice from the rest of the lattice").  The slabs are dynamically independent during the n_sub loop of
+ * ul_multilevel, so the loop may run slab group by slab group: all n_sub masked sub-updates, tables and accumulation
+ * passes of `n_slabs` consecutive slabs, then the next group -- the group's links and tables stay in L2 instead of
+ * streaming the whole lattice from HBM for every sub-step.  Counter-based RNG and per-entry accumulation make the
+ * links, the sweep counter, the slab sums, C(r) and G bit-identical to the sub-update-major order (tested); only the
+ * vacuum sums are added in a different order (1e-16 relative).  n_slabs = 0: off; -1: automatic (groups of ~32 MB of
+ * links on lattices whose links exceed 96 MB); > 0: that many slabs per group.  UL_ESTATE: a measurement is open.
+ * ul_substep_slabs is the test hook underneath: ul_substep restricted to the slabs s_begin <= s < s_end of
+ * thickness slab_d >= 1 (UL_EINVAL on a bad range). */
+int ul_set_slab_group(ul_ctx* h, int n_slabs);
+int ul_substep_slabs(ul_ctx* h, int kind, int parity, int mu, int slab_d, int s_begin, int s_end);
 
 /* Analytic multihit inside the two-link operators: with on = 1 the sums of
  * T^(d)(x,s,r mu) for r >= 2 are built from multihit temporal links Ubar_0 = (I1(beta k)/I0(beta k)) e^{i alpha}
@@ -209,7 +232,10 @@ int ul_slab_partial_product(ul_ctx* h, int s_begin, int s_end, void* dev_out);
  *                          orientations (0,mu) (0,nu) (0,rho) (nu,rho) (rho,mu) (mu,nu),
  *                          kind 0 = 1 - cos theta_P, 1 = sin theta_P (Eqs. 28-29
  *                          without the beta factors)
- * vacuum[12]               <O_ch> over all sites, times and the three frames.
+ * vacuum[12]               <O_ch> over all sites, times and the three frames: the mean over the measured
+ *                          configurations when field points were requested; with n_fp = 0 (nothing to
+ *                          subtract from, Eq. 30) the plaquettes are not evaluated per sub-update and
+ *                          the values are those of the final configuration of the measurement.
  * UL_ESTATE before any measurement.  Synchronises. */
 int ul_read_correlators(ul_ctx* h, double* corr, double* field, double* vacuum);
 

@@ -126,8 +126,11 @@ struct ul_ctx {
     bool open = false;
     int d = 0, r_max = 0, n_fp = 0, n_slab = 0, d_out = 0, n_outer = 0;
     long long n_acc = 0;
+    int n_comb = 0, n_in_seen = 0, n_inner_acc = 0;   // two-level hooks: outer iterations combined, inner configurations per iteration / since the last combine
     int n_pending = 0;       // configurations tabulated but not yet added to the accumulators
     bool multihit = false;   // ul_set_multihit: sums of T at r >= 2 from multihit temporal links
+    bool vac_deferred = false; // no field points: the plaquette column sums are taken once, on the final configuration
+    int slab_group = 0;      // ul_set_slab_group: slabs per group of the slab-group-major sub-update loop (0 = off)
     bool skip_colsum = false; // replayed configurations: their plaquette column sums are already in the vacuum sums
     float* staging2 = nullptr; // second configuration copy (two-level replay)
     char* plane_buf = nullptr; // full-plane maps through the transverse DFT: Ohat, group partials, Ghat (library-owned)
@@ -196,11 +199,18 @@ cudaError_t launch_update_mu(const ul_ctx* c, int mu, const ulk::UpdateArgs& a, 
 }
 
 // one sub-step (kind, parity, mu), optionally slab-masked: rows a3-a6
-int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
-    int n_t = c->Nt;
-    if (slab_d > 0 && mu != 0) n_t = c->Nt / slab_d * (slab_d - 1);
+// s_begin <= s < s_end: the slabs (of thickness slab_d) this launch covers; the whole lattice when slab_d = 0
+int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin = 0, int s_end = -1) {
+    int n_t = c->Nt, z0 = 0;
+    if (slab_d > 0) {
+        if (s_end < 0) s_end = c->Nt / slab_d;
+        const int per = mu != 0 ? slab_d - 1 : slab_d;    // layers of a slab this direction updates
+        n_t = (s_end - s_begin) * per;
+        z0 = s_begin * per;
+    }
     if (n_t == 0) return UL_OK;                       // thickness 1: every spatial link is frozen
     ulk::UpdateArgs a;
+    a.z0 = z0;
     a.th = c->th; a.Vh = (int)c->Vh; a.Ns = c->Ns; a.Nh = c->Nh; a.Nt = c->Nt;
     a.parity = parity; a.slab_d = slab_d; a.beta = (float)c->beta;
     a.key0 = (uint32_t)(c->seed & 0xffffffffu); a.key1 = (uint32_t)(c->seed >> 32);
@@ -225,10 +235,10 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
     }
     return UL_OK;
 }
-int one_sweep(ul_ctx* c, int kind, int slab_d) {      // O5: parity outer, direction inner
+int one_sweep(ul_ctx* c, int kind, int slab_d, int s_begin = 0, int s_end = -1) {      // O5: parity outer, direction inner
     for (int parity = 0; parity < 2; ++parity)
         for (int mu = 0; mu < 4; ++mu) {
-            const int rc = substep(c, kind, parity, mu, slab_d);
+            const int rc = substep(c, kind, parity, mu, slab_d, s_begin, s_end);
             if (rc) return rc;
         }
     if (kind != 1) {                                  // heatbath and Metropolis sweeps consume the counter
@@ -237,9 +247,9 @@ int one_sweep(ul_ctx* c, int kind, int slab_d) {      // O5: parity outer, direc
     }
     return UL_OK;
 }
-int compound_direct(ul_ctx* c, int n_hb, int n_or, int slab_d) {
-    for (int i = 0; i < n_hb; ++i) { const int rc = one_sweep(c, c->alg == 1 ? 2 : 0, slab_d); if (rc) return rc; }
-    for (int i = 0; i < n_or; ++i) { const int rc = one_sweep(c, 1, slab_d); if (rc) return rc; }
+int compound_direct(ul_ctx* c, int n_hb, int n_or, int slab_d, int s_begin = 0, int s_end = -1) {
+    for (int i = 0; i < n_hb; ++i) { const int rc = one_sweep(c, c->alg == 1 ? 2 : 0, slab_d, s_begin, s_end); if (rc) return rc; }
+    for (int i = 0; i < n_or; ++i) { const int rc = one_sweep(c, 1, slab_d, s_begin, s_end); if (rc) return rc; }
     return UL_OK;
 }
 
@@ -290,6 +300,17 @@ int compound(ul_ctx* c, int n_hb, int n_or, int slab_d) {
     return UL_OK;
 }
 
+// slabs per group of the slab-group-major sub-update loop; 0 = sub-update-major (one launch over all slabs)
+int slab_group_size(const ul_ctx* c, int d) {
+    if (c->slab_group >= 0) return c->slab_group;
+    // auto: lattices whose links do not fit L2 -- groups of ~32 MB of links (4 links x 4 B per site)
+    const double link_bytes = 16.0 * (double)c->V;
+    if (link_bytes <= 96e6) return 0;
+    const double per_slab = 16.0 * (double)c->Vs * d;
+    int g = (int)(32e6 / per_slab);
+    return g < 1 ? 1 : g;
+}
+
 int check_meas_args(ul_ctx* c, int d, int r_max, const int* fps, int n_fp) {
     if (d < 1 || c->Nt % d != 0) return fail(c, UL_EINVAL, "Nt % slab_thickness != 0");
     if (r_max < 1 || r_max > c->Ns / 2) return fail(c, UL_EINVAL, "r_max out of range [1, Ns/2]");
@@ -317,6 +338,7 @@ int open_measurement(ul_ctx* c, int d_in, int d_out, int r_max, const int* fps, 
     c->n_pending = 0;
     c->acc_fresh = true;
     c->plane_fresh = true;
+    c->vac_deferred = false;
     c->have = false;
     if (n_fp > 0) UL_CUDA(c, cudaMemcpyAsync(c->work + w.fps, fps, sizeof(int) * 3 * (size_t)n_fp, cudaMemcpyHostToDevice, c->stream));
     if (w.partial > w.A4) UL_CUDA(c, cudaMemsetAsync(c->work + w.A4, 0, w.partial - w.A4, c->stream));   // A4, B4 (A2, B2: first pass writes)
@@ -330,11 +352,14 @@ double* res_colsum(ul_ctx* c) { return wsp<double>(c, c->ws.result) + 2 * (size_
 double* res_vacuum(ul_ctx* c) { return wsp<double>(c, c->ws.result) + 2 * (size_t)c->r_max * (1 + 12 * (size_t)c->n_fp); }
 
 // adds the tabulated configurations (slots 0..n_pending-1) to the accumulators: rows a7, a8
-int flush(ul_ctx* c) {
+// (restricted to the slabs s_begin <= s < s_end when s_end >= 0: slab-group-major order)
+int flush(ul_ctx* c, int s_begin = 0, int s_end = -1) {
     if (c->n_pending == 0) return UL_OK;
-    const long long n = (long long)c->n_slab * c->Vs;
+    if (s_end < 0) s_end = c->n_slab;
+    const long long n = (long long)(s_end - s_begin) * c->Vs;
     const int nb = (int)((n + 255) / 256);
     ulk::AccumArgs a;
+    a.idx0 = (long long)s_begin * c->Vs; a.n_idx = n;
     a.g = geom(c); a.d = c->d; a.n_slab = c->n_slab; a.r_max = c->r_max; a.n_fp = c->n_fp; a.nk = c->n_pending; a.first = c->acc_fresh ? 1 : 0;
     a.U = wsp<double2>(c, c->ws.U); a.Ot = wsp<float>(c, c->ws.Ot); a.fps = wsp<int>(c, c->ws.fps);
     a.A = wsp<double2>(c, c->ws.A2); a.B = wsp<double2>(c, c->ws.B2);
@@ -377,9 +402,28 @@ int flush(ul_ctx* c) {
     return UL_OK;
 }
 
+// the plaquette column sums of the current configuration, added to the vacuum sums (no table is written)
+int vacuum_pass(ul_ctx* c) {
+    ulk::TableArgs t;
+    t.g = geom(c); t.th = c->th; t.d = c->d; t.n_slab = c->n_slab;
+    t.U = nullptr; t.Um = nullptr; t.beta = (float)c->beta; t.Ot = nullptr;
+    t.partial = wsp<double>(c, c->ws.partial);
+    t.row0 = 0; t.n_rows = c->n_slab * c->Ns;
+    const int gx = (c->Ns * c->Ns + 255) / 256, rows = t.n_rows;
+    const int gy = rows < TBLK / gx ? rows : (TBLK / gx > 0 ? TBLK / gx : 1);
+    ulk::k_slab_tables<<<dim3(gx, gy), 256, 0, c->stream>>>(t);
+    ulk::k_sum_partials<<<12, 256, 0, c->stream>>>(t.partial, gx * gy, res_colsum(c), 1.0, 1);
+    UL_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    return UL_OK;
+}
+
 // tabulates the current configuration (U, Ot, column sums of O) into the next batch slot; the batch is
-// added to the accumulators when it is full, and before anything reads them
-int accumulate(ul_ctx* c) {
+// added to the accumulators when it is full, and before anything reads them.  With a slab range (s_end >= 0) only
+// those slabs are tabulated, and the caller counts the configuration and flushes (slab-group-major order).
+int accumulate(ul_ctx* c, int s_begin = 0, int s_end = -1) {
+    const bool ranged = s_end >= 0;
+    if (!ranged) s_end = c->n_slab;
     const long long n = (long long)c->n_slab * c->Vs;
     ulk::TableArgs t;
     t.g = geom(c); t.th = c->th; t.d = c->d; t.n_slab = c->n_slab;
@@ -388,12 +432,22 @@ int accumulate(ul_ctx* c) {
     t.beta = (float)c->beta;
     t.Ot = (c->n_fp > 0 && !c->replay) ? wsp<float>(c, c->ws.Ot) + (size_t)c->n_pending * 12 * n : nullptr;
     t.partial = wsp<double>(c, c->ws.partial);
-    const int gx = (c->Ns * c->Ns + 255) / 256, rows = c->n_slab * c->Ns;
-    const int gy = rows < TBLK / gx ? rows : (TBLK / gx > 0 ? TBLK / gx : 1);
-    ulk::k_slab_tables<<<dim3(gx, gy), 256, 0, c->stream>>>(t);
-    if (!c->skip_colsum) { ulk::k_sum_partials<<<12, 256, 0, c->stream>>>(t.partial, gx * gy, res_colsum(c), 1.0, 1); c->launches += 1; }
+    t.row0 = s_begin * c->Ns; t.n_rows = (s_end - s_begin) * c->Ns;
+    if (c->n_fp == 0 && !c->multihit) {
+        // nothing needs the plaquettes: U table only (row a7); the vacuum values are then taken on the final
+        // configuration of the measurement (finish())
+        const long long threads = (long long)t.n_rows * c->Ns * c->Nh;
+        ulk::k_slab_tables_u<<<(unsigned)((threads + 255) / 256), 256, 0, c->stream>>>(t);
+        c->vac_deferred = true;
+    } else {
+        const int gx = (c->Ns * c->Ns + 255) / 256, rows = t.n_rows;
+        const int gy = rows < TBLK / gx ? rows : (TBLK / gx > 0 ? TBLK / gx : 1);
+        ulk::k_slab_tables<<<dim3(gx, gy), 256, 0, c->stream>>>(t);
+        if (!c->skip_colsum) { ulk::k_sum_partials<<<12, 256, 0, c->stream>>>(t.partial, gx * gy, res_colsum(c), 1.0, 1); c->launches += 1; }
+    }
     UL_CUDA(c, cudaGetLastError());
     c->launches += 1;
+    if (ranged) return UL_OK;
     c->n_acc += 1;
     c->n_pending += 1;
     if (c->n_pending == c->ws.kb) return flush(c);
@@ -418,6 +472,12 @@ int finish(ul_ctx* c, const double2* A, const double2* B, int n_slab, double inv
         ulk::k_sum_partials<<<2 * (n_entries - R), 256, 0, c->stream>>>(a.partial + (size_t)2 * R * NBLK, NBLK, res + 2 * R,
                                                                         1.0 / (3.0 * (double)c->Vs * (double)c->Nt), 0);
         c->launches += 1;
+    }
+    if (c->vac_deferred) {                          // no field points: vacuum values of the final configuration (include/ul.h)
+        const int rc = vacuum_pass(c);
+        if (rc) return rc;
+        vac_inv = 1.0;
+        c->vac_deferred = false;
     }
     ulk::k_vacuum<<<1, 32, 0, c->stream>>>(res_colsum(c), vac_inv / (3.0 * (double)c->V), res_vacuum(c));
     c->launches += 1;
@@ -599,6 +659,18 @@ int ul_substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
     if (slab_d > 0 && c->Nt % slab_d != 0) return fail(c, UL_EINVAL, "Nt % slab_d != 0");
     return substep(c, kind, parity, mu, slab_d);
 }
+int ul_substep_slabs(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin, int s_end) {
+    if (!c || kind < 0 || kind > 2 || (parity != 0 && parity != 1) || mu < 0 || mu > 3 || slab_d < 1 || c->Nt % slab_d != 0)
+        return fail(c, UL_EINVAL, "bad sub-step arguments");
+    if (s_begin < 0 || s_begin > s_end || s_end > c->Nt / slab_d) return fail(c, UL_EINVAL, "bad slab range");
+    return substep(c, kind, parity, mu, slab_d, s_begin, s_end);
+}
+int ul_set_slab_group(ul_ctx* c, int n_slabs) {
+    if (!c || n_slabs < -1) return fail(c, UL_EINVAL, "n_slabs must be >= -1");
+    if (c->open) return fail(c, UL_ESTATE, "a measurement is open");
+    c->slab_group = n_slabs;
+    return UL_OK;
+}
 int ul_set_update_algorithm(ul_ctx* c, int alg, double delta) {
     if (!c || (alg != 0 && alg != 1) || (alg == 1 && !(delta > 0.0 && delta <= 3.14159265358979323846)))
         return fail(c, UL_EINVAL, "alg must be 0 (heatbath) or 1 (Metropolis with 0 < delta <= pi)");
@@ -632,11 +704,13 @@ int ul_set_accum_batch(ul_ctx* c, int depth) {
 int ul_accumulate(ul_ctx* c) {
     if (!c) return fail(c, UL_EINVAL, "null handle");
     if (!c->open) return fail(c, UL_ESTATE, "no open measurement");
-    return accumulate(c);
+    const int rc = accumulate(c);
+    if (!rc && c->d_out > 0) c->n_inner_acc += 1;
+    return rc;
 }
 int ul_measure_end(ul_ctx* c) {
     if (!c) return fail(c, UL_EINVAL, "null handle");
-    if (!c->open || c->n_acc == 0) return fail(c, UL_ESTATE, "nothing accumulated");
+    if (!c->open || c->n_acc == 0 || c->d_out > 0) return fail(c, UL_ESTATE, "nothing accumulated (or a two-level measurement is open)");
     const int rc = flush(c);
     if (rc) return rc;
     const double inv = 1.0 / (double)c->n_acc;
@@ -647,13 +721,39 @@ int ul_multilevel(ul_ctx* c, int d, int n_sub, int r_max, const int* fps, int n_
     if (!c || n_sub < 0) return fail(c, UL_EINVAL, "n_sub must be >= 0");
     int rc = ul_measure_begin(c, d, r_max, fps, n_fp);
     if (rc) return rc;
-    if (n_sub == 0) { rc = accumulate(c); if (rc) return rc; }
-    for (int j = 0; j < n_sub; ++j) {
-        for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d); if (rc) return rc; }
-        rc = accumulate(c);
-        if (rc) return rc;
+    auto bail = [&](int code) { c->open = false; return code; };
+    if (n_sub == 0) { rc = accumulate(c); if (rc) return bail(rc); }
+    const int grp = slab_group_size(c, d);
+    if (n_sub > 0 && grp > 0 && grp < c->n_slab) {
+        // Slab-group-major order (while the boundary layers are frozen the slabs are dynamically independent): the
+        // whole n_sub loop -- masked sub-updates, tables, accumulation -- runs for one group of slabs, whose links and
+        // tables stay in L2, before the next group is touched.  Same Philox counters (the sweep counter restarts for
+        // every group), same per-entry order of additions: links, counter, slab sums and correlators are bit-identical
+        // to the sub-update-major order.
+        const uint64_t sweep0 = c->sweep;
+        for (int s0 = 0; s0 < c->n_slab; s0 += grp) {
+            const int s1 = s0 + grp < c->n_slab ? s0 + grp : c->n_slab;
+            c->sweep = sweep0; c->d_sweep_stale = true;
+            c->acc_fresh = true;
+            c->n_pending = 0;
+            for (int j = 0; j < n_sub; ++j) {
+                for (int k = 0; k < c->sub_k; ++k) { rc = compound_direct(c, c->sub_hb, c->sub_or, d, s0, s1); if (rc) return bail(rc); }
+                rc = accumulate(c, s0, s1);
+                if (rc) return bail(rc);
+                c->n_pending += 1;
+                if (c->n_pending == c->ws.kb || j == n_sub - 1) { rc = flush(c, s0, s1); if (rc) return bail(rc); }
+            }
+        }
+        c->n_acc = n_sub;
+    } else {
+        for (int j = 0; j < n_sub; ++j) {
+            for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d); if (rc) return bail(rc); }
+            rc = accumulate(c);
+            if (rc) return bail(rc);
+        }
     }
-    return ul_measure_end(c);
+    rc = ul_measure_end(c);
+    return rc ? bail(rc) : rc;
 }
 
 // the field points are a full transverse plane fp = b + Ns c <-> (a, b, c) with one a?  (host array)
@@ -778,6 +878,7 @@ int ul_multilevel_replay(ul_ctx* c, int d, int n_sub, int r_max, const int* fps,
     t.g = geom(c); t.th = c->th; t.d = c->d; t.n_slab = c->n_slab;
     t.U = wsp<double2>(c, c->ws.U); t.Um = nullptr; t.beta = (float)c->beta;       // the TO sums use the plain T
     t.Ot = wsp<float>(c, c->ws.Ot); t.partial = wsp<double>(c, c->ws.partial);
+    t.row0 = 0; t.n_rows = c->n_slab * c->Ns;
     ulk::ReplayArgs ra;
     ra.g = geom(c); ra.n_slab = c->n_slab; ra.r_max = r_max; ra.n_fp = n_fp;
     ra.U = t.U; ra.Ot = t.Ot; ra.fps = wsp<int>(c, c->ws.fps); ra.W = wa.W; ra.partial = wsp<double>(c, c->ws.partial);
@@ -799,34 +900,77 @@ int ul_multilevel_replay(ul_ctx* c, int d, int n_sub, int r_max, const int* fps,
     return rc;
 }
 
-int ul_multilevel2(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, int r_max, const int* fps, int n_fp) {
-    if (!c || n_in < 1 || n_out < 1) return fail(c, UL_EINVAL, "n_in, n_out must be >= 1");
+// Two levels (S8(c)-O7), Alg. 1 lines 5 / 16 / 18 as three steps shared by ul_multilevel2 and the test hooks
+// ul_measure2_begin / ul_combine / ul_measure2_end.
+static int begin2(ul_ctx* c, int d_in, int d_out, int r_max, const int* fps, int n_fp) {
     int rc = check_meas_args(c, d_in, r_max, fps, n_fp);
     if (rc) return rc;
     if (d_out < d_in || d_out % d_in != 0 || c->Nt % d_out != 0) return fail(c, UL_EINVAL, "need d_in | d_out | Nt");
     rc = open_measurement(c, d_in, d_out, r_max, fps, n_fp);
     if (rc) return rc;
+    c->n_comb = 0; c->n_in_seen = 0; c->n_inner_acc = 0;
+    return UL_OK;
+}
+// Eqs. 32-33 on the inner averages (inner sums / number of configurations accumulated since the last combine),
+// added to the outer sums; the next inner sums start from zero
+static int combine2(ul_ctx* c) {
+    if (c->n_inner_acc < 1) return fail(c, UL_ESTATE, "nothing accumulated since the last combine");
+    if (c->n_comb > 0 && c->n_inner_acc != c->n_in_seen) return fail(c, UL_ESTATE, "every outer iteration must accumulate the same number of configurations");
+    const int rc = flush(c);
+    if (rc) return rc;
     const Workspace& w = c->ws;
     ulk::CombineArgs a;
-    a.Vs = c->Vs; a.r_max = r_max; a.n_fp = n_fp; a.n_inner = c->n_slab; a.n_outer = c->n_outer; a.m = d_out / d_in;
-    a.inv = 1.0 / (double)n_in;
+    a.Vs = c->Vs; a.r_max = c->r_max; a.n_fp = c->n_fp; a.n_inner = c->n_slab; a.n_outer = c->n_outer; a.m = c->d_out / c->d;
+    a.inv = 1.0 / (double)c->n_inner_acc;
     a.A2 = wsp<double2>(c, w.A2); a.B2 = wsp<double2>(c, w.B2); a.A4 = wsp<double2>(c, w.A4); a.B4 = wsp<double2>(c, w.B4);
-    const long long total = 3LL * r_max * c->n_outer * c->Vs;
+    const long long total = 3LL * c->r_max * c->n_outer * c->Vs;
+    ulk::k_combine<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>(a);
+    UL_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    c->n_in_seen = c->n_inner_acc;
+    c->n_inner_acc = 0;
+    c->n_comb += 1;
+    c->acc_fresh = true;                                                                     // A2, B2 <- 0
+    return UL_OK;
+}
+static int end2(ul_ctx* c) {
+    if (c->n_comb < 1 || c->n_inner_acc != 0) return fail(c, UL_ESTATE, "nothing combined, or configurations accumulated since the last combine");
+    const Workspace& w = c->ws;
+    return finish(c, wsp<double2>(c, w.A4), wsp<double2>(c, w.B4), c->n_outer, 1.0 / (double)c->n_comb,
+                  1.0 / ((double)c->n_in_seen * (double)c->n_comb));
+}
+int ul_multilevel2(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, int r_max, const int* fps, int n_fp) {
+    if (!c || n_in < 1 || n_out < 1) return fail(c, UL_EINVAL, "n_in, n_out must be >= 1");
+    int rc = begin2(c, d_in, d_out, r_max, fps, n_fp);
+    if (rc) return rc;
+    auto bail = [&](int code) { c->open = false; return code; };
     for (int J = 0; J < n_out; ++J) {
-        for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d_out); if (rc) return rc; }
-        c->acc_fresh = true;                                                                 // A2, B2 <- 0
+        for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d_out); if (rc) return bail(rc); }
         for (int j = 0; j < n_in; ++j) {
-            for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d_in); if (rc) return rc; }
+            for (int k = 0; k < c->sub_k; ++k) { rc = compound(c, c->sub_hb, c->sub_or, d_in); if (rc) return bail(rc); }
             rc = accumulate(c);
-            if (rc) return rc;
+            if (rc) return bail(rc);
+            c->n_inner_acc += 1;
         }
-        rc = flush(c);
-        if (rc) return rc;
-        ulk::k_combine<<<(unsigned)((total + 255) / 256), 256, 0, c->stream>>>(a);          // Eqs. 32-33
-        UL_CUDA(c, cudaGetLastError());
-        c->launches += 1;
+        rc = combine2(c);
+        if (rc) return bail(rc);
     }
-    return finish(c, a.A4, a.B4, c->n_outer, 1.0 / (double)n_out, 1.0 / ((double)n_in * (double)n_out));
+    rc = end2(c);
+    return rc ? bail(rc) : rc;
+}
+int ul_measure2_begin(ul_ctx* c, int d_in, int d_out, int r_max, const int* fps, int n_fp) {
+    if (!c) return fail(c, UL_EINVAL, "null handle");
+    return begin2(c, d_in, d_out, r_max, fps, n_fp);
+}
+int ul_combine(ul_ctx* c) {
+    if (!c) return fail(c, UL_EINVAL, "null handle");
+    if (!c->open || c->d_out == 0) return fail(c, UL_ESTATE, "no open two-level measurement");
+    return combine2(c);
+}
+int ul_measure2_end(ul_ctx* c) {
+    if (!c) return fail(c, UL_EINVAL, "null handle");
+    if (!c->open || c->d_out == 0) return fail(c, UL_ESTATE, "no open two-level measurement");
+    return end2(c);
 }
 
 // Two levels by replay (S8(f) rank 2 for BJ config 4): G is linear in O, with weights that need the inner averages of
@@ -896,6 +1040,7 @@ int ul_multilevel2_replay(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, i
     t.g = geom(c); t.th = c->th; t.d = c->d; t.n_slab = c->n_slab;
     t.U = wsp<double2>(c, w.U); t.Um = nullptr; t.beta = (float)c->beta;
     t.Ot = wsp<float>(c, w.Ot); t.partial = wsp<double>(c, w.partial);
+    t.row0 = 0; t.n_rows = c->n_slab * c->Ns;
     ulk::ReplayArgs ra;
     ra.g = geom(c); ra.n_slab = c->n_slab; ra.r_max = r_max; ra.n_fp = n_fp;
     ra.U = t.U; ra.Ot = t.Ot; ra.fps = wsp<int>(c, w.fps); ra.W = ga.Wc; ra.partial = wsp<double>(c, w.partial);

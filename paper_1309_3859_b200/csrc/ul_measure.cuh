@@ -271,6 +271,7 @@ struct TableArgs {
     float beta;
     float* Ot;
     double* partial;
+    int row0, n_rows;     // rows (s, x3) = s * Ns + x3 handled by this launch: [row0, row0 + n_rows)  (a range of slabs)
 };
 
 // I1(a)/I0(a) in fp32 by the backward recurrence R_{n-1} = 1/(2n/a + R_n) from R_N = 0, N = a + 20 (the start value is
@@ -296,7 +297,7 @@ __global__ void __launch_bounds__(256) k_slab_tables(const TableArgs P) {
     float vf[12];                                   // per-thread column sums: a few terms of magnitude <= 2 each, then fp64
 #pragma unroll
     for (int o = 0; o < 12; ++o) vf[o] = 0.0f;
-    for (unsigned row = blockIdx.y; row < (unsigned)P.n_slab * Ns; row += gridDim.y) {   // rows (s, x3): 32-bit divisions only
+    for (unsigned row = (unsigned)P.row0 + blockIdx.y; row < (unsigned)(P.row0 + P.n_rows); row += gridDim.y) {   // rows (s, x3): 32-bit divisions only
         const int s = (int)(row / Ns);
         x[3] = (int)(row - (unsigned)s * Ns);
         if (!in) continue;
@@ -344,7 +345,7 @@ __global__ void __launch_bounds__(256) k_slab_tables(const TableArgs P) {
         }
         double us, uc;
         ulm::sincos_bt_f64((int)acc, uc, us);
-        P.U[idx] = make_double2(uc, us);
+        if (P.U) P.U[idx] = make_double2(uc, us);
         if (P.Um) P.Um[idx] = make_double2(uc * mhr - us * mhi, uc * mhi + us * mhr);
 #pragma unroll
         for (int o = 0; o < 6; ++o) {
@@ -365,6 +366,36 @@ __global__ void __launch_bounds__(256) k_slab_tables(const TableArgs P) {
 #pragma unroll
         for (int o = 0; o < 12; ++o) P.partial[(long long)o * nblk + blk] = v[o];
     }
+}
+
+// The U table alone (no field points, no multihit: nothing needs the plaquettes): one thread per (row, h) = the two
+// sites x1 = 2h, 2h + 1 of a row (t, x3, x2), whose temporal links sit at the same offset of the two parity arrays;
+// reads V * 4 B, writes n_slab * Vs * 16 B, both coalesced (S8(d): the algorithmic traffic of row a7's table).
+__global__ void __launch_bounds__(256) k_slab_tables_u(const TableArgs P) {
+    const Geom& g = P.g;
+    const int Ns = g.Ns, Nh = g.Nh;
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;      // over (s - s0, x3, x2, h)
+    const long long total = (long long)P.n_rows * Ns * Nh;
+    if (i >= total) return;
+    const int h = (int)(i % Nh);
+    const long long rr = i / Nh;                                                // (s - s0, x3, x2)
+    const int x2 = (int)(rr % Ns);
+    const int row = P.row0 + (int)(rr / Ns);                                    // s * Ns + x3
+    const int s = row / Ns, x3 = row - s * Ns;
+    unsigned acc0 = 0u, acc1 = 0u;                                              // parity-0 / parity-1 array element
+    for (int t = s * P.d; t < (s + 1) * P.d; ++t) {
+        const long long e = (((long long)t * Ns + x3) * Ns + x2) * Nh + h;
+        // the site of parity par in this row pair is x1 = 2h + ((par + x2 + x3 + t) & 1): over a slab the two arrays swap
+        // roles with t, so add each element to the sum of the x1 it belongs to
+        const unsigned a = (unsigned)__ldg(P.th + e), b = (unsigned)__ldg(P.th + g.Vh + e);
+        if ((x2 + x3 + t) & 1) { acc0 += b; acc1 += a; } else { acc0 += a; acc1 += b; }   // acc0: x1 = 2h, acc1: x1 = 2h + 1
+    }
+    double c0, s0, c1, s1;
+    ulm::sincos_bt_f64((int)acc0, c0, s0);
+    ulm::sincos_bt_f64((int)acc1, c1, s1);
+    double2* out = P.U + (long long)row * (Ns * Ns) + (long long)x2 * Ns + 2 * h;
+    out[0] = make_double2(c0, s0);                                               // the accumulation kernel re-reads U 6 r_max times:
+    out[1] = make_double2(c1, s1);                                               // keep it in L2
 }
 
 // plaquette orientation (a,b) -> table column o and sign of the sin channel (theta_P(b,a) = -theta_P(a,b))
@@ -393,6 +424,7 @@ struct AccumArgs {
     int r_begin, r_end;   // separations handled by this launch (multihit: r = 1 from the plain table, r >= 2 from Um)
     int a_r_max;          // the sums of T are written only for r <= a_r_max (field launch with multihit: r = 1 only)
     int first;            // 1: first pass of a measurement: the sums start from zero (no read, no memset)
+    long long idx0, n_idx; // (s, xs) entries handled by this launch: [idx0, idx0 + n_idx)  (a range of slabs)
     const double2* U;     // [nk][n_slab*Vs]
     const float* Ot;      // [nk][12][n_slab*Vs]   (n_fp > 0 only)
     const int* fps;       // device int[n_fp][3]
@@ -421,8 +453,8 @@ template <int KB, bool FIELD, bool FULL>
 __global__ void __launch_bounds__(256, FIELD ? UL_ACCF_MINB : UL_ACC_MINB) k_accumulate(const AccumArgs P) {
     const Geom& g = P.g;
     const long long n = (long long)P.n_slab * g.Vs;
-    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= n) return;
+    const long long idx = P.idx0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= P.idx0 + P.n_idx) return;
     const int s = (int)(idx / g.Vs);
     const int xs = (int)(idx - (long long)s * g.Vs);
     const int Ns = g.Ns;

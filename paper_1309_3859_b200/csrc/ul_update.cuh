@@ -14,6 +14,10 @@
 #pragma once
 #include "ul_math.cuh"
 
+#ifndef UL_PACKED_TRIG
+#define UL_PACKED_TRIG 1   // staple trigonometry on pairs of links with FFMA2 / FMUL2
+#endif
+
 namespace ulk {
 
 struct UpdateArgs {
@@ -22,6 +26,8 @@ struct UpdateArgs {
     int Ns, Nh, Nt;
     int parity;           // sub-step parity p
     int slab_d;           // 0 = unmasked; else spatial links with t % slab_d == 0 are frozen
+    int z0;               // first time layer of the launch (blockIdx.z + z0; for a masked spatial direction in units of
+                          // the enumerated non-frozen layers): launches restricted to a range of slabs
     float beta;
     uint32_t key0, key1;  // Philox key = seed
     uint32_t sweep_lo, sweep_hi;
@@ -90,6 +96,21 @@ __device__ __forceinline__ void staple_pair(const int* __restrict__ th, int Vh, 
     load_row<VEC, m1 - n1, OFF>(th, a_nu_p + st.e0 + st.dp[MU] + st.dm[NU], st, D);     // theta_nu(x+mu-nu)
     load_row<VEC, -n1, OFF>(th, a_mu_q + st.e0 + st.dm[NU], st, E);                     // theta_mu(x-nu)
     load_row<VEC, -n1, OFF>(th, a_nu_q + st.e0 + st.dm[NU], st, F);                     // theta_nu(x-nu)
+#if UL_POLY_TRIG && UL_PACKED_TRIG && !defined(UL_DBG_NOTRIG)
+    if (VEC >= 2) {                                     // two links per FFMA2 / FMUL2 (bit-identical to the scalar form)
+#pragma unroll
+        for (int i = 0; i + 1 < VEC; i += 2) {
+            ulm::f32x2 sx = ulm::pack2(Sx[i], Sx[i + 1]), sy = ulm::pack2(Sy[i], Sy[i + 1]);
+            ulm::cis_pair_accumulate2((int)((unsigned)A[i] + (unsigned)B[i] - (unsigned)C[i]),
+                                      (int)((unsigned)D[i] + (unsigned)E[i] - (unsigned)F[i]),
+                                      (int)((unsigned)A[i + 1] + (unsigned)B[i + 1] - (unsigned)C[i + 1]),
+                                      (int)((unsigned)D[i + 1] + (unsigned)E[i + 1] - (unsigned)F[i + 1]), sx, sy);
+            ulm::unpack2(sx, Sx[i], Sx[i + 1]);
+            ulm::unpack2(sy, Sy[i], Sy[i + 1]);
+        }
+        return;
+    }
+#endif
 #pragma unroll
     for (int i = 0; i < VEC; ++i) {
         ulm::cis_pair_accumulate((int)((unsigned)A[i] + (unsigned)B[i] - (unsigned)C[i]),
@@ -270,7 +291,7 @@ __global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_up
     const int bz = blockDim.z >> 1;
     const int sel = threadIdx.z >= bz ? 1 : 0;
     const int x3 = blockIdx.y * bz + (threadIdx.z - sel * bz);
-    int t = blockIdx.z;
+    int t = blockIdx.z + P.z0;
     if (MU != 0 && P.slab_d > 0) {                    // enumerate only the non-frozen layers
         const int dm = P.slab_d - 1;
         const int s = t / dm;

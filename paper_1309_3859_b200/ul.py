@@ -17,9 +17,9 @@ UL_OK, UL_EINVAL, UL_ENOMEM, UL_ECUDA, UL_ESTATE = 0, -1, -2, -3, -4
 # every symbol include/ul.h declares (tests check that the library exports exactly these)
 SYMBOLS = [
     "ul_create", "ul_create_ext", "ul_workspace_bytes", "ul_destroy", "ul_init", "ul_set_beta",
-    "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep",
+    "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep", "ul_substep_slabs", "ul_set_slab_group",
     "ul_set_subupdate", "ul_set_update_algorithm", "ul_multilevel", "ul_multilevel_replay", "ul_workspace_bytes_replay", "ul_multilevel2_replay", "ul_workspace_bytes_replay2", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
-    "ul_measure_end", "ul_set_accum_batch", "ul_set_multihit", "ul_plaquette", "ul_polyakov", "ul_set_site_offset", "ul_slab_partial_product", "ul_read_correlators", "ul_read_slab_averages",
+    "ul_measure_end", "ul_measure2_begin", "ul_combine", "ul_measure2_end", "ul_set_accum_batch", "ul_set_multihit", "ul_plaquette", "ul_polyakov", "ul_set_site_offset", "ul_slab_partial_product", "ul_read_correlators", "ul_read_slab_averages",
     "ul_get_launch_count", "ul_philox_selftest", "ul_sync", "ul_last_error",
 ]
 
@@ -57,6 +57,8 @@ def lib():
         L.ul_set_counter.argtypes = [P, C.c_uint64]
         L.ul_sweep.argtypes = [P, C.c_int, C.c_int]
         L.ul_substep.argtypes = [P, C.c_int, C.c_int, C.c_int, C.c_int]
+        L.ul_substep_slabs.argtypes = [P] + [C.c_int] * 6
+        L.ul_set_slab_group.argtypes = [P, C.c_int]
         L.ul_set_subupdate.argtypes = [P, C.c_int, C.c_int, C.c_int]
         L.ul_set_update_algorithm.argtypes = [P, C.c_int, C.c_double]
         L.ul_multilevel.argtypes = [P, C.c_int, C.c_int, C.c_int, P, C.c_int]
@@ -75,6 +77,9 @@ def lib():
         L.ul_slab_partial_product.argtypes = [P, C.c_int, C.c_int, P]
         L.ul_accumulate.argtypes = [P]
         L.ul_measure_end.argtypes = [P]
+        L.ul_measure2_begin.argtypes = [P, C.c_int, C.c_int, C.c_int, P, C.c_int]
+        L.ul_combine.argtypes = [P]
+        L.ul_measure2_end.argtypes = [P]
         L.ul_plaquette.argtypes = [P, P]
         L.ul_read_correlators.argtypes = [P, P, P, P]
         L.ul_read_slab_averages.argtypes = [P, P]
@@ -211,6 +216,12 @@ class Lattice:
     def substep(self, kind, parity, mu, slab_d=0):
         self._ck(lib().ul_substep(self._h, int(kind), int(parity), int(mu), int(slab_d)))
 
+    def substep_slabs(self, kind, parity, mu, slab_d, s_begin, s_end):
+        self._ck(lib().ul_substep_slabs(self._h, int(kind), int(parity), int(mu), int(slab_d), int(s_begin), int(s_end)))
+
+    def set_slab_group(self, n_slabs):
+        self._ck(lib().ul_set_slab_group(self._h, int(n_slabs)))
+
     def set_update_algorithm(self, alg, delta=np.pi):
         self._ck(lib().ul_set_update_algorithm(self._h, int(alg), float(delta)))
 
@@ -253,6 +264,17 @@ class Lattice:
 
     def measure_end(self):
         self._ck(lib().ul_measure_end(self._h))
+
+    def measure2_begin(self, d_in, d_out, r_max, field_points=None):
+        fp, n = _fps(field_points)
+        self._ck(lib().ul_measure2_begin(self._h, int(d_in), int(d_out), int(r_max), _ptr(fp), n))
+        self._meas = (int(r_max), n, self.Nt // int(d_out))
+
+    def combine(self):
+        self._ck(lib().ul_combine(self._h))
+
+    def measure2_end(self):
+        self._ck(lib().ul_measure2_end(self._h))
 
     def plaquette(self):
         out = np.zeros(3)

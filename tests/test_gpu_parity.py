@@ -334,6 +334,110 @@ def test_p2_two_level_one_iteration_matches_oracle_combine(ul, ulo):
     assert np.allclose(c1, cg, atol=1e-12) and np.allclose(f1, fg, atol=1e-12)
 
 
+@pytest.mark.parametrize("Ns,Nt,d_in,d_out,n_in,n_out,batch", [(8, 8, 2, 4, 3, 2, 0), (6, 12, 2, 6, 4, 3, 3), (8, 8, 1, 4, 5, 2, 2)])
+def test_p2_two_level_with_averaging_on_oracle_configurations(ul, ulo, Ns, Nt, d_in, d_out, n_in, n_out, batch):
+    """Two-level estimator with REAL averaging (n_in >= 3, n_out >= 2; Eq. 27, Eqs. 32-34, Alg. 1
+    lines 5-18) against the oracle on the oracle's own trajectory: the oracle runs its sub-updates, every inner
+    configuration is handed to the GPU (ul_set_links) and added on both sides (ul_accumulate / ulo_accumulate), both
+    combine per outer iteration (k_combine with inv = 1/n_in vs Eqs. 32-33 in the oracle) and close (1/n_out, slab
+    product).  [T^(d_out)], C, G, vacuum to relative 1e-5 (R17) with the rms of the summed terms taken from the
+    oracle's slab averages."""
+    R = 3
+    fps = FPS[:4]
+    o = ulo.Oracle(Ns, Nt, 1.0, 11)
+    for _ in range(6):
+        o.sweep(1, 3)
+    g = ul.Lattice(Ns, Nt, 1.0, 11)
+    g.set_accum_batch(batch)
+    o.measure2_begin(d_in, d_out, R, fps)
+    g.measure2_begin(d_in, d_out, R, fps)
+
+    def masked_compound(d):
+        for parity in (0, 1):
+            for mu in range(4):
+                o.substep(0, parity, mu, d)
+        o.set_counter(o.get_counter() + 1)
+        for parity in (0, 1):
+            for mu in range(4):
+                o.substep(1, parity, mu, d)
+
+    for J in range(n_out):
+        masked_compound(d_out)
+        for j in range(n_in):
+            masked_compound(d_in)
+            g.set_links(o.get_links())
+            o.accumulate()
+            g.accumulate()
+        o.combine()
+        g.combine()
+    o.measure2_end()
+    g.measure2_end()
+    co, fo, vo = o.read_correlators()
+    cg, fg, vg = g.read_correlators()
+    T4, TO4 = o.read_slab_averages(), o.read_slab_field_averages()       # [3][R][S][Vs], [3][R][S][F][12][Vs]
+    assert np.abs(T4).max() < 0.999                                      # averaged: not single-configuration phases
+    assert np.abs(g.read_slab_averages() - T4).max() < 1e-5 * max(np.abs(T4).max(), 1e-2)
+    Vs, S = Ns ** 3, Nt // d_out
+    termC = T4.prod(axis=2)                                              # the 3 Vs summed terms of C(r)
+    termG = 0
+    for s_ in range(S):
+        termG = termG + TO4[:, :, s_] * np.delete(T4, s_, axis=2).prod(axis=2)[:, :, None, None, :]
+    rmsC = np.sqrt((np.abs(termC) ** 2).mean(axis=(0, 2)))               # [R]
+    rmsG = np.sqrt((np.abs(termG) ** 2).mean(axis=(0, 4))) / Nt          # [R][F][12]
+    ok, worst = rel_ok(cg, co, 3 * Vs, rms_term=rmsC)
+    assert ok, ("C", worst)
+    ok, worst = rel_ok(fg, fo, 3 * Vs, rms_term=rmsG)
+    assert ok, ("G", worst)
+    ok, worst = rel_ok(vg, vo, 3 * Vs * Nt)
+    assert ok, ("vacuum", worst)
+    # state errors of the hooks
+    g.measure2_begin(d_in, d_out, R, fps)
+    with pytest.raises(ul.UlError):
+        g.combine()
+    g.accumulate()
+    with pytest.raises(ul.UlError):
+        g.measure2_end()
+    with pytest.raises(ul.UlError):
+        g.measure_end()
+    g.combine()
+    g.accumulate(); g.accumulate()
+    with pytest.raises(ul.UlError):
+        g.combine()                                                      # 2 configurations after 1 in the first iteration
+
+
+def test_two_level_hooks_equal_multilevel2_on_device(ul):
+    """ul_measure2_begin / ul_accumulate / ul_combine / ul_measure2_end with the sweeps issued by hand reproduce
+    ul_multilevel2 bit for bit (same kernels, same order)."""
+    Ns, Nt, R, n_in, n_out = 8, 8, 3, 3, 2
+    a = ul.Lattice(Ns, Nt, 1.0, 5)
+    b = ul.Lattice(Ns, Nt, 1.0, 5)
+    a.sweep(3, 3); b.sweep(3, 3)
+    a.multilevel2(2, n_in, 4, n_out, R, FPS[:2])
+    b.measure2_begin(2, 4, R, FPS[:2])
+
+    def masked(d):
+        for parity in (0, 1):
+            for mu in range(4):
+                b.substep(0, parity, mu, d)
+        b.set_counter(b.get_counter() + 1)
+        for _ in range(3):
+            for parity in (0, 1):
+                for mu in range(4):
+                    b.substep(1, parity, mu, d)
+
+    for J in range(n_out):
+        masked(4)
+        for j in range(n_in):
+            masked(2)
+            b.accumulate()
+        b.combine()
+    b.measure2_end()
+    for x, y in zip(a.read_correlators(), b.read_correlators()):
+        assert np.array_equal(x, y)
+    assert np.array_equal(a.read_slab_averages(), b.read_slab_averages())
+    assert np.array_equal(a.get_links_raw(), b.get_links_raw())
+
+
 def test_p2_closed_forms_on_device(ul):
     """Pins that need no oracle: cold start, constant flux, Polyakov winding (SURVEY 8(c) pins)."""
     Ns, Nt = 8, 4
@@ -1108,3 +1212,57 @@ def test_beta_zero_heatbath_is_uniform_on_device(ul):
     th = g.get_links().astype(np.float64).ravel()
     _, p = stats.kstest(th, lambda x: (x + np.pi) / (2 * np.pi))
     assert p > 1e-3 and abs(g.plaquette()[0]) < 0.01
+
+
+# ----------------------------------------------------------------------------- slab-group-major order
+@pytest.mark.parametrize("Ns,Nt,d,grp,alg,n_fp", [(8, 8, 2, 1, 0, 0), (8, 12, 2, 4, 0, 3), (6, 8, 4, 1, 1, 2), (16, 16, 2, 3, 0, 0)])
+def test_slab_group_major_order_is_bit_identical(ul, Ns, Nt, d, grp, alg, n_fp):
+    """ul_set_slab_group: the n_sub loop run slab group by slab group (ragged last group, ragged last batch) gives
+    the same links, sweep counter, slab sums, C(r) and G bit for bit as the sub-update-major order; vacuum to 1e-13."""
+    R, n_sub = 3, 5
+    fps = FPS[:n_fp]
+    res = []
+    for mode in (0, grp):
+        g = ul.Lattice(Ns, Nt, 1.0, 9)
+        g.sweep(2, 2)
+        if alg:
+            g.set_update_algorithm(1, 1.3)
+        g.set_accum_batch(2)
+        g.set_slab_group(mode)
+        g.multilevel(d, n_sub, R, fps)
+        res.append((g.get_links_raw(), g.get_counter(), g.read_slab_averages(), *g.read_correlators()))
+    a, b = res
+    assert np.array_equal(a[0], b[0]) and a[1] == b[1]
+    assert np.array_equal(a[2], b[2]) and np.array_equal(a[3], b[3]) and np.array_equal(a[4], b[4])
+    assert np.allclose(a[5], b[5], rtol=0, atol=1e-13)
+
+
+def test_substep_slabs_covers_the_masked_substep(ul):
+    """ul_substep_slabs over a partition of the slabs == ul_substep with the same mask (heatbath, every direction)."""
+    Ns, Nt, d = 8, 12, 2
+    a = ul.Lattice(Ns, Nt, 1.0, 4)
+    b = ul.Lattice(Ns, Nt, 1.0, 4)
+    for parity in (0, 1):
+        for mu in range(4):
+            a.substep(0, parity, mu, d)
+            for s0, s1 in ((4, 6), (0, 1), (1, 4)):
+                b.substep_slabs(0, parity, mu, d, s0, s1)
+    assert np.array_equal(a.get_links_raw(), b.get_links_raw())
+    with pytest.raises(ul.UlError):
+        b.substep_slabs(0, 0, 0, d, 3, 7)
+
+
+def test_vacuum_without_field_points_is_that_of_the_final_configuration(ul, ulo):
+    """n_fp = 0: the plaquettes are not evaluated per sub-update (U-table fast path); the vacuum values returned are
+    those of the final configuration (include/ul.h), checked against the oracle's frozen-configuration vacuum."""
+    Ns, Nt = 8, 4
+    g = ul.Lattice(Ns, Nt, 1.0, 2)
+    g.sweep(3, 3)
+    g.multilevel(2, 3, 3)
+    _, _, vg = g.read_correlators()
+    o = ulo.Oracle(Ns, Nt, 1.0, 2)
+    o.set_links(g.get_links())
+    o.multilevel(2, 0, 1)
+    _, _, vo = o.read_correlators()
+    ok, worst = rel_ok(vg, vo, 3 * Ns ** 3 * Nt)
+    assert ok, worst
