@@ -32,7 +32,7 @@ struct UpdateArgs {
     uint32_t key0, key1;  // Philox key = seed
     uint32_t sweep_lo, sweep_hi;
     const uint32_t* sweep_dev;   // DEVCTR kernels (CUDA-graph replays) read the sweep counter from here instead
-    int4* queue;          // heatbath stragglers: (element offset, site | tries << 29, Sx, Sy), see k_hb_stragglers
+    int4* queue;          // heatbath stragglers: (element offset in th[mu][parity] | tries << 28, site, Sx, Sy), see k_hb_stragglers
     int* qcount;          // entries queued per block (zeroed before the launch); segment b = queue[b*HB_QSEG ...]
     int qblocks;          // number of segments
     int local_rounds;     // lane-local retry rounds before a link is queued
@@ -192,18 +192,41 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
         const uint32_t c3 = ((uint32_t)p << 2) | (uint32_t)MU;                            // tag 0 = heatbath
         float pa[VEC], pq[VEC], pc[VEC], sn[VEC], cs[VEC];
         uint32_t pend = 0u, neg = 0u, tries = 0u, zero = 0u;                              // tries: 8 bits per link
+        if (VEC >= 2) {
 #pragma unroll
-        for (int i = 0; i < VEC; ++i) {
-            const float k2 = fmaf(Sx[i], Sx[i], Sy[i] * Sy[i]);
-            if (k2 == 0.0f) { Sx[i] = 1.0f; Sy[i] = 0.0f; zero |= 1u << i; }                // k = 0: alpha = 0 (O1)
+            for (int i = 0; i + 1 < VEC; i += 2) {                                        // two links per FFMA2 (ul_math.cuh)
+                float a2[2];
+                uint32_t w[2][4];
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    const float k2 = fmaf(Sx[i + j], Sx[i + j], Sy[i + j] * Sy[i + j]);
+                    if (k2 == 0.0f) { Sx[i + j] = 1.0f; Sy[i + j] = 0.0f; zero |= 1u << (i + j); }   // k = 0: alpha = 0 (O1)
+                    a2[j] = P.beta * ulm::mufu_sqrt(k2);
+                    ulm::philox4x32_10(site0 + 2u * (i + j), sweep_lo, sweep_hi, c3, P.key0, P.key1, w[j]);
+                }
+                ulm::HbParams h0, h1;
+                ulm::hb_setup2(a2[0], a2[1], h0, h1);
+                pa[i] = h0.a; pq[i] = h0.q; pc[i] = h0.c0; pa[i + 1] = h1.a; pq[i + 1] = h1.q; pc[i + 1] = h1.c0;
+                ulm::f32x2 sn2, cs2;
+                bool ok0, ok1;
+                ulm::hb_attempt2(h0, h1, w[0][0], w[0][1], w[1][0], w[1][1], sn2, cs2, ok0, ok1);
+                ulm::unpack2(sn2, sn[i], sn[i + 1]);
+                ulm::unpack2(cs2, cs[i], cs[i + 1]);
+                neg |= ((w[0][2] >> 31) << i) | ((w[1][2] >> 31) << (i + 1));
+                pend |= ((ok0 ? 0u : 1u) << i) | ((ok1 ? 0u : 1u) << (i + 1));
+                tries |= (1u << (8 * i)) | (1u << (8 * (i + 1)));
+            }
+        } else {
+            const float k2 = fmaf(Sx[0], Sx[0], Sy[0] * Sy[0]);
+            if (k2 == 0.0f) { Sx[0] = 1.0f; Sy[0] = 0.0f; zero |= 1u; }                    // k = 0: alpha = 0 (O1)
             const ulm::HbParams hp = ulm::hb_setup(P.beta * ulm::mufu_sqrt(k2));
-            pa[i] = hp.a; pq[i] = hp.q; pc[i] = hp.c0;
+            pa[0] = hp.a; pq[0] = hp.q; pc[0] = hp.c0;
             uint32_t w[4];
-            ulm::philox4x32_10(site0 + 2u * i, sweep_lo, sweep_hi, c3, P.key0, P.key1, w);
-            const bool ok = ulm::hb_attempt(hp, w[0], w[1], sn[i], cs[i]);
-            neg |= (w[2] >> 31) << i;
-            pend |= (ok ? 0u : 1u) << i;
-            tries |= 1u << (8 * i);
+            ulm::philox4x32_10(site0, sweep_lo, sweep_hi, c3, P.key0, P.key1, w);
+            const bool ok = ulm::hb_attempt(hp, w[0], w[1], sn[0], cs[0]);
+            neg |= w[2] >> 31;
+            pend |= ok ? 0u : 1u;
+            tries |= 1u;
         }
         auto retry_one = [&]() {                                                          // one more attempt of this lane's first pending link
             const int j = __ffs(pend) - 1;
@@ -225,10 +248,15 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
         // queue instead of keeping the whole warp looping for its unluckiest lane; k_hb_stragglers finishes
         // them (same attempt counters, same arithmetic) right after this kernel.  One atomic per warp on the
         // block's own counter; links that do not fit in the segment are simply finished here.
-        const unsigned wmask = __activemask();
+        // the lanes of this warp that exist: every thread of the block reaches this point (no early exits), so the mask is
+        // known from the block size and the warp is re-converged explicitly after the divergent retry rounds
+        const int tid_ = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+        const int in_warp = min(32, (int)(blockDim.x * blockDim.y * blockDim.z) - (tid_ & ~31));
+        const unsigned wmask = in_warp == 32 ? 0xffffffffu : ((1u << in_warp) - 1u);
+        __syncwarp(wmask);
         const unsigned lanes = __ballot_sync(wmask, pend != 0u);
         if (lanes) {
-            const int lane = (threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z)) & 31;
+            const int lane = tid_ & 31;
             const int blk = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
             int mine = __popc(pend), incl = mine;
 #pragma unroll
@@ -246,7 +274,7 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
             for (int i = 0; i < VEC; ++i)
                 if (((pend >> i) & 1u) && pos < HB_QSEG) {
                     const uint32_t n = (tries >> (8 * i)) & 0xffu;                        // <= 1 + local_rounds <= 7
-                    P.queue[blk * HB_QSEG + pos] = make_int4((MU * 2 + p) * P.Vh + st.e0 + i, (int)((site0 + 2u * i) | (n << 29)),
+                    P.queue[blk * HB_QSEG + pos] = make_int4((st.e0 + i) | (int)(n << 28), (int)(site0 + 2u * i),
                                                              __float_as_int(((zero >> i) & 1u) ? 0.0f : Sx[i]), __float_as_int(Sy[i]));
                     ++pos;
                     pend &= ~(1u << i);
@@ -255,8 +283,14 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
                 }
             while (pend) retry_one();
         }
+        if (VEC >= 2) {
 #pragma unroll
-        for (int i = 0; i < VEC; ++i) out[i] = ulm::hb_finish(Sx[i], Sy[i], sn[i], cs[i], ((neg >> i) & 1u) != 0);
+            for (int i = 0; i + 1 < VEC; i += 2)
+                ulm::hb_finish2(ulm::pack2(Sx[i], Sx[i + 1]), ulm::pack2(Sy[i], Sy[i + 1]), ulm::pack2(sn[i], sn[i + 1]), ulm::pack2(cs[i], cs[i + 1]),
+                                ((neg >> i) & 1u) != 0, ((neg >> (i + 1)) & 1u) != 0, out[i], out[i + 1]);
+        } else {
+            out[0] = ulm::hb_finish(Sx[0], Sy[0], sn[0], cs[0], (neg & 1u) != 0);
+        }
     }
     if (VEC == 4) *reinterpret_cast<int4*>(own) = make_int4(out[0], out[1 % VEC], out[2 % VEC], out[3 % VEC]);
     else if (VEC == 2) *reinterpret_cast<int2*>(own) = make_int2(out[0], out[1 % VEC]);
@@ -337,8 +371,8 @@ __global__ void __launch_bounds__(256) k_hb_stragglers(const UpdateArgs P, int m
         if (e % HB_QSEG == 0 && seg < P.qblocks) P.qcount[seg] = 0;                       // zero it for the next heatbath sub-step
         if ((e % HB_QSEG) >= cnt) return;
         const int4 q = P.queue[e];
-        const uint32_t site = (uint32_t)q.y & 0x1fffffffu;
-        uint32_t n = (uint32_t)q.y >> 29;
+        const uint32_t site = (uint32_t)q.y;                                              // all 32 bits: ghost-layer sites of a shard wrap
+        uint32_t n = (uint32_t)q.x >> 28;                                                 // V/2 <= 2^28 elements per array (ul_create)
         float Sx = __int_as_float(q.z);
         const float Sy = __int_as_float(q.w);
         const float k2 = fmaf(Sx, Sx, Sy * Sy);
@@ -352,7 +386,7 @@ __global__ void __launch_bounds__(256) k_hb_stragglers(const UpdateArgs P, int m
             if (ok || n == 63u) break;
             ++n;
         }
-        P.th[q.x] = ulm::hb_finish(Sx, Sy, sn, cs, (w[2] >> 31) != 0);
+        P.th[(mu * 2 + P.parity) * P.Vh + (q.x & 0x0fffffff)] = ulm::hb_finish(Sx, Sy, sn, cs, (w[2] >> 31) != 0);
     }
 }
 
