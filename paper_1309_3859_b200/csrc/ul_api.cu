@@ -64,8 +64,7 @@ Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_f
     if (np < 12 * (TBLK / NBLK)) np = 12 * (TBLK / NBLK);
     size_t partial_doubles = np * NBLK;
     if (replay) {                                   // fields: replay_blocks() partials per entry; correlators: NBLK per entry
-        size_t nb = replay_blocks((long long)(n_in * Vs));
-        if (nb < 12) nb = 12;                       // the plane kernel writes up to 3 * 4 partials per entry
+        const size_t nb = replay_blocks((long long)(n_in * Vs));
         partial_doubles = 2 * R * NBLK + 2 * R * F12 * nb;
         if (partial_doubles < (size_t)12 * TBLK) partial_doubles = (size_t)12 * TBLK;
     }
@@ -764,7 +763,7 @@ bool full_plane(const ul_ctx* c, const int* fps, int n_fp, int* a_out) {
     *a_out = fps[0];
     return true;
 }
-// one configuration's W T O reduction into the result sums: k_replay_reduce, or the tiled plane kernel for full planes
+// one configuration's W T O reduction into the result sums: k_replay_reduce, or the transverse-DFT route for full planes
 int reduce_fields(ul_ctx* c, const ulk::ReplayArgs& ra, bool plane, int plane_a, int n_entries, double scale) {
     double* res = wsp<double>(c, c->ws.result);
     const long long n = (long long)c->n_slab * c->Vs;

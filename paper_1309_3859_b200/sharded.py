@@ -15,7 +15,8 @@ rest of the lattice"), so the lattice is cut in t into shards of whole slabs, on
     CPU tests), multiply them in rank order and average over the lattice: row a10, Eq. 24.
 
 This module holds the partition arithmetic and that exchange; every arithmetic step of the method still runs in
-the CUDA kernels.  Full (unmasked) sweeps would need a halo layer per sub-step and are not sharded here.
+the CUDA kernels.  Full (unmasked) sweeps exchange one halo of the written array per sub-step:
+ShardedSweeper / sharded_sweep below.
 """
 import numpy as np
 
