@@ -132,6 +132,10 @@ static void k_alpha(const cplx& S, double* k, double* alpha) {
 
 // ---------------------------------------------------------------- heatbath (S8(c)-O3, DESIGN R2)
 // Best-Fisher wrapped-Cauchy rejection for phi ~ exp(a cos phi) on (-pi, pi).
+// Word-to-variate map (DESIGN R19, as revised in round 2): a Philox block holds four words and an attempt needs two
+// uniforms and a sign, so attempt n takes block n >> 1 (counter word 3 = (block << 8) | c3low) and, of that block,
+// the word pair (w[0], w[1]) when n is even, (w[2], w[3]) when n is odd: u1 = U(first), u2 = U(second), and the
+// sign is bit 0 of the first word (U() reads bits 9..31 only, so the sign is independent of u1).
 static double heatbath_phi(double a, const uint32_t key[2], uint32_t c0, uint32_t c1, uint32_t c2,
                            uint32_t c3low, int* attempts_out) {
     const double tau = 1.0 + std::sqrt(1.0 + 4.0 * a * a);
@@ -141,20 +145,23 @@ static double heatbath_phi(double a, const uint32_t key[2], uint32_t c0, uint32_
     const double ar = (1.0 + rho * rho) * s / 4.0;
     double phi = 0.0;
     int n = 0;
+    uint32_t w[4] = {0, 0, 0, 0};
     for (; n < 64; ++n) {
-        const uint32_t ctr[4] = {c0, c1, c2, ((uint32_t)n << 8) | c3low};
-        uint32_t w[4];
-        ulo_philox4x32_10(ctr, key, w);
-        const double u1 = U_of(w[0]);
-        const double u2 = U_of(w[1]);
-        const double sgn = (w[2] >> 31) ? -1.0 : 1.0;
+        if ((n & 1) == 0) {
+            const uint32_t ctr[4] = {c0, c1, c2, ((uint32_t)(n >> 1) << 8) | c3low};
+            ulo_philox4x32_10(ctr, key, w);
+        }
+        const uint32_t wa = w[2 * (n & 1)], wb = w[2 * (n & 1) + 1];
+        const double u1 = U_of(wa);
+        const double u2 = U_of(wb);
+        const double sgn = (wa & 1u) ? -1.0 : 1.0;
         const double T = q * std::tan(PI * u1 / 2.0);
         const double f = (1.0 - T * T) / (1.0 + T * T);
         const double cc = ar - a * f;
         phi = sgn * 2.0 * std::atan(T);
         if (u2 <= cc * std::exp(1.0 - cc)) { ++n; break; }
     }
-    if (attempts_out) *attempts_out = n;  // number of Philox blocks consumed (cap 64: last proposal kept)
+    if (attempts_out) *attempts_out = n;  // number of attempts made (cap 64: the last proposal is kept)
     return phi;
 }
 

@@ -87,6 +87,36 @@ def test_heatbath_stream_is_counter_based(ulo):
     assert a == b and a != c
 
 
+def test_heatbath_word_to_variate_map(ulo):
+    # DESIGN R19 (round 2): attempt n takes Philox block n >> 1 (counter word 3 = (block << 8) | c3low) and of it the words
+    # (w0, w1) for even n, (w2, w3) for odd n: u1 = U(first), u2 = U(second), sign = bit 0 of the first word;
+    # U(w) = (2 (w >> 9) + 1) 2^-24.  Restated here from the pinned Philox block function, attempt by attempt.
+    seed, c3low = 0x9E3779B97F4A7C15, (1 << 2) | 3
+    seen = set()
+    for a in (0.3, 2.0, 4.1, 12.0):
+        tau = 1 + np.sqrt(1 + 4 * a * a)
+        s = tau + np.sqrt(2 * tau)
+        rho = 2 * a / s
+        q, ar = (1 - rho) / (1 + rho), (1 + rho * rho) * s / 4
+        for site in range(400):
+            phi, att = ulo.heatbath_phi(a, seed, site, 11, 2, c3low)
+            n, w = 0, None
+            while True:
+                if n % 2 == 0:
+                    w = ulo.philox4x32_10([site, 11, 2, ((n >> 1) << 8) | c3low], [seed & 0xffffffff, seed >> 32])
+                wa, wb = int(w[2 * (n & 1)]), int(w[2 * (n & 1) + 1])
+                u1, u2 = (2 * (wa >> 9) + 1) * 2.0 ** -24, (2 * (wb >> 9) + 1) * 2.0 ** -24
+                T = q * np.tan(np.pi * u1 / 2)
+                cc = ar - a * (1 - T * T) / (1 + T * T)
+                n += 1
+                if u2 <= cc * np.exp(1 - cc):
+                    break
+            assert att == n, (a, site, att, n)
+            assert abs(phi - (-1.0 if wa & 1 else 1.0) * 2 * np.arctan(T)) < 1e-12
+            seen.add(n)
+    assert {1, 2, 3}.issubset(seen)                       # both halves of a block and a second block were exercised
+
+
 def test_hot_start_matches_keying(ulo):
     # S8(c)-O4: theta = fp32(2 pi w0 2^-32 - pi), ctr = (site, 0, 0, (1<<3)|mu), key = seed words
     seed = (0x1234 << 32) | 0xABCDEF01
