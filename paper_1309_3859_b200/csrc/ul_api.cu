@@ -77,11 +77,11 @@ Workspace plan_workspace(int Ns, int Nt, int d_in, int d_out, int r_max, int n_f
 }  // namespace
 
 struct GraphKey {
-    int n_hb, n_or, slab_d, alg, local_rounds;
+    int n_hb, n_or, slab_d, alg;
     double beta, met_delta;
     uint32_t site_offset;
     bool operator==(const GraphKey& o) const {
-        return n_hb == o.n_hb && n_or == o.n_or && slab_d == o.slab_d && alg == o.alg && local_rounds == o.local_rounds &&
+        return n_hb == o.n_hb && n_or == o.n_or && slab_d == o.slab_d && alg == o.alg &&
                beta == o.beta && met_delta == o.met_delta && site_offset == o.site_offset;
     }
 };
@@ -109,7 +109,6 @@ struct ul_ctx {
     int4* hb_queue = nullptr; // heatbath straggler queue (library-owned)
     int* hb_qcount = nullptr;
     int hb_qblocks = 0;
-    int hb_local_rounds = 2;
     uint32_t* d_sweep = nullptr;      // device copy of the sweep counter for graph replays
     bool d_sweep_stale = true;
     bool use_graphs = false, capturing = false;
@@ -216,7 +215,7 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin = 0
     a.sweep_lo = (uint32_t)(c->sweep & 0xffffffffu); a.sweep_hi = (uint32_t)(c->sweep >> 32); a.sweep_dev = c->d_sweep;
     const dim3 block(c->bx, c->by, 2 * c->bz), grid(c->Nh / c->by, c->Ns / c->bz, n_t);   // by = x2 row PAIRS per block
     a.site_offset = c->site_offset;
-    a.queue = c->hb_queue; a.qcount = c->hb_qcount; a.qblocks = (int)(grid.x * grid.y * grid.z); a.local_rounds = c->hb_local_rounds;
+    a.queue = c->hb_queue; a.qcount = c->hb_qcount; a.qblocks = (int)(grid.x * grid.y * grid.z);
     {
         const double units = c->met_delta * (4294967296.0 / 6.283185307179586476925286766559);
         a.met_delta_bt = units >= 2147483647.0 ? 2147483647 : (int)(units + 0.5);
@@ -226,7 +225,7 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin = 0
     if (e != cudaSuccess) return fail(c, UL_ECUDA, std::string("k_update launch: ") + cudaGetErrorString(e));
     c->launches += 1;
     if (kind == 0) {                                  // finish the links the heatbath kernel queued
-        const int nb = (a.qblocks * ulk::HB_QSEG + 255) / 256;        // it also zeroes the counters for the next sub-step
+        const int nb = (a.qblocks + ulk::HB_SPB - 1) / ulk::HB_SPB;   // it also zeroes the counters for the next sub-step
         if (c->capturing) ulk::k_hb_stragglers<true><<<nb, 256, 0, c->stream>>>(a, mu);
         else ulk::k_hb_stragglers<false><<<nb, 256, 0, c->stream>>>(a, mu);
         if (cudaGetLastError() != cudaSuccess) return fail(c, UL_ECUDA, "k_hb_stragglers launch");
@@ -258,7 +257,7 @@ int compound_direct(ul_ctx* c, int n_hb, int n_or, int slab_d, int s_begin = 0, 
 // never changes -- and replayed on the caller's stream.  Same kernels, same arithmetic, same results.
 int compound(ul_ctx* c, int n_hb, int n_or, int slab_d) {
     if (!c->use_graphs || n_hb + n_or == 0) return compound_direct(c, n_hb, n_or, slab_d);
-    GraphKey key{n_hb, n_or, slab_d, c->alg, c->hb_local_rounds, c->beta, c->met_delta, c->site_offset};
+    GraphKey key{n_hb, n_or, slab_d, c->alg, c->beta, c->met_delta, c->site_offset};
     CachedGraph* g = nullptr;
     for (auto& e : c->graphs) if (e.key == key) g = &e;
     if (!g) {

@@ -32,15 +32,14 @@ struct UpdateArgs {
     uint32_t key0, key1;  // Philox key = seed
     uint32_t sweep_lo, sweep_hi;
     const uint32_t* sweep_dev;   // DEVCTR kernels (CUDA-graph replays) read the sweep counter from here instead
-    int4* queue;          // heatbath stragglers: (element offset in th[mu][parity] | tries << 28, site, Sx, Sy), see k_hb_stragglers
+    int4* queue;          // heatbath stragglers: (element offset in th[mu][parity], site, Sx, Sy), see k_hb_stragglers
     int* qcount;          // entries queued per block (zeroed before the launch); segment b = queue[b*HB_QSEG ...]
     int qblocks;          // number of segments
-    int local_rounds;     // lane-local retry rounds before a link is queued
     uint32_t site_offset; // added to the local canonical site index in the Philox counter (slab sharding: t0 * Ns^3)
     int met_delta_bt;     // Metropolis proposal half-width delta as a binary angle (0 < delta <= pi -> up to 2^31 - 1)
 };
 
-constexpr int HB_QSEG = 128;   // straggler-queue entries per thread block (expected use ~25 of 1024 links)
+constexpr int HB_QSEG = 192;   // straggler-queue entries per thread block (expected use 85-120 of 1024 links: both attempts of block 0 rejected)
 
 // per-thread addressing state
 struct Site {
@@ -184,112 +183,72 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
             out[i] = accept ? (int)((unsigned)old[i] + (unsigned)d) : old[i];
         }
     } else {
-        // Heatbath (O3).  Attempt n of a link is a pure function of (site, sweep, n), so the order in
-        // which a thread works through its rejections is free: every link gets attempt 0 with the warp
-        // converged; a lane then retries its own rejected links one at a time (lane-local queue), which
-        // bounds the warp's extra rounds by the worst lane's total instead of the sum of per-link maxima.
+        // Heatbath (O3).  Attempt n of a link is a pure function of (site, sweep, n): Philox block n >> 1, word pair
+        // n & 1 (DESIGN R19).  Every link gets its block 0, i.e. attempts 0 and 1, here with the warp converged: the two
+        // attempts of a link are the two lanes of the packed arithmetic, and the first accepted one is taken.  The links
+        // that rejected both (8-12 %) go to this block's segment of the straggler queue and k_hb_stragglers finishes them
+        // from block 1 on (same counters, same device functions), so no warp loops for its unluckiest lane.
         const uint32_t site0 = (uint32_t)((st.e0 - h0) * 2 + 2 * h0 + st.off) + P.site_offset;            // canonical site index
-        const uint32_t c3 = ((uint32_t)p << 2) | (uint32_t)MU;                            // tag 0 = heatbath
-        float pa[VEC], pq[VEC], pc[VEC], sn[VEC], cs[VEC];
-        uint32_t pend = 0u, neg = 0u, tries = 0u, zero = 0u;                              // tries: 8 bits per link
-        if (VEC >= 2) {
+        const uint32_t c3 = ((uint32_t)p << 2) | (uint32_t)MU;                            // tag 0 = heatbath, block 0
+        // A pair of links is taken all the way to its new angles before the next pair starts (short live ranges: 64
+        // registers); the angle written for a link that is still pending is a placeholder that k_hb_stragglers overwrites.
+        uint32_t pend = 0u, zero = 0u;
+        float a[VEC];
 #pragma unroll
-            for (int i = 0; i + 1 < VEC; i += 2) {                                        // two links per FFMA2 (ul_math.cuh)
-                float a2[2];
-                uint32_t w[2][4];
-#pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                    const float k2 = fmaf(Sx[i + j], Sx[i + j], Sy[i + j] * Sy[i + j]);
-                    if (k2 == 0.0f) { Sx[i + j] = 1.0f; Sy[i + j] = 0.0f; zero |= 1u << (i + j); }   // k = 0: alpha = 0 (O1)
-                    a2[j] = P.beta * ulm::mufu_sqrt(k2);
-                    ulm::philox4x32_10(site0 + 2u * (i + j), sweep_lo, sweep_hi, c3, P.key0, P.key1, w[j]);
-                }
-                ulm::HbParams h0, h1;
-                ulm::hb_setup2(a2[0], a2[1], h0, h1);
-                pa[i] = h0.a; pq[i] = h0.q; pc[i] = h0.c0; pa[i + 1] = h1.a; pq[i + 1] = h1.q; pc[i + 1] = h1.c0;
-                ulm::f32x2 sn2, cs2;
-                bool ok0, ok1;
-                ulm::hb_attempt2(h0, h1, w[0][0], w[0][1], w[1][0], w[1][1], sn2, cs2, ok0, ok1);
-                ulm::unpack2(sn2, sn[i], sn[i + 1]);
-                ulm::unpack2(cs2, cs[i], cs[i + 1]);
-                neg |= ((w[0][2] >> 31) << i) | ((w[1][2] >> 31) << (i + 1));
-                pend |= ((ok0 ? 0u : 1u) << i) | ((ok1 ? 0u : 1u) << (i + 1));
-                tries |= (1u << (8 * i)) | (1u << (8 * (i + 1)));
-            }
-        } else {
-            const float k2 = fmaf(Sx[0], Sx[0], Sy[0] * Sy[0]);
-            if (k2 == 0.0f) { Sx[0] = 1.0f; Sy[0] = 0.0f; zero |= 1u; }                    // k = 0: alpha = 0 (O1)
-            const ulm::HbParams hp = ulm::hb_setup(P.beta * ulm::mufu_sqrt(k2));
-            pa[0] = hp.a; pq[0] = hp.q; pc[0] = hp.c0;
-            uint32_t w[4];
-            ulm::philox4x32_10(site0, sweep_lo, sweep_hi, c3, P.key0, P.key1, w);
-            const bool ok = ulm::hb_attempt(hp, w[0], w[1], sn[0], cs[0]);
-            neg |= w[2] >> 31;
-            pend |= ok ? 0u : 1u;
-            tries |= 1u;
+        for (int i = 0; i < VEC; ++i) {
+            const float k2 = fmaf(Sx[i], Sx[i], Sy[i] * Sy[i]);
+            if (k2 == 0.0f) { Sx[i] = 1.0f; Sy[i] = 0.0f; zero |= 1u << i; }               // k = 0: alpha = 0 (O1)
+            a[i] = P.beta * ulm::mufu_sqrt(k2);
         }
-        auto retry_one = [&]() {                                                          // one more attempt of this lane's first pending link
-            const int j = __ffs(pend) - 1;
-            ulm::HbParams hp;
-            hp.a = pick<float, VEC>(pa, j); hp.q = pick<float, VEC>(pq, j); hp.c0 = pick<float, VEC>(pc, j);
-            const uint32_t n = (tries >> (8 * j)) & 0xffu;
-            uint32_t w[4];
-            ulm::philox4x32_10(site0 + 2u * (uint32_t)j, sweep_lo, sweep_hi, (n << 8) | c3, P.key0, P.key1, w);
-            float s1, c1;
-            const bool ok = ulm::hb_attempt(hp, w[0], w[1], s1, c1);
 #pragma unroll
-            for (int i = 0; i < VEC; ++i) { sn[i] = (j == i) ? s1 : sn[i]; cs[i] = (j == i) ? c1 : cs[i]; }
-            neg = (neg & ~(1u << j)) | ((w[2] >> 31) << j);
-            tries += 1u << (8 * j);
-            if (ok || n == 63u) pend &= ~(1u << j);                                       // cap 64: keep the last proposal (O3)
-        };
-        for (int round = 0; round < P.local_rounds && pend; ++round) retry_one();
-        // Links still rejected after the lane-local rounds (a few %) go to this block's segment of the straggler
-        // queue instead of keeping the whole warp looping for its unluckiest lane; k_hb_stragglers finishes
-        // them (same attempt counters, same arithmetic) right after this kernel.  One atomic per warp on the
-        // block's own counter; links that do not fit in the segment are simply finished here.
-        // the lanes of this warp that exist: every thread of the block reaches this point (no early exits), so the mask is
-        // known from the block size and the warp is re-converged explicitly after the divergent retry rounds
+        for (int i = 0; i < VEC; i += 2) {
+            ulm::HbParams hp[2];
+            if (i + 1 < VEC) ulm::hb_setup2(a[i], a[(i + 1) % VEC], hp[0], hp[1]);        // the per-link constants on pairs of links
+            else hp[0] = ulm::hb_setup(a[i]);
+            float sn[2], cs[2];
+            bool ng[2] = {false, false};
+#pragma unroll
+            for (int j = 0; j < 2 && i + j < VEC; ++j) {
+                uint32_t w[4];
+                ulm::philox4x32_10(site0 + 2u * (i + j), sweep_lo, sweep_hi, c3, P.key0, P.key1, w);
+                bool acc;
+                ulm::hb_block(hp[j], w, sn[j], cs[j], acc, ng[j]);
+                pend |= (acc ? 0u : 1u) << (i + j);
+            }
+            if (i + 1 < VEC)
+                ulm::hb_finish2(ulm::pack2(Sx[i], Sx[(i + 1) % VEC]), ulm::pack2(Sy[i], Sy[(i + 1) % VEC]), ulm::pack2(sn[0], sn[1]),
+                                ulm::pack2(cs[0], cs[1]), ng[0], ng[1], out[i], out[(i + 1) % VEC]);
+            else
+                out[i] = ulm::hb_finish(Sx[i], Sy[i], sn[0], cs[0], ng[0]);
+        }
+        // the lanes of this warp that exist: every thread of the block reaches this point (no early exits), so the mask
+        // is known from the block size
         const int tid_ = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
         const int in_warp = min(32, (int)(blockDim.x * blockDim.y * blockDim.z) - (tid_ & ~31));
         const unsigned wmask = in_warp == 32 ? 0xffffffffu : ((1u << in_warp) - 1u);
-        __syncwarp(wmask);
-        const unsigned lanes = __ballot_sync(wmask, pend != 0u);
-        if (lanes) {
-            const int lane = tid_ & 31;
+        if (__ballot_sync(wmask, pend != 0u)) {                                           // warp-uniform
+            const unsigned lt = (1u << (tid_ & 31)) - 1u;
             const int blk = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
-            int mine = __popc(pend), incl = mine;
+            int off[VEC], total = 0;
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {                                            // inclusive warp prefix sum
-                const int v = __shfl_up_sync(wmask, incl, o);
-                if (lane >= o) incl += v;
+            for (int i = 0; i < VEC; ++i) {                                               // slots: link index major, lane minor
+                const unsigned b = __ballot_sync(wmask, ((pend >> i) & 1u) != 0u);
+                off[i] = total + __popc(b & lt);
+                total += __popc(b);
             }
-            const int last = 31 - __clz(wmask);
-            const int total = __shfl_sync(wmask, incl, last);
             int base = 0;
-            if (lane == last) base = atomicAdd(P.qcount + blk, total);
-            base = __shfl_sync(wmask, base, last);
-            int pos = base + incl - mine;                                                 // slots are handed out contiguously, so every
-#pragma unroll                                                                            // slot below min(count, HB_QSEG) gets written
-            for (int i = 0; i < VEC; ++i)
-                if (((pend >> i) & 1u) && pos < HB_QSEG) {
-                    const uint32_t n = (tries >> (8 * i)) & 0xffu;                        // <= 1 + local_rounds <= 7
-                    P.queue[blk * HB_QSEG + pos] = make_int4((st.e0 + i) | (int)(n << 28), (int)(site0 + 2u * i),
-                                                             __float_as_int(((zero >> i) & 1u) ? 0.0f : Sx[i]), __float_as_int(Sy[i]));
-                    ++pos;
-                    pend &= ~(1u << i);
-                } else if ((pend >> i) & 1u) {
-                    ++pos;
-                }
-            while (pend) retry_one();
-        }
-        if (VEC >= 2) {
+            if ((tid_ & 31) == 0) base = atomicAdd(P.qcount + blk, total);                // one atomic per warp, on the block's own counter
+            base = __shfl_sync(wmask, base, 0);
 #pragma unroll
-            for (int i = 0; i + 1 < VEC; i += 2)
-                ulm::hb_finish2(ulm::pack2(Sx[i], Sx[i + 1]), ulm::pack2(Sy[i], Sy[i + 1]), ulm::pack2(sn[i], sn[i + 1]), ulm::pack2(cs[i], cs[i + 1]),
-                                ((neg >> i) & 1u) != 0, ((neg >> (i + 1)) & 1u) != 0, out[i], out[i + 1]);
-        } else {
-            out[0] = ulm::hb_finish(Sx[0], Sy[0], sn[0], cs[0], (neg & 1u) != 0);
+            for (int i = 0; i < VEC; ++i)
+                if ((pend >> i) & 1u) {
+                    const int pos = base + off[i];
+                    const float sx = ((zero >> i) & 1u) ? 0.0f : Sx[i];
+                    if (pos < HB_QSEG)
+                        P.queue[(size_t)blk * HB_QSEG + pos] = make_int4(st.e0 + i, (int)(site0 + 2u * i), __float_as_int(sx), __float_as_int(Sy[i]));
+                    else                                                                  // segment full (never seen): finish here
+                        out[i] = ulm::hb_straggler_call(sx, Sy[i], P.beta, site0 + 2u * i, sweep_lo, sweep_hi, c3, P.key0, P.key1);
+                }
         }
     }
     if (VEC == 4) *reinterpret_cast<int4*>(own) = make_int4(out[0], out[1 % VEC], out[2 % VEC], out[3 % VEC]);
@@ -356,37 +315,40 @@ __global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_up
     }
 }
 
-// Finishes the heatbath links that k_update<0,...> queued: one thread per entry, attempts n = tries, tries+1, ...
-// with the same Philox counters and the same device functions as the main kernel (so the result does not
-// depend on where a link is finished), until accept or the cap of 64 attempts (O3).
+// Finishes the heatbath links that k_update<0,...> queued: blocks 1, 2, ... of their Philox streams with the same
+// counters and the same device functions as the main kernel (so the result does not depend on where a link is finished),
+// until accept or the cap of 64 attempts (O3).  A thread block takes HB_SPB queue segments and spreads their entries
+// over its threads (prefix sum of the counts), so that every lane has work; it also zeroes the counters for the
+// next heatbath sub-step.
+constexpr int HB_SPB = 8;
 template <bool DEVCTR>
 __global__ void __launch_bounds__(256) k_hb_stragglers(const UpdateArgs P, int mu) {
     const uint32_t c3 = ((uint32_t)P.parity << 2) | (uint32_t)mu;
     const uint32_t sweep_lo = DEVCTR ? __ldg(P.sweep_dev) : P.sweep_lo, sweep_hi = DEVCTR ? __ldg(P.sweep_dev + 1) : P.sweep_hi;
-    {   // one thread per queue slot: grid = qblocks * HB_QSEG / 256 blocks, most of which leave at once
-        const int e = blockIdx.x * blockDim.x + threadIdx.x;
-        const int seg = e / HB_QSEG;
-        const int cnt = seg < P.qblocks ? P.qcount[seg] : 0;                              // a count above HB_QSEG: the rest was finished in place
-        __syncthreads();                                                                  // every thread of the block holds its count:
-        if (e % HB_QSEG == 0 && seg < P.qblocks) P.qcount[seg] = 0;                       // zero it for the next heatbath sub-step
-        if ((e % HB_QSEG) >= cnt) return;
-        const int4 q = P.queue[e];
-        const uint32_t site = (uint32_t)q.y;                                              // all 32 bits: ghost-layer sites of a shard wrap
-        uint32_t n = (uint32_t)q.x >> 28;                                                 // V/2 <= 2^28 elements per array (ul_create)
-        float Sx = __int_as_float(q.z);
-        const float Sy = __int_as_float(q.w);
-        const float k2 = fmaf(Sx, Sx, Sy * Sy);
-        if (k2 == 0.0f) Sx = 1.0f;                                                        // k = 0: alpha = 0 (O1); Sy is 0 then
-        const ulm::HbParams hp = ulm::hb_setup(P.beta * ulm::mufu_sqrt(k2));
-        float sn, cs;
-        uint32_t w[4];
-        for (;;) {
-            ulm::philox4x32_10(site, sweep_lo, sweep_hi, (n << 8) | c3, P.key0, P.key1, w);
-            const bool ok = ulm::hb_attempt(hp, w[0], w[1], sn, cs);
-            if (ok || n == 63u) break;
-            ++n;
-        }
-        P.th[(mu * 2 + P.parity) * P.Vh + (q.x & 0x0fffffff)] = ulm::hb_finish(Sx, Sy, sn, cs, (w[2] >> 31) != 0);
+    __shared__ int pre[HB_SPB + 1];
+    const int seg0 = blockIdx.x * HB_SPB;
+    if (threadIdx.x < HB_SPB) {
+        const int seg = seg0 + threadIdx.x;
+        int cnt = 0;
+        if (seg < P.qblocks) { cnt = min(P.qcount[seg], HB_QSEG); P.qcount[seg] = 0; }  // a count above HB_QSEG: the rest was finished in place
+        pre[threadIdx.x + 1] = cnt;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        pre[0] = 0;
+#pragma unroll
+        for (int j = 1; j <= HB_SPB; ++j) pre[j] += pre[j - 1];
+    }
+    __syncthreads();
+    const int total = pre[HB_SPB];
+    for (int e = threadIdx.x; e < total; e += blockDim.x) {
+        int seg = 0;
+#pragma unroll
+        for (int j = 1; j < HB_SPB; ++j) seg += (e >= pre[j]) ? 1 : 0;
+        const int4 q = P.queue[(size_t)(seg0 + seg) * HB_QSEG + (e - pre[seg])];
+        // q.y = the site index, all 32 bits (ghost-layer sites of a shard wrap); (q.z, q.w) = the staple sum, (0, 0) if k = 0
+        P.th[(mu * 2 + P.parity) * P.Vh + q.x] = ulm::hb_straggler(__int_as_float(q.z), __int_as_float(q.w), P.beta, (uint32_t)q.y,
+                                                                   sweep_lo, sweep_hi, c3, P.key0, P.key1);
     }
 }
 
