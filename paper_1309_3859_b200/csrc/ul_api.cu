@@ -108,7 +108,8 @@ struct ul_ctx {
     int* d_bad = nullptr;
     int4* hb_queue = nullptr; // heatbath straggler queue (library-owned)
     int* hb_qcount = nullptr;
-    int hb_qblocks = 0;
+    int hb_qcap = 0;          // entries per sub-queue
+    int hb_qb = 1;            // thread blocks per sub-queue of k_hb_stragglers (grid = one wave)
     uint32_t* d_sweep = nullptr;      // device copy of the sweep counter for graph replays
     bool d_sweep_stale = true;
     bool use_graphs = false, capturing = false;
@@ -215,7 +216,7 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin = 0
     a.sweep_lo = (uint32_t)(c->sweep & 0xffffffffu); a.sweep_hi = (uint32_t)(c->sweep >> 32); a.sweep_dev = c->d_sweep;
     const dim3 block(c->bx, c->by, 2 * c->bz), grid(c->Nh / c->by, c->Ns / c->bz, n_t);   // by = x2 row PAIRS per block
     a.site_offset = c->site_offset;
-    a.queue = c->hb_queue; a.qcount = c->hb_qcount; a.qblocks = (int)(grid.x * grid.y * grid.z);
+    a.queue = c->hb_queue; a.qcount = c->hb_qcount; a.qcap = c->hb_qcap;
     {
         const double units = c->met_delta * (4294967296.0 / 6.283185307179586476925286766559);
         a.met_delta_bt = units >= 2147483647.0 ? 2147483647 : (int)(units + 0.5);
@@ -225,9 +226,15 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin = 0
     if (e != cudaSuccess) return fail(c, UL_ECUDA, std::string("k_update launch: ") + cudaGetErrorString(e));
     c->launches += 1;
     if (kind == 0) {                                  // finish the links the heatbath kernel queued
-        const int nb = (a.qblocks + ulk::HB_SPB - 1) / ulk::HB_SPB;   // it also zeroes the counters for the next sub-step
-        if (c->capturing) ulk::k_hb_stragglers<true><<<nb, 256, 0, c->stream>>>(a, mu);
-        else ulk::k_hb_stragglers<false><<<nb, 256, 0, c->stream>>>(a, mu);
+        // grid: the sub-queues in use x enough blocks for ~12 % of the launch's links at one entry per thread, at most one wave
+        const long long nblk = (long long)grid.x * grid.y * grid.z;
+        const int nq = nblk < ulk::HB_NQ ? (int)nblk : ulk::HB_NQ;
+        const long long links = nblk * (long long)(block.x * block.y * block.z) * c->vec;
+        long long qb = (links / 8 / nq + 255) / 256;
+        qb = qb < 1 ? 1 : (qb > c->hb_qb ? c->hb_qb : qb);
+        const dim3 sgrid(nq, (unsigned)qb);
+        if (c->capturing) ulk::k_hb_stragglers<true><<<sgrid, 256, 0, c->stream>>>(a, mu);
+        else ulk::k_hb_stragglers<false><<<sgrid, 256, 0, c->stream>>>(a, mu);
         if (cudaGetLastError() != cudaSuccess) return fail(c, UL_ECUDA, "k_hb_stragglers launch");
         c->launches += 1;
     }
@@ -530,12 +537,22 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     if (cudaMalloc(&s, sizeof(double) * (2 * NBLK + 4) + 256) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ENOMEM, "cudaMalloc scratch"); }
     c->scratch = (double*)s;
     c->d_bad = (int*)((char*)s + sizeof(double) * (2 * NBLK + 4));
-    c->hb_qblocks = (c->Nh / c->by) * (c->Ns / c->bz) * c->Nt;    // blocks of an unmasked sub-step
+    // heatbath straggler queue: HB_NQ compact sub-queues, together a quarter of the links of a sub-step (8-12 % are used)
+    c->hb_qcap = (int)(c->Vh / 4 / ulk::HB_NQ);
+    if (c->hb_qcap < 256) c->hb_qcap = 256;
+    {
+        int dev = 0, sms = 148, per_sm = 4;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ulk::k_hb_stragglers<false>, 256, 0) != cudaSuccess || per_sm < 1) per_sm = 4;
+        c->hb_qb = sms * per_sm / ulk::HB_NQ;
+        if (c->hb_qb < 1) c->hb_qb = 1;
+    }
     void* q = nullptr;
-    if (cudaMalloc(&q, (sizeof(int4) * ulk::HB_QSEG + sizeof(int)) * (size_t)c->hb_qblocks) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ENOMEM, "cudaMalloc straggler queue"); }
+    if (cudaMalloc(&q, sizeof(int4) * (size_t)ulk::HB_NQ * c->hb_qcap + sizeof(int) * (ulk::HB_NQ + 1)) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ENOMEM, "cudaMalloc straggler queue"); }
     c->hb_queue = (int4*)q;
-    c->hb_qcount = (int*)(c->hb_queue + (size_t)ulk::HB_QSEG * c->hb_qblocks);
-    if (cudaMemset(c->hb_qcount, 0, sizeof(int) * (size_t)c->hb_qblocks) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ECUDA, "memset straggler counters"); }
+    c->hb_qcount = (int*)(c->hb_queue + (size_t)ulk::HB_NQ * c->hb_qcap);
+    if (cudaMemset(c->hb_qcount, 0, sizeof(int) * (ulk::HB_NQ + 1)) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ECUDA, "memset straggler counters"); }
     c->d_sweep = (uint32_t*)(c->d_bad + 2);
     c->use_graphs = c->V <= (1LL << 21) && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) == cudaSuccess;
     *h = c;

@@ -33,13 +33,13 @@ struct UpdateArgs {
     uint32_t sweep_lo, sweep_hi;
     const uint32_t* sweep_dev;   // DEVCTR kernels (CUDA-graph replays) read the sweep counter from here instead
     int4* queue;          // heatbath stragglers: (element offset in th[mu][parity], site, Sx, Sy), see k_hb_stragglers
-    int* qcount;          // entries queued per block (zeroed before the launch); segment b = queue[b*HB_QSEG ...]
-    int qblocks;          // number of segments
+    int* qcount;          // [HB_NQ] entries in each sub-queue (zero before the launch) + [1] ticket of k_hb_stragglers
+    int qcap;             // capacity of a sub-queue; sub-queue i = queue[i * qcap ...]
     uint32_t site_offset; // added to the local canonical site index in the Philox counter (slab sharding: t0 * Ns^3)
     int met_delta_bt;     // Metropolis proposal half-width delta as a binary angle (0 < delta <= pi -> up to 2^31 - 1)
 };
 
-constexpr int HB_QSEG = 192;   // straggler-queue entries per thread block (expected use 85-120 of 1024 links: both attempts of block 0 rejected)
+constexpr int HB_NQ = 64;      // the straggler queue is striped over HB_NQ compact sub-queues (thread block b appends to sub-queue b % HB_NQ)
 
 // per-thread addressing state
 struct Site {
@@ -237,16 +237,17 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
                 total += __popc(b);
             }
             int base = 0;
-            if ((tid_ & 31) == 0) base = atomicAdd(P.qcount + blk, total);                // one atomic per warp, on the block's own counter
+            const int qi = blk & (HB_NQ - 1);
+            if ((tid_ & 31) == 0) base = atomicAdd(P.qcount + qi, total);                 // one atomic per warp, spread over HB_NQ counters
             base = __shfl_sync(wmask, base, 0);
 #pragma unroll
             for (int i = 0; i < VEC; ++i)
                 if ((pend >> i) & 1u) {
                     const int pos = base + off[i];
                     const float sx = ((zero >> i) & 1u) ? 0.0f : Sx[i];
-                    if (pos < HB_QSEG)
-                        P.queue[(size_t)blk * HB_QSEG + pos] = make_int4(st.e0 + i, (int)(site0 + 2u * i), __float_as_int(sx), __float_as_int(Sy[i]));
-                    else                                                                  // segment full (never seen): finish here
+                    if (pos < P.qcap)
+                        P.queue[(size_t)qi * P.qcap + pos] = make_int4(st.e0 + i, (int)(site0 + 2u * i), __float_as_int(sx), __float_as_int(Sy[i]));
+                    else                                                                  // sub-queue full (never seen): finish here
                         out[i] = ulm::hb_straggler_call(sx, Sy[i], P.beta, site0 + 2u * i, sweep_lo, sweep_hi, c3, P.key0, P.key1);
                 }
         }
@@ -317,38 +318,28 @@ __global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_up
 
 // Finishes the heatbath links that k_update<0,...> queued: blocks 1, 2, ... of their Philox streams with the same
 // counters and the same device functions as the main kernel (so the result does not depend on where a link is finished),
-// until accept or the cap of 64 attempts (O3).  A thread block takes HB_SPB queue segments and spreads their entries
-// over its threads (prefix sum of the counts), so that every lane has work; it also zeroes the counters for the
-// next heatbath sub-step.
-constexpr int HB_SPB = 8;
+// until accept or the cap of 64 attempts (O3).  Grid (HB_NQ, QB): the QB thread blocks of a sub-queue stride over its
+// entries, one entry per thread and step (no shared memory, no barrier: the grid is one wave and every lane has work).
+// The last block to finish zeroes the counters for the next heatbath sub-step.
 template <bool DEVCTR>
 __global__ void __launch_bounds__(256) k_hb_stragglers(const UpdateArgs P, int mu) {
     const uint32_t c3 = ((uint32_t)P.parity << 2) | (uint32_t)mu;
     const uint32_t sweep_lo = DEVCTR ? __ldg(P.sweep_dev) : P.sweep_lo, sweep_hi = DEVCTR ? __ldg(P.sweep_dev + 1) : P.sweep_hi;
-    __shared__ int pre[HB_SPB + 1];
-    const int seg0 = blockIdx.x * HB_SPB;
-    if (threadIdx.x < HB_SPB) {
-        const int seg = seg0 + threadIdx.x;
-        int cnt = 0;
-        if (seg < P.qblocks) { cnt = min(P.qcount[seg], HB_QSEG); P.qcount[seg] = 0; }  // a count above HB_QSEG: the rest was finished in place
-        pre[threadIdx.x + 1] = cnt;
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        pre[0] = 0;
-#pragma unroll
-        for (int j = 1; j <= HB_SPB; ++j) pre[j] += pre[j - 1];
-    }
-    __syncthreads();
-    const int total = pre[HB_SPB];
-    for (int e = threadIdx.x; e < total; e += blockDim.x) {
-        int seg = 0;
-#pragma unroll
-        for (int j = 1; j < HB_SPB; ++j) seg += (e >= pre[j]) ? 1 : 0;
-        const int4 q = P.queue[(size_t)(seg0 + seg) * HB_QSEG + (e - pre[seg])];
+    const int n = min(P.qcount[blockIdx.x], P.qcap);                                      // a count above qcap: the rest was finished in place
+    const int4* q0 = P.queue + (size_t)blockIdx.x * P.qcap;
+    int* own = P.th + (mu * 2 + P.parity) * P.Vh;
+    for (int e = blockIdx.y * blockDim.x + threadIdx.x; e < n; e += gridDim.y * blockDim.x) {
+        const int4 q = q0[e];
         // q.y = the site index, all 32 bits (ghost-layer sites of a shard wrap); (q.z, q.w) = the staple sum, (0, 0) if k = 0
-        P.th[(mu * 2 + P.parity) * P.Vh + q.x] = ulm::hb_straggler(__int_as_float(q.z), __int_as_float(q.w), P.beta, (uint32_t)q.y,
-                                                                   sweep_lo, sweep_hi, c3, P.key0, P.key1);
+        own[q.x] = ulm::hb_straggler(__int_as_float(q.z), __int_as_float(q.w), P.beta, (uint32_t)q.y, sweep_lo, sweep_hi, c3, P.key0, P.key1);
+    }
+    __syncthreads();                                                                      // every thread of the block has read its count
+    if (threadIdx.x == 0) {
+        const int nblk = gridDim.x * gridDim.y;
+        if (atomicAdd(P.qcount + HB_NQ, 1) == nblk - 1) {                                 // the last block: nobody reads the counts any more
+#pragma unroll 1
+            for (int i = 0; i <= HB_NQ; ++i) P.qcount[i] = 0;
+        }
     }
 }
 
