@@ -8,6 +8,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -113,6 +114,7 @@ struct ul_ctx {
     uint32_t* d_sweep = nullptr;      // device copy of the sweep counter for graph replays
     bool d_sweep_stale = true;
     bool use_graphs = false, capturing = false;
+    bool use_pdl = true;      // programmatic dependent launch between the update kernels (UL_NO_PDL=1 turns it off)
     cudaStream_t cap_stream = nullptr;
     std::vector<CachedGraph> graphs;
     uint32_t site_offset = 0; // ul_set_site_offset
@@ -178,14 +180,24 @@ int largest_divisor_le(int n, int cap) {
     return best;
 }
 
+// update kernels are launched with programmatic stream serialization (ul_update.cuh: pdl_wait)
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(const ul_ctx* c, void (*kernel)(KArgs...), dim3 grid, dim3 block, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = c->use_pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
 template <int KIND, int MU>
 cudaError_t launch_update_vec(const ul_ctx* c, const ulk::UpdateArgs& a, dim3 grid, dim3 block) {
     switch (c->vec) {
-        case 4: if (c->capturing) ulk::k_update<KIND, MU, 4, true><<<grid, block, 0, c->stream>>>(a); else ulk::k_update<KIND, MU, 4, false><<<grid, block, 0, c->stream>>>(a); break;
-        case 2: if (c->capturing) ulk::k_update<KIND, MU, 2, true><<<grid, block, 0, c->stream>>>(a); else ulk::k_update<KIND, MU, 2, false><<<grid, block, 0, c->stream>>>(a); break;
-        default: if (c->capturing) ulk::k_update<KIND, MU, 1, true><<<grid, block, 0, c->stream>>>(a); else ulk::k_update<KIND, MU, 1, false><<<grid, block, 0, c->stream>>>(a); break;
+        case 4: return c->capturing ? launch_pdl(c, ulk::k_update<KIND, MU, 4, true>, grid, block, a) : launch_pdl(c, ulk::k_update<KIND, MU, 4, false>, grid, block, a);
+        case 2: return c->capturing ? launch_pdl(c, ulk::k_update<KIND, MU, 2, true>, grid, block, a) : launch_pdl(c, ulk::k_update<KIND, MU, 2, false>, grid, block, a);
+        default: return c->capturing ? launch_pdl(c, ulk::k_update<KIND, MU, 1, true>, grid, block, a) : launch_pdl(c, ulk::k_update<KIND, MU, 1, false>, grid, block, a);
     }
-    return cudaGetLastError();
 }
 template <int KIND>
 cudaError_t launch_update_mu(const ul_ctx* c, int mu, const ulk::UpdateArgs& a, dim3 grid, dim3 block) {
@@ -233,9 +245,9 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin = 0
         long long qb = (links / 8 / nq + 255) / 256;
         qb = qb < 1 ? 1 : (qb > c->hb_qb ? c->hb_qb : qb);
         const dim3 sgrid(nq, (unsigned)qb);
-        if (c->capturing) ulk::k_hb_stragglers<true><<<sgrid, 256, 0, c->stream>>>(a, mu);
-        else ulk::k_hb_stragglers<false><<<sgrid, 256, 0, c->stream>>>(a, mu);
-        if (cudaGetLastError() != cudaSuccess) return fail(c, UL_ECUDA, "k_hb_stragglers launch");
+        const cudaError_t es = c->capturing ? launch_pdl(c, ulk::k_hb_stragglers<true>, sgrid, dim3(256), a, mu)
+                                            : launch_pdl(c, ulk::k_hb_stragglers<false>, sgrid, dim3(256), a, mu);
+        if (es != cudaSuccess) return fail(c, UL_ECUDA, std::string("k_hb_stragglers launch: ") + cudaGetErrorString(es));
         c->launches += 1;
     }
     return UL_OK;
@@ -554,6 +566,7 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     c->hb_qcount = (int*)(c->hb_queue + (size_t)ulk::HB_NQ * c->hb_qcap);
     if (cudaMemset(c->hb_qcount, 0, sizeof(int) * (ulk::HB_NQ + 1)) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ECUDA, "memset straggler counters"); }
     c->d_sweep = (uint32_t*)(c->d_bad + 2);
+    { const char* e = getenv("UL_NO_PDL"); if (e && e[0] == '1') c->use_pdl = false; }
     c->use_graphs = c->V <= (1LL << 21) && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) == cudaSuccess;
     *h = c;
     const int rc = ul_init(c, 1);

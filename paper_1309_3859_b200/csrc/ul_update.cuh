@@ -41,6 +41,12 @@ struct UpdateArgs {
 
 constexpr int HB_NQ = 64;      // the straggler queue is striped over HB_NQ compact sub-queues (thread block b appends to sub-queue b % HB_NQ)
 
+// Programmatic dependent launch (sm_90+): with the launch attribute programmaticStreamSerialization a kernel's blocks are
+// scheduled while the previous kernel of the stream drains; griddepcontrol.wait then blocks until that kernel has completed
+// and its writes are visible.  Without the attribute both are no-ops.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // per-thread addressing state
 struct Site {
     int e0;               // element offset of the thread's own chunk inside one array
@@ -303,6 +309,8 @@ __global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_up
     st.dp[3] = (x3 == Ns - 1) ? -(Ns - 1) * sz : sz;    st.dm[3] = (x3 == 0) ? (Ns - 1) * sz : -sz;
     st.dxp = (h0 + VEC >= Nh) ? VEC - Nh : VEC;
     st.dxm = (h0 == 0) ? Nh - 1 : -1;
+    pdl_launch_dependents();                          // the next launch of the stream may start its own index arithmetic
+    pdl_wait();                                       // ... but nothing is read or written before the previous launch is complete
     float Sx[VEC], Sy[VEC];
     if (KIND != 0) {
         // overrelaxation, Metropolis: the short tail is compiled into both branches (56 registers, 4 blocks per SM)
@@ -325,6 +333,8 @@ template <bool DEVCTR>
 __global__ void __launch_bounds__(256) k_hb_stragglers(const UpdateArgs P, int mu) {
     const uint32_t c3 = ((uint32_t)P.parity << 2) | (uint32_t)mu;
     const uint32_t sweep_lo = DEVCTR ? __ldg(P.sweep_dev) : P.sweep_lo, sweep_hi = DEVCTR ? __ldg(P.sweep_dev + 1) : P.sweep_hi;
+    pdl_launch_dependents();
+    pdl_wait();
     const int n = min(P.qcount[blockIdx.x], P.qcap);                                      // a count above qcap: the rest was finished in place
     const int4* q0 = P.queue + (size_t)blockIdx.x * P.qcap;
     int* own = P.th + (mu * 2 + P.parity) * P.Vh;
