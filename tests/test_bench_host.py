@@ -57,7 +57,7 @@ def test_max_over_ranks_world_size_2_gloo(tmp_path):
 @pytest.mark.timeout(300)
 def test_reference_arm_prints_one_json_line():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1", "--warmup", "0",
-                          "--budget-s", "0.5"], capture_output=True, text=True, timeout=280)
+                          "--sample-ns", "32"], capture_output=True, text=True, timeout=280)
     assert out.returncode == 0, out.stderr
     line = json.loads(out.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["metric"] == "link_updates_per_s" and line["value"] > 0
