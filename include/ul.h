@@ -225,6 +225,14 @@ int ul_polyakov(ul_ctx* h, int multihit, double* mean_P);
  * the partition arithmetic and the exchange over torch.distributed. */
 int ul_set_site_offset(ul_ctx* h, int64_t offset);
 int ul_slab_partial_product(ul_ctx* h, int s_begin, int s_end, void* dev_out);
+/* The last step of row a10 across shards (Eq. 24, Eq. 26): dev_parts[k], k = 0..n_parts-1 in rank
+ * order, are DEVICE buffers double[3][r_max][Ns^3][2] on this context's GPU (the own ul_slab_partial_product and the
+ * copies received from the other ranks; caller-owned); the kernel multiplies them in that order, site by site, and
+ * sums over the lattice and the three directions with the library's fixed two-stage tree (bitwise reproducible):
+ * corr[r_max][2] (HOST) = C(r) of the whole lattice, which ul_read_correlators returns from then on.  r_max is that of
+ * the last measurement.  Synchronises.  UL_ESTATE before any measurement; UL_EINVAL: null pointers, n_parts
+ * outside 1..64. */
+int ul_combine_partial_products(ul_ctx* h, const void* const* dev_parts, int n_parts, double* corr);
 
 /* Results of the last measurement, HOST buffers (any may be NULL):
  * corr[r_max][2]           C(r) = (1/3Ns^3) sum_x sum_mu prod_s [T](x,s,mu,r)       (re, im)

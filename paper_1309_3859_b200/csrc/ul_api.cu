@@ -1164,6 +1164,28 @@ int ul_slab_partial_product(ul_ctx* c, int s_begin, int s_end, void* dev_out) {
     c->launches += 1;
     return UL_OK;
 }
+int ul_combine_partial_products(ul_ctx* c, const void* const* dev_parts, int n_parts, double* corr) {
+    if (!c || !dev_parts || !corr) return fail(c, UL_EINVAL, "null pointer");
+    if (n_parts < 1 || n_parts > ulk::MAX_SHARDS) return fail(c, UL_EINVAL, "need 1 <= n_parts <= 64");
+    if (!c->have) return fail(c, UL_ESTATE, "no measurement yet");
+    ulk::CombinePartsArgs a;
+    a.Vs = c->Vs; a.r_max = c->res_r_max; a.n_parts = n_parts;
+    for (int k = 0; k < n_parts; ++k) {
+        if (!dev_parts[k]) return fail(c, UL_EINVAL, "null partial product");
+        a.part[k] = (const double2*)dev_parts[k];
+    }
+    a.partial = wsp<double>(c, c->ws.partial);                 // >= 2 r_max NBLK doubles (plan_workspace)
+    double* res = wsp<double>(c, c->ws.result);
+    const int R = c->res_r_max;
+    ulk::k_combine_partial_products<<<dim3(NBLK, R), 256, 0, c->stream>>>(a);
+    ulk::k_sum_partials<<<2 * R, 256, 0, c->stream>>>(a.partial, NBLK, res, 1.0 / (3.0 * (double)c->Vs), 0);
+    UL_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    UL_CUDA(c, cudaMemcpyAsync(corr, res, sizeof(double) * 2 * (size_t)R, cudaMemcpyDeviceToHost, c->stream));
+    UL_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->corr.assign(corr, corr + 2 * R);                        // ul_read_correlators now returns the global C(r)
+    return UL_OK;
+}
 int ul_get_launch_count(ul_ctx* c, uint64_t* n) { if (!c || !n) return fail(c, UL_EINVAL, "null pointer"); *n = c->launches; return UL_OK; }
 
 int ul_philox_selftest(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int n) {

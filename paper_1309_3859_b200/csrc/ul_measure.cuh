@@ -702,6 +702,35 @@ __global__ void __launch_bounds__(256) k_slab_partial_product(const WeightArgs P
     P.W[idx] = run;
 }
 
+// The shards' partial products multiplied in rank order and summed over the lattice and the three directions: the last
+// step of row a10 for a t-partitioned lattice (Eq. 24, Eq. 26).  part[k] = shard k's
+// [mu][r][xs] array (k_slab_partial_product; the own one or a copy received from rank k).  Grid (blocks, r_max);
+// partial[(2*(r-1) + reim)*gridDim.x + b], the layout k_sum_partials reads: a fixed two-stage tree.
+constexpr int MAX_SHARDS = 64;
+struct CombinePartsArgs {
+    long long Vs;
+    int r_max, n_parts;
+    const double2* part[MAX_SHARDS];
+    double* partial;
+};
+__global__ void __launch_bounds__(256) k_combine_partial_products(const CombinePartsArgs P) {
+    __shared__ double sm[2 * 32];
+    const int r1 = blockIdx.y;
+    double v[2] = {0.0, 0.0};
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < 3 * P.Vs; j += (long long)gridDim.x * blockDim.x) {
+        const int mu1 = (int)(j / P.Vs);
+        const long long idx = ((long long)mu1 * P.r_max + r1) * P.Vs + (j - (long long)mu1 * P.Vs);
+        double2 pp = P.part[0][idx];
+        for (int k = 1; k < P.n_parts; ++k) pp = cmul(pp, P.part[k][idx]);
+        v[0] += pp.x; v[1] += pp.y;
+    }
+    block_sum<2>(v, sm);
+    if (threadIdx.x == 0) {
+        P.partial[(long long)(2 * r1) * gridDim.x + blockIdx.x] = v[0];
+        P.partial[(long long)(2 * r1 + 1) * gridDim.x + blockIdx.x] = v[1];
+    }
+}
+
 // Two-level replay weights: for the inner slab s = S m + i of outer slab S,
 //   Wc(x,s) = W4(x,S) prod_{i' != i} [T2](x, S m + i'),  W4(x,S) = prod_{S' != S} [T4](x,S')   (Eqs. 32-34 with the TO term
 // factored out: G is linear in O), [T2] = A2 * inv (inner sums of THIS outer iteration).  One thread per (mu, r, xs).

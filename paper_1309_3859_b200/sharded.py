@@ -11,8 +11,9 @@ rest of the lattice"), so the lattice is cut in t into shards of whole slabs, on
     reproduces the unsharded trajectory of the own layers bit for bit (tested on one GPU, shard after shard);
   * the sub-update loop (masked sweeps + accumulation) needs NO communication;
   * one exchange per measurement: every rank forms prod_{own slabs} [T](x,s) on its device
-    (ul_slab_partial_product) and the ranks all-gather these arrays (torch.distributed: NCCL on GPUs, gloo in the
-    CPU tests), multiply them in rank order and average over the lattice: row a10, Eq. 24.
+    (ul_slab_partial_product), the ranks all-gather these arrays (torch.distributed: NCCL on GPUs, gloo in the CPU
+    tests) and ul_combine_partial_products multiplies them in rank order and averages over the lattice on the GPU:
+    row a10, Eq. 24.
 
 This module holds the partition arithmetic and that exchange; every arithmetic step of the method still runs in
 the CUDA kernels.  Full (unmasked) sweeps exchange one halo of the written array per sub-step:
@@ -60,23 +61,17 @@ def unshard_links(shards, parts):
     return np.concatenate([s[:, :n] for s, (_, n) in zip(shards, parts)], axis=1)
 
 
-def combine_partial_products(local, dist=None, gathered=None):
-    """local: complex128 tensor [3][r_max][Ns^3] = product of the own slab averages.  All-gathers over the ranks
-    (or takes `gathered`, the list in rank order, when the caller already holds it), multiplies in rank order
-    and returns (C(r) = lattice and direction average, Eq. 26, as a numpy array; the full product)."""
+def gather_partial_products(local, dist=None):
+    """local: complex128 tensor [3][r_max][Ns^3] = product of the own slab averages (ul_slab_partial_product).  All-gathers
+    it over the ranks and returns the list in rank order: bytes only; the ordered product and the lattice average
+    (row a10, Eq. 24, Eq. 26) run in the library (ul_combine_partial_products)."""
     import torch
-    if gathered is None:
-        if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
-            parts = [torch.empty_like(local) for _ in range(dist.get_world_size())]
-            re = [torch.view_as_real(p) for p in parts]                    # collectives on real views: every backend has them
-            dist.all_gather(re, torch.view_as_real(local.contiguous()))
-            gathered = parts
-        else:
-            gathered = [local]
-    full = gathered[0].clone()
-    for p in gathered[1:]:
-        full = full * p
-    return full.mean(dim=(0, 2)).cpu().numpy(), full
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return [local]
+    parts = [torch.empty_like(local) for _ in range(dist.get_world_size())]
+    re = [torch.view_as_real(p) for p in parts]                            # collectives on real views: every backend has them
+    dist.all_gather(re, torch.view_as_real(local.contiguous()))
+    return parts
 
 
 class ShardedLattice:
@@ -104,8 +99,15 @@ class ShardedLattice:
     def partial_product(self):
         return self.lat.slab_partial_product(0, self.nt_loc // self.d)
 
-    def correlators(self, dist=None):
-        return combine_partial_products(self.partial_product(), dist)[0]
+    def correlators(self, dist=None, stage_on_host=False):
+        """The global C(r).  stage_on_host: the all-gather runs on host copies (a process group without a GPU backend,
+        e.g. gloo with several ranks on one device); the product and the reduction still run on the GPU."""
+        local = self.partial_product()
+        if stage_on_host:
+            parts = [p.to(local.device) for p in gather_partial_products(local.cpu(), dist)]
+        else:
+            parts = gather_partial_products(local, dist)
+        return self.lat.combine_partial_products(parts)
 
     def own_links(self):
         return self.lat.get_links()[:, : self.nt_loc]
@@ -194,22 +196,35 @@ def internal_view(lat):
     return lat.links.view(torch.int32).view(8, lat.Nt, -1)
 
 
-def exchange_halos(view, arr, nt_loc, dist, rank, world):
-    """After a sub-step wrote array `arr`: send the first / last GL own layers down / up, receive the neighbours'."""
+def exchange_halos(view, arr, nt_loc, dist, rank, world, stage_on_host=False):
+    """After a sub-step wrote array `arr`: send the first / last GL own layers down / up, receive the neighbours'.
+    The operations are ordered after the kernels by the stream (NCCL enqueues behind torch's current stream, which is the
+    lattice's stream: no host synchronisation); stage_on_host: through host copies, for a process group without a GPU
+    backend (gloo with several ranks on one device)."""
     send_dn, send_up, recv_lo, recv_hi = halo_ranges(nt_loc)
     dn, up = (rank - 1) % world, (rank + 1) % world
-    ops = [dist.P2POp(dist.isend, view[arr, send_dn[0]:send_dn[1]], dn), dist.P2POp(dist.isend, view[arr, send_up[0]:send_up[1]], up),
-           dist.P2POp(dist.irecv, view[arr, recv_hi[0]:recv_hi[1]], up), dist.P2POp(dist.irecv, view[arr, recv_lo[0]:recv_lo[1]], dn)]
+    s_dn, s_up = view[arr, send_dn[0]:send_dn[1]], view[arr, send_up[0]:send_up[1]]
+    r_hi, r_lo = view[arr, recv_hi[0]:recv_hi[1]], view[arr, recv_lo[0]:recv_lo[1]]
+    if stage_on_host:
+        import torch
+        s_dn, s_up = s_dn.cpu(), s_up.cpu()                                # (synchronises with the stream)
+        r_hi, r_lo = torch.empty_like(s_dn), torch.empty_like(s_up)
+    ops = [dist.P2POp(dist.isend, s_dn, dn), dist.P2POp(dist.isend, s_up, up),
+           dist.P2POp(dist.irecv, r_hi, up), dist.P2POp(dist.irecv, r_lo, dn)]
     for req in dist.batch_isend_irecv(ops):
         req.wait()
+    if stage_on_host:
+        view[arr, recv_hi[0]:recv_hi[1]].copy_(r_hi)
+        view[arr, recv_lo[0]:recv_lo[1]].copy_(r_lo)
 
 
 class ShardedSweeper:
     """Full sweeps of one lattice cut in t.  `group`: None under torch.distributed (one shard per process), or the list
     of all shards when they live in one process (shard-after-shard emulation on one GPU: the exchange is then a copy)."""
 
-    def __init__(self, Ns, Nt, beta, seed, rank, world, links, counter=0, device="cuda:0"):
+    def __init__(self, Ns, Nt, beta, seed, rank, world, links, counter=0, device="cuda:0", stage_on_host=False):
         from . import ul
+        self.stage_on_host = stage_on_host
         if Nt % world or (Nt // world) % 2:
             raise ValueError("Nt / world must be an even number of layers")
         self.nt_loc, self.rank, self.world = Nt // world, rank, world
@@ -237,8 +252,7 @@ def sharded_sweep(shards, n_hb, n_or, dist=None):
                     arr = 2 * mu + parity
                     if dist is not None:
                         sh = shards[0]
-                        sh.lat.sync()
-                        exchange_halos(sh.view, arr, sh.nt_loc, dist, sh.rank, sh.world)
+                        exchange_halos(sh.view, arr, sh.nt_loc, dist, sh.rank, sh.world, sh.stage_on_host)
                     else:
                         n = shards[0].nt_loc
                         send_dn, send_up, recv_lo, recv_hi = halo_ranges(n)

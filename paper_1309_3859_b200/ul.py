@@ -19,7 +19,7 @@ SYMBOLS = [
     "ul_create", "ul_create_ext", "ul_workspace_bytes", "ul_destroy", "ul_init", "ul_set_beta",
     "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep", "ul_substep_slabs", "ul_set_slab_group",
     "ul_set_subupdate", "ul_set_update_algorithm", "ul_multilevel", "ul_multilevel_replay", "ul_workspace_bytes_replay", "ul_multilevel2_replay", "ul_workspace_bytes_replay2", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
-    "ul_measure_end", "ul_measure2_begin", "ul_combine", "ul_measure2_end", "ul_set_accum_batch", "ul_set_multihit", "ul_plaquette", "ul_polyakov", "ul_set_site_offset", "ul_slab_partial_product", "ul_read_correlators", "ul_read_slab_averages",
+    "ul_measure_end", "ul_measure2_begin", "ul_combine", "ul_measure2_end", "ul_set_accum_batch", "ul_set_multihit", "ul_plaquette", "ul_polyakov", "ul_set_site_offset", "ul_slab_partial_product", "ul_combine_partial_products", "ul_read_correlators", "ul_read_slab_averages",
     "ul_get_launch_count", "ul_philox_selftest", "ul_sync", "ul_last_error",
 ]
 
@@ -75,6 +75,7 @@ def lib():
         L.ul_polyakov.argtypes = [P, C.c_int, P]
         L.ul_set_site_offset.argtypes = [P, C.c_int64]
         L.ul_slab_partial_product.argtypes = [P, C.c_int, C.c_int, P]
+        L.ul_combine_partial_products.argtypes = [P, P, C.c_int, P]
         L.ul_accumulate.argtypes = [P]
         L.ul_measure_end.argtypes = [P]
         L.ul_measure2_begin.argtypes = [P, C.c_int, C.c_int, C.c_int, P, C.c_int]
@@ -313,6 +314,19 @@ class Lattice:
         self._ck(lib().ul_slab_partial_product(self._h, int(s_begin), int(s_end), C.c_void_p(out.data_ptr())))
         self.sync()
         return out
+
+    def combine_partial_products(self, parts):
+        """parts: the shards' partial products in rank order (complex128 device tensors [3][r_max][Ns^3] on this GPU).
+        Returns the global C(r) (complex numpy array): ordered product and lattice sum run in the library."""
+        R = self._meas[0]
+        parts = [p.contiguous() for p in parts]
+        for p in parts:
+            if not p.is_cuda or p.dtype != self._torch.complex128 or p.numel() != 3 * R * self.Ns ** 3:
+                raise ValueError("partial products must be complex128 [3][r_max][Ns^3] tensors on the lattice's device")
+        ptrs = (C.c_void_p * len(parts))(*[p.data_ptr() for p in parts])
+        corr = np.empty((R, 2), dtype=np.float64)
+        self._ck(lib().ul_combine_partial_products(self._h, ptrs, len(parts), _ptr(corr)))
+        return corr[:, 0] + 1j * corr[:, 1]
 
     def launch_count(self):
         v = C.c_uint64()

@@ -51,11 +51,10 @@ T = rng.standard_normal((3, 4, 6, 64)) + 1j * rng.standard_normal((3, 4, 6, 64))
 parts = sharded.partition(12, 2, 2)                  # 6 slabs of thickness 2 -> 3 + 3
 s0 = parts[r][0] // 2
 local = torch.from_numpy(np.prod(T[:, :, s0:s0 + parts[r][1] // 2], axis=2))
-C, full = sharded.combine_partial_products(local, dist)
-want = np.prod(T, axis=2)
-ok = np.allclose(full.numpy(), want, rtol=1e-13) and np.allclose(C, want.mean(axis=(0, 2)), rtol=1e-13)
+got = sharded.gather_partial_products(local, dist)      # bytes only: the ordered product itself runs in libul (GPU tests)
+ok = len(got) == 2 and all(np.array_equal(got[k].numpy(), np.prod(T[:, :, 3 * k:3 * k + 3], axis=2)) for k in range(2))
 dist.barrier()
-print("RESULT", r, bool(ok), C.shape)
+print("RESULT", r, bool(ok), tuple(got[0].shape))
 dist.destroy_process_group()
 """
 
@@ -72,7 +71,7 @@ def test_exchange_world_size_2_gloo(tmp_path):
     assert all(p.returncode == 0 for p in procs), outs
     for r in range(2):
         line = [l for l in outs[r][0].splitlines() if l.startswith("RESULT")][0]
-        assert line == f"RESULT {r} True (4,)", line
+        assert line == f"RESULT {r} True (3, 4, 64)", line
 
 
 def test_halo_ranges_and_shard_with_halo():
