@@ -114,6 +114,8 @@ struct ul_ctx {
     uint32_t* d_sweep = nullptr;      // device copy of the sweep counter for graph replays
     bool d_sweep_stale = true;
     bool use_graphs = false, capturing = false;
+    int zflip = 0;            // alternates per sub-step launch (UpdateArgs::zflip)
+    bool zflip_on = true;     // UL_NO_ZFLIP=1 turns the alternation off
     bool use_pdl = true;      // programmatic dependent launch between the update kernels (UL_NO_PDL=1 turns it off)
     cudaStream_t cap_stream = nullptr;
     std::vector<CachedGraph> graphs;
@@ -222,6 +224,7 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin = 0
     if (n_t == 0) return UL_OK;                       // thickness 1: every spatial link is frozen
     ulk::UpdateArgs a;
     a.z0 = z0;
+    a.zflip = c->zflip_on ? (c->zflip ^= 1) : 0;
     a.th = c->th; a.Vh = (int)c->Vh; a.Ns = c->Ns; a.Nh = c->Nh; a.Nt = c->Nt;
     a.parity = parity; a.slab_d = slab_d; a.beta = (float)c->beta;
     a.key0 = (uint32_t)(c->seed & 0xffffffffu); a.key1 = (uint32_t)(c->seed >> 32);
@@ -566,6 +569,7 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     c->hb_qcount = (int*)(c->hb_queue + (size_t)ulk::HB_NQ * c->hb_qcap);
     if (cudaMemset(c->hb_qcount, 0, sizeof(int) * (ulk::HB_NQ + 1)) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ECUDA, "memset straggler counters"); }
     c->d_sweep = (uint32_t*)(c->d_bad + 2);
+    { const char* e = getenv("UL_NO_ZFLIP"); if (e && e[0] == '1') c->zflip_on = false; }
     { const char* e = getenv("UL_NO_PDL"); if (e && e[0] == '1') c->use_pdl = false; }
     c->use_graphs = c->V <= (1LL << 21) && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) == cudaSuccess;
     *h = c;

@@ -28,6 +28,9 @@ struct UpdateArgs {
     int slab_d;           // 0 = unmasked; else spatial links with t % slab_d == 0 are frozen
     int z0;               // first time layer of the launch (blockIdx.z + z0; for a masked spatial direction in units of
                           // the enumerated non-frozen layers): launches restricted to a range of slabs
+    int zflip;            // 1: the launch walks through its time layers from the last to the first (blocks are scheduled in
+                          // grid order, so alternating the direction from sub-step to sub-step starts every sub-step on the
+                          // layers the previous one left in L2; the result does not depend on the block order)
     float beta;
     uint32_t key0, key1;  // Philox key = seed
     uint32_t sweep_lo, sweep_hi;
@@ -291,7 +294,7 @@ __global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_up
     const int bz = blockDim.z >> 1;
     const int sel = threadIdx.z >= bz ? 1 : 0;
     const int x3 = blockIdx.y * bz + (threadIdx.z - sel * bz);
-    int t = blockIdx.z + P.z0;
+    int t = (P.zflip ? gridDim.z - 1 - blockIdx.z : blockIdx.z) + P.z0;
     if (MU != 0 && P.slab_d > 0) {                    // enumerate only the non-frozen layers
         const int dm = P.slab_d - 1;
         const int s = t / dm;
