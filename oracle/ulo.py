@@ -15,14 +15,18 @@ _SRC = [os.path.join(_HERE, "ulo.cpp"), os.path.join(_HERE, "ulo.h")]
 
 
 def build(force=False):
-    """Compile oracle/ulo.cpp with g++ (plain -O2, no fast-math, single thread)."""
-    if not force and os.path.exists(_SO) and all(os.path.getmtime(_SO) >= os.path.getmtime(s) for s in _SRC):
-        return _SO
-    cmd = ["g++", "-std=c++17", "-O2", "-fPIC", "-shared", "-fno-fast-math", "-ffp-contract=off",
-           "-o", _SO + ".tmp", _SRC[0]]
+    """Compile oracle/ulo.cpp with g++ (plain -O2, no fast-math, single thread).  With ULO_SANITIZE=1 in the environment
+    the library is the AddressSanitizer + UndefinedBehaviorSanitizer build instead (tests/test_oracle_sanitizers.py; the
+    process must then be started with LD_PRELOAD=libasan)."""
+    san = os.environ.get("ULO_SANITIZE") == "1"
+    so = _SO.replace(".so", "_san.so") if san else _SO
+    if not force and os.path.exists(so) and all(os.path.getmtime(so) >= os.path.getmtime(s) for s in _SRC):
+        return so
+    flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=all", "-fno-omit-frame-pointer"] if san else ["-O2"]
+    cmd = ["g++", "-std=c++17"] + flags + ["-fPIC", "-shared", "-fno-fast-math", "-ffp-contract=off", "-o", so + ".tmp", _SRC[0]]
     subprocess.run(cmd, check=True, cwd=_HERE)
-    os.replace(_SO + ".tmp", _SO)
-    return _SO
+    os.replace(so + ".tmp", so)
+    return so
 
 
 _lib = None

@@ -6,6 +6,7 @@
 #include "../../include/ul.h"
 
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 
 #include <cstdio>
 #include <cstdlib>
@@ -18,6 +19,12 @@
 #include "ul_update.cuh"
 
 namespace {
+
+// NVTX ranges around the host-side steps (visible in nsys / ncu --nvtx; a no-op without a tool attached)
+struct NvtxRange {
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
 
 constexpr int NBLK = 592;   // blocks of the two-stage reductions: 4 per SM on 148 SMs
 constexpr int TBLK = 8 * NBLK;   // blocks of the slab-table kernel (grid-stride; one partial per block and column)
@@ -214,6 +221,9 @@ cudaError_t launch_update_mu(const ul_ctx* c, int mu, const ulk::UpdateArgs& a, 
 // one sub-step (kind, parity, mu), optionally slab-masked: rows a3-a6
 // s_begin <= s < s_end: the slabs (of thickness slab_d) this launch covers; the whole lattice when slab_d = 0
 int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin = 0, int s_end = -1) {
+    static const char* const names[2][3] = {{"ul:hb_substep", "ul:or_substep", "ul:metropolis_substep"},
+                                            {"ul:hb_substep_masked", "ul:or_substep_masked", "ul:metropolis_substep_masked"}};
+    NvtxRange range(names[slab_d > 0 ? 1 : 0][kind]);
     int n_t = c->Nt, z0 = 0;
     if (slab_d > 0) {
         if (s_end < 0) s_end = c->Nt / slab_d;
@@ -375,6 +385,7 @@ double* res_vacuum(ul_ctx* c) { return wsp<double>(c, c->ws.result) + 2 * (size_
 // (restricted to the slabs s_begin <= s < s_end when s_end >= 0: slab-group-major order)
 int flush(ul_ctx* c, int s_begin = 0, int s_end = -1) {
     if (c->n_pending == 0) return UL_OK;
+    NvtxRange range("ul:accumulate_batch");
     if (s_end < 0) s_end = c->n_slab;
     const long long n = (long long)(s_end - s_begin) * c->Vs;
     const int nb = (int)((n + 255) / 256);
@@ -442,6 +453,7 @@ int vacuum_pass(ul_ctx* c) {
 // added to the accumulators when it is full, and before anything reads them.  With a slab range (s_end >= 0) only
 // those slabs are tabulated, and the caller counts the configuration and flushes (slab-group-major order).
 int accumulate(ul_ctx* c, int s_begin = 0, int s_end = -1) {
+    NvtxRange range("ul:slab_tables");
     const bool ranged = s_end >= 0;
     if (!ranged) s_end = c->n_slab;
     const long long n = (long long)c->n_slab * c->Vs;
@@ -476,6 +488,7 @@ int accumulate(ul_ctx* c, int s_begin = 0, int s_end = -1) {
 
 // row a10 on accumulators (A, B) with n_slab slabs, scaled by inv; results to the host vectors
 int finish(ul_ctx* c, const double2* A, const double2* B, int n_slab, double inv, double vac_inv) {
+    NvtxRange range("ul:slab_product");
     const int R = c->r_max, F = c->n_fp;
     const int n_entries = R * (1 + 12 * F);
     ulk::ReduceArgs a;
@@ -683,6 +696,7 @@ int ul_set_counter(ul_ctx* c, uint64_t v) { if (!c) return fail(c, UL_EINVAL, "n
 
 int ul_sweep(ul_ctx* c, int n_hb, int n_or) {
     if (!c || n_hb < 0 || n_or < 0) return fail(c, UL_EINVAL, "n_hb, n_or must be >= 0");
+    NvtxRange range("ul_sweep");
     return compound(c, n_hb, n_or, 0);
 }
 int ul_substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
@@ -751,6 +765,7 @@ int ul_measure_end(ul_ctx* c) {
 
 int ul_multilevel(ul_ctx* c, int d, int n_sub, int r_max, const int* fps, int n_fp) {
     if (!c || n_sub < 0) return fail(c, UL_EINVAL, "n_sub must be >= 0");
+    NvtxRange range("ul_multilevel");
     int rc = ul_measure_begin(c, d, r_max, fps, n_fp);
     if (rc) return rc;
     auto bail = [&](int code) { c->open = false; return code; };

@@ -332,8 +332,11 @@ __global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_up
 // until accept or the cap of 64 attempts (O3).  Grid (HB_NQ, QB): the QB thread blocks of a sub-queue stride over its
 // entries, one entry per thread and step (no shared memory, no barrier: the grid is one wave and every lane has work).
 // The last block to finish zeroes the counters for the next heatbath sub-step.
+#ifndef UL_HBS_MINB
+#define UL_HBS_MINB 4
+#endif
 template <bool DEVCTR>
-__global__ void __launch_bounds__(256) k_hb_stragglers(const UpdateArgs P, int mu) {
+__global__ void __launch_bounds__(256, UL_HBS_MINB) k_hb_stragglers(const UpdateArgs P, int mu) {
     const uint32_t c3 = ((uint32_t)P.parity << 2) | (uint32_t)mu;
     const uint32_t sweep_lo = DEVCTR ? __ldg(P.sweep_dev) : P.sweep_lo, sweep_hi = DEVCTR ? __ldg(P.sweep_dev + 1) : P.sweep_hi;
     pdl_launch_dependents();
