@@ -17,6 +17,7 @@
 
 #include "ul_measure.cuh"
 #include "ul_update.cuh"
+#include "ul_persist.cuh"
 
 namespace {
 
@@ -121,6 +122,10 @@ struct ul_ctx {
     uint32_t* d_sweep = nullptr;      // device copy of the sweep counter for graph replays
     bool d_sweep_stale = true;
     bool use_graphs = false, capturing = false;
+    bool use_persist = false; // lattices that live in L2: one cooperative launch per compound sweep (ul_persist.cuh)
+    int pvec = 1, pbx = 1, pby = 1, pbz = 1, pgrid = 0;   // its tile shape and the largest co-resident grid
+    unsigned* d_bar = nullptr; // grid barrier counter
+    unsigned bar_base = 0;
     int zflip = 0;            // alternates per sub-step launch (UpdateArgs::zflip)
     bool zflip_on = true;     // UL_NO_ZFLIP=1 turns the alternation off
     bool use_pdl = true;      // programmatic dependent launch between the update kernels (UL_NO_PDL=1 turns it off)
@@ -287,7 +292,42 @@ int compound_direct(ul_ctx* c, int n_hb, int n_or, int slab_d, int s_begin = 0, 
 // compound sweep (8 (n_hb + n_or) sub-steps, straggler kernels, counter bump) is captured ONCE per recipe into a
 // CUDA graph -- on a side stream, with kernels that read the sweep counter from device memory, so that the graph
 // never changes -- and replayed on the caller's stream.  Same kernels, same arithmetic, same results.
+// One cooperative launch for the whole compound sweep (ul_persist.cuh)
+int compound_persistent(ul_ctx* c, int n_hb, int n_or, int slab_d) {
+    NvtxRange range("ul:compound_sweep_persistent");
+    ulk::PersistArgs a;
+    a.u = ulk::UpdateArgs();
+    a.u.th = c->th; a.u.Vh = (int)c->Vh; a.u.Ns = c->Ns; a.u.Nh = c->Nh; a.u.Nt = c->Nt;
+    a.u.parity = 0; a.u.slab_d = slab_d; a.u.z0 = 0; a.u.zflip = 0; a.u.beta = (float)c->beta;
+    a.u.key0 = (uint32_t)(c->seed & 0xffffffffu); a.u.key1 = (uint32_t)(c->seed >> 32);
+    a.u.sweep_lo = (uint32_t)(c->sweep & 0xffffffffu); a.u.sweep_hi = (uint32_t)(c->sweep >> 32); a.u.sweep_dev = nullptr;
+    a.u.queue = nullptr; a.u.qcount = nullptr; a.u.qcap = 0;
+    a.u.site_offset = c->site_offset;
+    {
+        const double units = c->met_delta * (4294967296.0 / 6.283185307179586476925286766559);
+        a.u.met_delta_bt = units >= 2147483647.0 ? 2147483647 : (int)(units + 0.5);
+    }
+    a.n_hb = n_hb; a.n_or = n_or; a.stoch_kind = c->alg == 1 ? 2 : 0;
+    a.gx = c->Nh / c->pby; a.gy = c->Ns / c->pbz;
+    a.nt_time = c->Nt; a.nt_space = slab_d > 0 ? c->Nt / slab_d * (slab_d - 1) : c->Nt;
+    const int tiles = a.gx * a.gy * c->Nt;
+    const int grid = tiles < c->pgrid ? tiles : c->pgrid;
+    a.bar = c->d_bar; a.bar_base = c->bar_base;
+    const dim3 block(c->pbx, c->pby, 2 * c->pbz);
+    void* args[] = {&a};
+    const void* fn = c->pvec == 4 ? (const void*)ulk::k_sweep_persistent<4> : c->pvec == 2 ? (const void*)ulk::k_sweep_persistent<2>
+                                                                                             : (const void*)ulk::k_sweep_persistent<1>;
+    const cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(grid), block, args, 0, c->stream);
+    if (e != cudaSuccess) return fail(c, UL_ECUDA, std::string("k_sweep_persistent launch: ") + cudaGetErrorString(e));
+    c->bar_base += 8u * (unsigned)(n_hb + n_or);
+    c->sweep += (uint64_t)n_hb;
+    c->d_sweep_stale = true;
+    c->launches += 1;
+    return UL_OK;
+}
+
 int compound(ul_ctx* c, int n_hb, int n_or, int slab_d) {
+    if (c->use_persist && n_hb + n_or > 0) return compound_persistent(c, n_hb, n_or, slab_d);
     if (!c->use_graphs || n_hb + n_or == 0) return compound_direct(c, n_hb, n_or, slab_d);
     GraphKey key{n_hb, n_or, slab_d, c->alg, c->beta, c->met_delta, c->site_offset};
     CachedGraph* g = nullptr;
@@ -585,6 +625,37 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     { const char* e = getenv("UL_NO_ZFLIP"); if (e && e[0] == '1') c->zflip_on = false; }
     { const char* e = getenv("UL_NO_PDL"); if (e && e[0] == '1') c->use_pdl = false; }
     c->use_graphs = c->V <= (1LL << 21) && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) == cudaSuccess;
+    // persistent compound sweeps: tiles with shorter per-thread chains (2 links per thread) than the streaming kernels
+    if (c->V <= (1LL << 21)) {
+        const char* env = getenv("UL_PERSIST_VEC");
+        int pv = env ? atoi(env) : 2;
+        if (pv != 1 && pv != 2 && pv != 4) pv = 2;
+        while (pv > 1 && c->Nh % pv != 0) pv >>= 1;
+        c->pvec = pv; c->pbx = Nh / pv;
+        if (c->pbx <= 128) {
+            c->pby = largest_divisor_le(Nh, 128 / c->pbx);
+            c->pbz = largest_divisor_le(Ns, 128 / (c->pbx * c->pby));
+            int dev = 0, sms = 0, per_sm = 0, coop = 0;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+            const void* fn = pv == 4 ? (const void*)ulk::k_sweep_persistent<4> : pv == 2 ? (const void*)ulk::k_sweep_persistent<2>
+                                                                                         : (const void*)ulk::k_sweep_persistent<1>;
+            const int threads = c->pbx * c->pby * 2 * c->pbz;
+            const long long tiles = (long long)(Nh / c->pby) * (Ns / c->pbz) * Nt;
+            if (coop && tiles <= ulk::PERSIST_MAX_TILES && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, 0) == cudaSuccess && per_sm > 0) {
+                c->pgrid = sms * per_sm;
+                const size_t bar_bytes = 128;
+                void* bp = nullptr;
+                const char* off = getenv("UL_NO_PERSIST");
+                if (!(off && off[0] == '1') && cudaMalloc(&bp, bar_bytes) == cudaSuccess) {
+                    c->d_bar = (unsigned*)bp;
+                    c->use_persist = cudaMemset(c->d_bar, 0, bar_bytes) == cudaSuccess;
+                }
+            }
+            cudaGetLastError();
+        }
+    }
     *h = c;
     const int rc = ul_init(c, 1);
     if (rc) { g_err = c->err; ul_destroy(c); *h = nullptr; }
@@ -626,6 +697,7 @@ int ul_destroy(ul_ctx* c) {
     if (c->plane_buf) cudaFree(c->plane_buf);
     if (c->scratch) cudaFree(c->scratch);
     if (c->hb_queue) cudaFree(c->hb_queue);
+    if (c->d_bar) cudaFree(c->d_bar);
     for (auto& e : c->graphs) if (e.exec) cudaGraphExecDestroy(e.exec);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);

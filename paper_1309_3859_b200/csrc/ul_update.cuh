@@ -58,29 +58,36 @@ struct Site {
     int off;              // x1 = 2h + off
 };
 
+// Global loads of link angles.  COH = false: the read-only path (ld.global.nc), fine when the whole kernel only reads the
+// arrays it does not write (one sub-step per launch).  COH = true: L2-coherent loads (ld.global.cg) for the persistent
+// kernel, where other thread blocks wrote the data earlier in the same launch.
+template <bool COH> __device__ __forceinline__ int4 ld4(const int* p) { return COH ? __ldcg(reinterpret_cast<const int4*>(p)) : __ldg(reinterpret_cast<const int4*>(p)); }
+template <bool COH> __device__ __forceinline__ int2 ld2(const int* p) { return COH ? __ldcg(reinterpret_cast<const int2*>(p)) : __ldg(reinterpret_cast<const int2*>(p)); }
+template <bool COH> __device__ __forceinline__ int ld1(const int* p) { return COH ? __ldcg(p) : __ldg(p); }
+
 // Loads the VEC angles at element offset `idx` shifted by the x1-displacement D1 (-1, 0, +1):
 // x1 + 1 lives at h + off, x1 - 1 at h - 1 + off of the other-parity row.
-template <int VEC, int D1, int OFF>
+template <int VEC, int D1, int OFF, bool COH>
 __device__ __forceinline__ void load_row(const int* __restrict__ th, int idx, const Site& st, int v[VEC]) {
     if (VEC == 4) {
-        const int4 q = __ldg(reinterpret_cast<const int4*>(th + idx));
+        const int4 q = ld4<COH>(th + idx);
         v[0] = q.x; v[1 % VEC] = q.y; v[2 % VEC] = q.z; v[3 % VEC] = q.w;
     } else if (VEC == 2) {
-        const int2 q = __ldg(reinterpret_cast<const int2*>(th + idx));
+        const int2 q = ld2<COH>(th + idx);
         v[0] = q.x; v[1 % VEC] = q.y;
     } else {
-        v[0] = __ldg(th + idx);
+        v[0] = ld1<COH>(th + idx);
     }
     if (D1 > 0) {
         if (OFF) {                                    // shift by +1: need element h0 + VEC
-            const int x = __ldg(th + idx + st.dxp);
+            const int x = ld1<COH>(th + idx + st.dxp);
 #pragma unroll
             for (int i = 0; i < VEC - 1; ++i) v[i] = v[i + 1];
             v[VEC - 1] = x;
         }
     } else if (D1 < 0) {
         if (!OFF) {                                   // shift by -1: need element h0 - 1
-            const int x = __ldg(th + idx + st.dxm);
+            const int x = ld1<COH>(th + idx + st.dxm);
 #pragma unroll
             for (int i = VEC - 1; i > 0; --i) v[i] = v[i - 1];
             v[0] = x;
@@ -92,18 +99,18 @@ __device__ __forceinline__ void load_row(const int* __restrict__ th, int idx, co
 //   S += e^{-i sigma+} + e^{-i sigma-},  -sigma+ = th_nu(x) + th_mu(x+nu) - th_nu(x+mu),
 //                                        -sigma- = th_nu(x+mu-nu) + th_mu(x-nu) - th_nu(x-nu).
 // The phase sums are wrapping int32 adds: exact and already reduced mod 2 pi.
-template <int MU, int NU, int VEC, int OFF>
+template <int MU, int NU, int VEC, int OFF, bool COH>
 __device__ __forceinline__ void staple_pair(const int* __restrict__ th, int Vh, int p, const Site& st,
                                             float Sx[VEC], float Sy[VEC]) {
     constexpr int m1 = (MU == 1), n1 = (NU == 1);
     const int a_nu_p = (NU * 2 + p) * Vh, a_nu_q = (NU * 2 + 1 - p) * Vh, a_mu_q = (MU * 2 + 1 - p) * Vh;
     int A[VEC], B[VEC], C[VEC], D[VEC], E[VEC], F[VEC];
-    load_row<VEC, 0, OFF>(th, a_nu_p + st.e0, st, A);                                   // theta_nu(x)
-    load_row<VEC, n1, OFF>(th, a_mu_q + st.e0 + st.dp[NU], st, B);                      // theta_mu(x+nu)
-    load_row<VEC, m1, OFF>(th, a_nu_q + st.e0 + st.dp[MU], st, C);                      // theta_nu(x+mu)
-    load_row<VEC, m1 - n1, OFF>(th, a_nu_p + st.e0 + st.dp[MU] + st.dm[NU], st, D);     // theta_nu(x+mu-nu)
-    load_row<VEC, -n1, OFF>(th, a_mu_q + st.e0 + st.dm[NU], st, E);                     // theta_mu(x-nu)
-    load_row<VEC, -n1, OFF>(th, a_nu_q + st.e0 + st.dm[NU], st, F);                     // theta_nu(x-nu)
+    load_row<VEC, 0, OFF, COH>(th, a_nu_p + st.e0, st, A);                                   // theta_nu(x)
+    load_row<VEC, n1, OFF, COH>(th, a_mu_q + st.e0 + st.dp[NU], st, B);                      // theta_mu(x+nu)
+    load_row<VEC, m1, OFF, COH>(th, a_nu_q + st.e0 + st.dp[MU], st, C);                      // theta_nu(x+mu)
+    load_row<VEC, m1 - n1, OFF, COH>(th, a_nu_p + st.e0 + st.dp[MU] + st.dm[NU], st, D);     // theta_nu(x+mu-nu)
+    load_row<VEC, -n1, OFF, COH>(th, a_mu_q + st.e0 + st.dm[NU], st, E);                     // theta_mu(x-nu)
+    load_row<VEC, -n1, OFF, COH>(th, a_nu_q + st.e0 + st.dm[NU], st, F);                     // theta_nu(x-nu)
 #if UL_POLY_TRIG && UL_PACKED_TRIG && !defined(UL_DBG_NOTRIG)
     if (VEC >= 2) {                                     // two links per FFMA2 / FMUL2 (bit-identical to the scalar form)
 #pragma unroll
@@ -137,27 +144,27 @@ __device__ __forceinline__ T pick(const T v[VEC], int j) {        // v[j] withou
 // The staple sums of the VEC links of one thread, compiled separately for the two values of the row's
 // offset bit OFF (x1 = 2h + OFF) so that the x1-shifted neighbour rows are selected by register naming at
 // compile time instead of predicated moves.
-template <int MU, int VEC, int OFF>
+template <int MU, int VEC, int OFF, bool COH>
 __device__ __forceinline__ void gather_staples(const UpdateArgs& P, const Site& st, float Sx[VEC], float Sy[VEC]) {
 #pragma unroll
     for (int i = 0; i < VEC; ++i) { Sx[i] = 0.0f; Sy[i] = 0.0f; }
-    staple_pair<MU, (MU + 1) & 3, VEC, OFF>(P.th, P.Vh, P.parity, st, Sx, Sy);
-    staple_pair<MU, (MU + 2) & 3, VEC, OFF>(P.th, P.Vh, P.parity, st, Sx, Sy);
-    staple_pair<MU, (MU + 3) & 3, VEC, OFF>(P.th, P.Vh, P.parity, st, Sx, Sy);
+    staple_pair<MU, (MU + 1) & 3, VEC, OFF, COH>(P.th, P.Vh, P.parity, st, Sx, Sy);
+    staple_pair<MU, (MU + 2) & 3, VEC, OFF, COH>(P.th, P.Vh, P.parity, st, Sx, Sy);
+    staple_pair<MU, (MU + 3) & 3, VEC, OFF, COH>(P.th, P.Vh, P.parity, st, Sx, Sy);
 }
 
 // The update proper from the staple sums.  KIND 0 = heatbath, 1 = overrelaxation.
-template <int KIND, int MU, int VEC>
+template <int KIND, int MU, int VEC, bool COH>
 __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st, const int h0, float Sx[VEC], float Sy[VEC],
-                                             const uint32_t sweep_lo, const uint32_t sweep_hi) {
+                                             const uint32_t sweep_lo, const uint32_t sweep_hi, const int blk) {
     const int p = P.parity;
     int* own = P.th + ((MU * 2 + p) * P.Vh + st.e0);
     int out[VEC];
     if (KIND == 1) {
         int old[VEC];
-        if (VEC == 4) { const int4 q = *reinterpret_cast<const int4*>(own); old[0] = q.x; old[1 % VEC] = q.y; old[2 % VEC] = q.z; old[3 % VEC] = q.w; }
-        else if (VEC == 2) { const int2 q = *reinterpret_cast<const int2*>(own); old[0] = q.x; old[1 % VEC] = q.y; }
-        else old[0] = own[0];
+        if (VEC == 4) { const int4 q = COH ? __ldcg(reinterpret_cast<const int4*>(own)) : *reinterpret_cast<const int4*>(own); old[0] = q.x; old[1 % VEC] = q.y; old[2 % VEC] = q.z; old[3 % VEC] = q.w; }
+        else if (VEC == 2) { const int2 q = COH ? __ldcg(reinterpret_cast<const int2*>(own)) : *reinterpret_cast<const int2*>(own); old[0] = q.x; old[1 % VEC] = q.y; }
+        else old[0] = COH ? __ldcg(own) : own[0];
 #pragma unroll
         for (int i = 0; i < VEC; ++i)                 // overrelaxation (O2): theta' = 2 alpha - theta, exact mod 2 pi
             out[i] = (int)(2u * (unsigned)ulm::atan2_bt(Sy[i], Sx[i]) - (unsigned)old[i]);
@@ -167,9 +174,9 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
         // number of binary-angle units: v delta 2^-23, v = 2^24 u1 - 2^23 odd) the exponent is, without alpha and
         // without cancellation,  beta 2 sin(d/2) [Sy cos(theta + d/2) - Sx sin(theta + d/2)].
         int old[VEC];
-        if (VEC == 4) { const int4 q = *reinterpret_cast<const int4*>(own); old[0] = q.x; old[1 % VEC] = q.y; old[2 % VEC] = q.z; old[3 % VEC] = q.w; }
-        else if (VEC == 2) { const int2 q = *reinterpret_cast<const int2*>(own); old[0] = q.x; old[1 % VEC] = q.y; }
-        else old[0] = own[0];
+        if (VEC == 4) { const int4 q = COH ? __ldcg(reinterpret_cast<const int4*>(own)) : *reinterpret_cast<const int4*>(own); old[0] = q.x; old[1 % VEC] = q.y; old[2 % VEC] = q.z; old[3 % VEC] = q.w; }
+        else if (VEC == 2) { const int2 q = COH ? __ldcg(reinterpret_cast<const int2*>(own)) : *reinterpret_cast<const int2*>(own); old[0] = q.x; old[1 % VEC] = q.y; }
+        else old[0] = COH ? __ldcg(own) : own[0];
         const uint32_t site0 = (uint32_t)((st.e0 - h0) * 2 + 2 * h0 + st.off) + P.site_offset;            // canonical site index
         const uint32_t c3 = (3u << 3) | ((uint32_t)p << 2) | (uint32_t)MU;                // tag 3 = Metropolis, attempt 0
 #pragma unroll
@@ -237,7 +244,6 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
         const unsigned wmask = in_warp == 32 ? 0xffffffffu : ((1u << in_warp) - 1u);
         if (__ballot_sync(wmask, pend != 0u)) {                                           // warp-uniform
             const unsigned lt = (1u << (tid_ & 31)) - 1u;
-            const int blk = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
             int off[VEC], total = 0;
 #pragma unroll
             for (int i = 0; i < VEC; ++i) {                                               // slots: link index major, lane minor
@@ -285,23 +291,24 @@ __global__ void k_set_sweep(uint32_t* sweep, uint32_t lo, uint32_t hi) { sweep[0
 #ifndef UL_OR_MINB
 #define UL_OR_MINB 0   // 0 = unspecified
 #endif
-template <int KIND, int MU, int VEC, bool DEVCTR>
-__global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_update(const UpdateArgs P) {
-    // the sweep counter: a kernel argument (uniform registers), or, for launches replayed from a CUDA graph, device memory
-    const uint32_t sweep_lo = DEVCTR ? __ldg(P.sweep_dev) : P.sweep_lo, sweep_hi = DEVCTR ? __ldg(P.sweep_dev + 1) : P.sweep_hi;
+// One tile (= one thread block's worth) of a sub-step: tile coordinates (tx, ty, tz) of a (gx, gy, ntz) tile grid, blk = the
+// tile's linear index (picks the straggler sub-queue).
+template <int KIND, int MU, int VEC, bool COH, bool PDL>
+__device__ __forceinline__ void update_tile(const UpdateArgs& P, const int tx, const int ty, const int tz, const int ntz, const int blk,
+                                            const uint32_t sweep_lo, const uint32_t sweep_hi) {
     const int Ns = P.Ns, Nh = P.Nh, Nt = P.Nt;
     const int h0 = threadIdx.x * VEC;
     const int bz = blockDim.z >> 1;
     const int sel = threadIdx.z >= bz ? 1 : 0;
-    const int x3 = blockIdx.y * bz + (threadIdx.z - sel * bz);
-    int t = (P.zflip ? gridDim.z - 1 - blockIdx.z : blockIdx.z) + P.z0;
+    const int x3 = ty * bz + (threadIdx.z - sel * bz);
+    int t = (P.zflip ? ntz - 1 - tz : tz) + P.z0;
     if (MU != 0 && P.slab_d > 0) {                    // enumerate only the non-frozen layers
         const int dm = P.slab_d - 1;
         const int s = t / dm;
         t = s * P.slab_d + 1 + (t - s * dm);
     }
     const int p = P.parity;
-    const int x2 = 2 * (blockIdx.x * blockDim.y + threadIdx.y) + ((sel + p + x3 + t) & 1);
+    const int x2 = 2 * (tx * blockDim.y + threadIdx.y) + ((sel + p + x3 + t) & 1);
     const int sy = Nh, sz = Ns * Nh, stt = Ns * Ns * Nh;     // element strides of x2, x3, t
     Site st;
     st.off = sel;                                     // = (p + x2 + x3 + t) & 1: x1 = 2h + off for the links of this thread
@@ -312,19 +319,29 @@ __global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_up
     st.dp[3] = (x3 == Ns - 1) ? -(Ns - 1) * sz : sz;    st.dm[3] = (x3 == 0) ? (Ns - 1) * sz : -sz;
     st.dxp = (h0 + VEC >= Nh) ? VEC - Nh : VEC;
     st.dxm = (h0 == 0) ? Nh - 1 : -1;
-    pdl_launch_dependents();                          // the next launch of the stream may start its own index arithmetic
-    pdl_wait();                                       // ... but nothing is read or written before the previous launch is complete
+    if (PDL) {
+        pdl_launch_dependents();                      // the next launch of the stream may start its own index arithmetic
+        pdl_wait();                                   // ... but nothing is read or written before the previous launch is complete
+    }
     float Sx[VEC], Sy[VEC];
     if (KIND != 0) {
         // overrelaxation, Metropolis: the short tail is compiled into both branches (56 registers, 4 blocks per SM)
-        if (sel) { gather_staples<MU, VEC, 1>(P, st, Sx, Sy); update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy, sweep_lo, sweep_hi); }
-        else { gather_staples<MU, VEC, 0>(P, st, Sx, Sy); update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy, sweep_lo, sweep_hi); }
+        if (sel) { gather_staples<MU, VEC, 1, COH>(P, st, Sx, Sy); update_links<KIND, MU, VEC, COH>(P, st, h0, Sx, Sy, sweep_lo, sweep_hi, blk); }
+        else { gather_staples<MU, VEC, 0, COH>(P, st, Sx, Sy); update_links<KIND, MU, VEC, COH>(P, st, h0, Sx, Sy, sweep_lo, sweep_hi, blk); }
     } else {
         // heatbath: one copy of the sampler after the branch keeps it at 64 registers (4 blocks per SM)
-        if (sel) gather_staples<MU, VEC, 1>(P, st, Sx, Sy);
-        else gather_staples<MU, VEC, 0>(P, st, Sx, Sy);
-        update_links<KIND, MU, VEC>(P, st, h0, Sx, Sy, sweep_lo, sweep_hi);
+        if (sel) gather_staples<MU, VEC, 1, COH>(P, st, Sx, Sy);
+        else gather_staples<MU, VEC, 0, COH>(P, st, Sx, Sy);
+        update_links<KIND, MU, VEC, COH>(P, st, h0, Sx, Sy, sweep_lo, sweep_hi, blk);
     }
+}
+
+template <int KIND, int MU, int VEC, bool DEVCTR>
+__global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_update(const UpdateArgs P) {
+    // the sweep counter: a kernel argument (uniform registers), or, for launches replayed from a CUDA graph, device memory
+    const uint32_t sweep_lo = DEVCTR ? __ldg(P.sweep_dev) : P.sweep_lo, sweep_hi = DEVCTR ? __ldg(P.sweep_dev + 1) : P.sweep_hi;
+    update_tile<KIND, MU, VEC, false, true>(P, blockIdx.x, blockIdx.y, blockIdx.z, gridDim.z, blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z),
+                                            sweep_lo, sweep_hi);
 }
 
 // Finishes the heatbath links that k_update<0,...> queued: blocks 1, 2, ... of their Philox streams with the same

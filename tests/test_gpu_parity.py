@@ -1046,13 +1046,21 @@ def test_slab_sharding_reproduces_the_unsharded_run(ul, ulo, world, alg):
         assert ok, worst
 
 
-def test_graph_replayed_sweeps_equal_directly_launched_substeps(ul):
-    """Lattices of <= 2^21 sites replay their compound sweeps from a CUDA graph whose kernels read the sweep counter
-    from device memory; ul_substep launches the same kernels directly with the counter as an argument.  Both must
-    give the same bits, sweep after sweep, full and slab-masked, heatbath and Metropolis."""
-    Ns, Nt = 8, 8
+@pytest.mark.parametrize("mode,Ns,Nt", [("graph", 8, 8), ("persistent", 8, 8), ("persistent", 24, 8), ("persistent", 6, 4), ("graph", 6, 4)])
+def test_graph_replayed_sweeps_equal_directly_launched_substeps(ul, monkeypatch, mode, Ns, Nt):
+    """Small lattices run a compound sweep as ONE cooperative launch (ul_persist.cuh: resident blocks, grid barriers, L2-coherent
+    loads, block-local straggler queue); lattices of <= 2^21 sites beyond that (and these, with UL_NO_PERSIST=1) replay it
+    from a CUDA graph whose kernels read the sweep counter from device memory; ul_substep launches the same kernels
+    directly with the counter as an argument.  All must give the same bits, sweep after sweep, full and slab-masked,
+    heatbath and Metropolis."""
+    if mode == "graph":
+        monkeypatch.setenv("UL_NO_PERSIST", "1")
     for alg in (0, 1):
         a = ul.Lattice(Ns, Nt, 0.99, 13)
+        n0 = a.launch_count()
+        a.sweep(1, 1)
+        assert (a.launch_count() - n0 == 1) == (mode == "persistent")   # one launch per compound sweep, or 8 + 8 + 8 + 1
+        a.init(1); a.set_counter(0)
         b = ul.Lattice(Ns, Nt, 0.99, 13)
         for L in (a, b):
             L.set_update_algorithm(alg, 1.3)
