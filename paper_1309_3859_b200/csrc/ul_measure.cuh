@@ -474,11 +474,20 @@ __global__ void __launch_bounds__(256, FIELD ? UL_ACCF_MINB : UL_ACC_MINB) k_acc
     for (int mu = 1; mu <= 3; ++mu) {
         const int nu = 1 + (mu % 3), rho = 1 + ((mu + 1) % 3);
         double2* Ap = P.A + (((long long)(mu - 1) * P.r_max + (P.r_begin - 1)) * P.n_slab + s) * g.Vs + xs;
+        // the accumulator entries of the NEXT step are requested before the current ones are worked on (software pipelining:
+        // the kernel is bound by the latency of these reads, not by bandwidth or arithmetic)
+        double2 an[ACC_RB];
+#pragma unroll
+        for (int i = 0; i < ACC_RB; ++i)
+            an[i] = (P.first || P.r_begin + i > P.r_end || P.r_begin + i > P.a_r_max) ? make_double2(0.0, 0.0) : __ldcs(Ap + i * stepA);
         for (int r0 = P.r_begin; r0 <= P.r_end; r0 += ACC_RB) {
             double2 a[ACC_RB];
 #pragma unroll
-            for (int i = 0; i < ACC_RB; ++i)
-                if (r0 + i <= P.r_end) a[i] = (P.first || r0 + i > P.a_r_max) ? make_double2(0.0, 0.0) : __ldcs(Ap + i * stepA);
+            for (int i = 0; i < ACC_RB; ++i) {
+                a[i] = an[i];
+                const int rn = r0 + ACC_RB + i;
+                an[i] = (P.first || rn > P.r_end || rn > P.a_r_max) ? make_double2(0.0, 0.0) : __ldcs(Ap + (ACC_RB + i) * stepA);
+            }
 #pragma unroll
             for (int i = 0; i < ACC_RB; ++i) {
                 const int r = r0 + i;
