@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libul.so")
 SOURCES = ["ul_api.cu"]
-HEADERS = ["ul_math.cuh", "ul_update.cuh", "ul_persist.cuh", "ul_measure.cuh", os.path.join("..", "..", "include", "ul.h")]
+HEADERS = ["ul_math.cuh", "ul_update.cuh", "ul_persist.cuh", "ul_update_tma.cuh", "ul_measure.cuh", os.path.join("..", "..", "include", "ul.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "-ldl"]
 

@@ -18,6 +18,7 @@
 #include "ul_measure.cuh"
 #include "ul_update.cuh"
 #include "ul_persist.cuh"
+#include "ul_update_tma.cuh"
 
 namespace {
 
@@ -128,6 +129,7 @@ struct ul_ctx {
     unsigned bar_base = 0;
     int zflip = 0;            // alternates per sub-step launch (UpdateArgs::zflip)
     bool zflip_on = true;     // UL_NO_ZFLIP=1 turns the alternation off
+    bool or_tma = false, or_tma_attr = false;   // UL_OR_TMA=1: overrelaxation through the bulk-copy staged kernel
     bool use_pdl = true;      // programmatic dependent launch between the update kernels (UL_NO_PDL=1 turns it off)
     cudaStream_t cap_stream = nullptr;
     std::vector<CachedGraph> graphs;
@@ -250,6 +252,27 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin = 0
     {
         const double units = c->met_delta * (4294967296.0 / 6.283185307179586476925286766559);
         a.met_delta_bt = units >= 2147483647.0 ? 2147483647 : (int)(units + 0.5);
+    }
+    if (kind == 1 && c->or_tma && c->vec == 4 && c->bz == 1 && !c->capturing) {       // A/B partner of the direct gather (ul_update_tma.cuh)
+        const size_t smem = (size_t)18 * 2 * c->by * c->Nh * sizeof(int);
+        if (!c->or_tma_attr) {
+            cudaFuncSetAttribute(ulk::k_update_or_tma<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaFuncSetAttribute(ulk::k_update_or_tma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaFuncSetAttribute(ulk::k_update_or_tma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            cudaFuncSetAttribute(ulk::k_update_or_tma<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            c->or_tma_attr = true;
+        }
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr; cfg.numAttrs = c->use_pdl ? 1 : 0;
+        const cudaError_t et = mu == 0 ? cudaLaunchKernelEx(&cfg, ulk::k_update_or_tma<0>, a) : mu == 1 ? cudaLaunchKernelEx(&cfg, ulk::k_update_or_tma<1>, a)
+                             : mu == 2 ? cudaLaunchKernelEx(&cfg, ulk::k_update_or_tma<2>, a) : cudaLaunchKernelEx(&cfg, ulk::k_update_or_tma<3>, a);
+        if (et != cudaSuccess) return fail(c, UL_ECUDA, std::string("k_update_or_tma launch: ") + cudaGetErrorString(et));
+        c->launches += 1;
+        return UL_OK;
     }
     const cudaError_t e = kind == 0 ? launch_update_mu<0>(c, mu, a, grid, block)
                         : kind == 1 ? launch_update_mu<1>(c, mu, a, grid, block) : launch_update_mu<2>(c, mu, a, grid, block);
@@ -623,6 +646,7 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     if (cudaMemset(c->hb_qcount, 0, sizeof(int) * (ulk::HB_NQ + 1)) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ECUDA, "memset straggler counters"); }
     c->d_sweep = (uint32_t*)(c->d_bad + 2);
     { const char* e = getenv("UL_NO_ZFLIP"); if (e && e[0] == '1') c->zflip_on = false; }
+    { const char* e = getenv("UL_OR_TMA"); if (e && e[0] == '1' && 18 * 2 * c->by * c->Nh * 4 <= 200 * 1024) c->or_tma = true; }
     { const char* e = getenv("UL_NO_PDL"); if (e && e[0] == '1') c->use_pdl = false; }
     c->use_graphs = c->V <= (1LL << 21) && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) == cudaSuccess;
     // persistent compound sweeps: tiles with shorter per-thread chains (2 links per thread) than the streaming kernels

@@ -95,22 +95,11 @@ __device__ __forceinline__ void load_row(const int* __restrict__ th, int idx, co
     }
 }
 
-// Adds the two staples of the (MU, NU) plane to S for the VEC links of one thread (row a2):
-//   S += e^{-i sigma+} + e^{-i sigma-},  -sigma+ = th_nu(x) + th_mu(x+nu) - th_nu(x+mu),
-//                                        -sigma- = th_nu(x+mu-nu) + th_mu(x-nu) - th_nu(x-nu).
-// The phase sums are wrapping int32 adds: exact and already reduced mod 2 pi.
-template <int MU, int NU, int VEC, int OFF, bool COH>
-__device__ __forceinline__ void staple_pair(const int* __restrict__ th, int Vh, int p, const Site& st,
-                                            float Sx[VEC], float Sy[VEC]) {
-    constexpr int m1 = (MU == 1), n1 = (NU == 1);
-    const int a_nu_p = (NU * 2 + p) * Vh, a_nu_q = (NU * 2 + 1 - p) * Vh, a_mu_q = (MU * 2 + 1 - p) * Vh;
-    int A[VEC], B[VEC], C[VEC], D[VEC], E[VEC], F[VEC];
-    load_row<VEC, 0, OFF, COH>(th, a_nu_p + st.e0, st, A);                                   // theta_nu(x)
-    load_row<VEC, n1, OFF, COH>(th, a_mu_q + st.e0 + st.dp[NU], st, B);                      // theta_mu(x+nu)
-    load_row<VEC, m1, OFF, COH>(th, a_nu_q + st.e0 + st.dp[MU], st, C);                      // theta_nu(x+mu)
-    load_row<VEC, m1 - n1, OFF, COH>(th, a_nu_p + st.e0 + st.dp[MU] + st.dm[NU], st, D);     // theta_nu(x+mu-nu)
-    load_row<VEC, -n1, OFF, COH>(th, a_mu_q + st.e0 + st.dm[NU], st, E);                     // theta_mu(x-nu)
-    load_row<VEC, -n1, OFF, COH>(th, a_nu_q + st.e0 + st.dm[NU], st, F);                     // theta_nu(x-nu)
+// S += e^{i(A+B-C)} + e^{i(D+E-F)} for the VEC links of one thread: the arithmetic of staple_pair, apart from where the six
+// angles come from (global memory here, shared memory in ul_update_tma.cuh)
+template <int VEC>
+__device__ __forceinline__ void staple_pair_math(const int A[VEC], const int B[VEC], const int C[VEC], const int D[VEC], const int E[VEC],
+                                                 const int F[VEC], float Sx[VEC], float Sy[VEC]) {
 #if UL_POLY_TRIG && UL_PACKED_TRIG && !defined(UL_DBG_NOTRIG)
     if (VEC >= 2) {                                     // two links per FFMA2 / FMUL2 (bit-identical to the scalar form)
 #pragma unroll
@@ -131,6 +120,25 @@ __device__ __forceinline__ void staple_pair(const int* __restrict__ th, int Vh, 
         ulm::cis_pair_accumulate((int)((unsigned)A[i] + (unsigned)B[i] - (unsigned)C[i]),
                                  (int)((unsigned)D[i] + (unsigned)E[i] - (unsigned)F[i]), Sx[i], Sy[i]);
     }
+}
+
+// Adds the two staples of the (MU, NU) plane to S for the VEC links of one thread (row a2):
+//   S += e^{-i sigma+} + e^{-i sigma-},  -sigma+ = th_nu(x) + th_mu(x+nu) - th_nu(x+mu),
+//                                        -sigma- = th_nu(x+mu-nu) + th_mu(x-nu) - th_nu(x-nu).
+// The phase sums are wrapping int32 adds: exact and already reduced mod 2 pi.
+template <int MU, int NU, int VEC, int OFF, bool COH>
+__device__ __forceinline__ void staple_pair(const int* __restrict__ th, int Vh, int p, const Site& st,
+                                            float Sx[VEC], float Sy[VEC]) {
+    constexpr int m1 = (MU == 1), n1 = (NU == 1);
+    const int a_nu_p = (NU * 2 + p) * Vh, a_nu_q = (NU * 2 + 1 - p) * Vh, a_mu_q = (MU * 2 + 1 - p) * Vh;
+    int A[VEC], B[VEC], C[VEC], D[VEC], E[VEC], F[VEC];
+    load_row<VEC, 0, OFF, COH>(th, a_nu_p + st.e0, st, A);                                   // theta_nu(x)
+    load_row<VEC, n1, OFF, COH>(th, a_mu_q + st.e0 + st.dp[NU], st, B);                      // theta_mu(x+nu)
+    load_row<VEC, m1, OFF, COH>(th, a_nu_q + st.e0 + st.dp[MU], st, C);                      // theta_nu(x+mu)
+    load_row<VEC, m1 - n1, OFF, COH>(th, a_nu_p + st.e0 + st.dp[MU] + st.dm[NU], st, D);     // theta_nu(x+mu-nu)
+    load_row<VEC, -n1, OFF, COH>(th, a_mu_q + st.e0 + st.dm[NU], st, E);                     // theta_mu(x-nu)
+    load_row<VEC, -n1, OFF, COH>(th, a_nu_q + st.e0 + st.dm[NU], st, F);                     // theta_nu(x-nu)
+    staple_pair_math<VEC>(A, B, C, D, E, F, Sx, Sy);
 }
 
 template <typename T, int VEC>
