@@ -1091,6 +1091,36 @@ def test_graph_replayed_sweeps_equal_directly_launched_substeps(ul, monkeypatch,
         assert np.array_equal(a.get_links_raw(), b.get_links_raw()) and a.get_counter() == b.get_counter()
 
 
+def test_tma_staged_overrelaxation_equals_direct_gather(ul, ulo, monkeypatch):
+    """The bulk-copy (TMA) staged overrelaxation kernel (UL_OR_TMA=1; ul_update_tma.cuh), the A/B partner of the direct
+    gather: same links bit for bit after full and slab-masked sweeps on a lattice whose tiles have its shape (Ns = 64), and one
+    of its sub-steps against the oracle on every updated link."""
+    Ns, Nt = 64, 4
+    a = ul.Lattice(Ns, Nt, 0.98, 9)
+    monkeypatch.setenv("UL_OR_TMA", "1")
+    b = ul.Lattice(Ns, Nt, 0.98, 9)
+    monkeypatch.delenv("UL_OR_TMA")
+    for L in (a, b):
+        L.sweep(1, 2)
+        for parity in (0, 1):
+            for mu in range(4):
+                L.substep(1, parity, mu, 2)
+    assert b.launch_count() == a.launch_count()
+    assert np.array_equal(a.get_links_raw(), b.get_links_raw())
+    o = ulo.Oracle(Ns, Nt, 0.98, 9)
+    before = b.get_links()
+    o.set_links(before)
+    b.set_links(before)
+    ob = ulo.Oracle(Ns, Nt, 0.98, 1)
+    ob.set_links(before)
+    for parity, mu, d in ((1, 2, 0), (0, 3, 2)):
+        o.substep(1, parity, mu, d)
+        b.substep(1, parity, mu, d)
+    # (two sub-steps in a row: the second starts from the first's output on both sides, overrelaxation has no flips)
+    diff = wrapdiff(b.get_links(), o.get_links())
+    assert (diff > TOL).sum() <= 1e-4 * diff.size and (diff > 1e-3).sum() == 0
+
+
 # ----------------------------------------------------------------------------- multihit inside the two-link operators
 @pytest.mark.parametrize("Ns,Nt,d", [(4, 4, 2), (8, 4, 2), (8, 8, 4), (6, 4, 1)])
 def test_multihit_two_link_against_oracle(ul, ulo, Ns, Nt, d):
