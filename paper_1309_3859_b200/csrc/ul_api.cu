@@ -907,6 +907,8 @@ bool full_plane(const ul_ctx* c, const int* fps, int n_fp, int* a_out) {
     *a_out = fps[0];
     return true;
 }
+// entries per thread of the transverse-DFT kernels: Ns^2 / ept threads per block, at most 1024 (Ns even: Ns^2 % 4 == 0)
+int plane_ept(int N2) { return N2 <= 1024 ? 1 : (N2 <= 2048 ? 2 : 4); }
 // one configuration's W T O reduction into the result sums: k_replay_reduce, or the transverse-DFT route for full planes
 int reduce_fields(ul_ctx* c, const ulk::ReplayArgs& ra, bool plane, int plane_a, int n_entries, double scale) {
     double* res = wsp<double>(c, c->ws.result);
@@ -937,15 +939,30 @@ int reduce_fields(ul_ctx* c, const ulk::ReplayArgs& ra, bool plane, int plane_a,
         static bool attr_set = false;
         if (!attr_set) {
             const int cap = 3 * ulk::PLANE_MAX_NS * ulk::PLANE_MAX_NS * (int)sizeof(double2);
-            cudaFuncSetAttribute(ulk::k_plane_dft_o, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
-            cudaFuncSetAttribute(ulk::k_plane_spectral, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
-            cudaFuncSetAttribute(ulk::k_plane_idft, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+            cudaFuncSetAttribute(ulk::k_plane_dft_o<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+            cudaFuncSetAttribute(ulk::k_plane_dft_o<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+            cudaFuncSetAttribute(ulk::k_plane_dft_o<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+            cudaFuncSetAttribute(ulk::k_plane_spectral<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+            cudaFuncSetAttribute(ulk::k_plane_spectral<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+            cudaFuncSetAttribute(ulk::k_plane_spectral<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+            cudaFuncSetAttribute(ulk::k_plane_idft<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+            cudaFuncSetAttribute(ulk::k_plane_idft<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+            cudaFuncSetAttribute(ulk::k_plane_idft<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
             attr_set = true;
         }
         const long long ne = (long long)R * 12 * N2;
+        const int ept = plane_ept(N2);                                   // entries per thread: Ns^2 / ept <= 1024 threads
         for (int mu = 1; mu <= 3; ++mu) {
-            ulk::k_plane_dft_o<<<dim3(n_planes, 12), N2, smem, c->stream>>>(ra, mu, Oh);
-            ulk::k_plane_spectral<<<dim3(R, groups, 2), N2, smem, c->stream>>>(ra, mu, plane_a, Oh, Ghp);
+            if (ept == 1) {
+                ulk::k_plane_dft_o<1><<<dim3(n_planes, 12), N2, smem, c->stream>>>(ra, mu, Oh);
+                ulk::k_plane_spectral<1><<<dim3(R, groups, 2), N2, smem, c->stream>>>(ra, mu, plane_a, Oh, Ghp);
+            } else if (ept == 2) {
+                ulk::k_plane_dft_o<2><<<dim3(n_planes, 12), N2 / 2, smem, c->stream>>>(ra, mu, Oh);
+                ulk::k_plane_spectral<2><<<dim3(R, groups, 4), N2 / 2, smem, c->stream>>>(ra, mu, plane_a, Oh, Ghp);
+            } else {
+                ulk::k_plane_dft_o<4><<<dim3(n_planes, 12), N2 / 4, smem, c->stream>>>(ra, mu, Oh);
+                ulk::k_plane_spectral<4><<<dim3(R, groups, 12), N2 / 4, smem, c->stream>>>(ra, mu, plane_a, Oh, Ghp);
+            }
             ulk::k_plane_gh_accum<<<(unsigned)((ne + 255) / 256), 256, 0, c->stream>>>(Ghp, groups, ne, Gh);
         }
         c->launches += 9;
@@ -967,7 +984,11 @@ int plane_finish(ul_ctx* c, int r_max) {
     const size_t oh_b = (size_t)12 * n_planes * N2 * 16, ghp_b = (size_t)groups * r_max * 12 * N2 * 16;
     const double2* Gh = (const double2*)(c->plane_buf + align_up(oh_b) + align_up(ghp_b));
     double2* field = (double2*)(wsp<double>(c, c->ws.result) + 2 * r_max);
-    ulk::k_plane_idft<<<dim3(r_max, 12), N2, (size_t)3 * N2 * sizeof(double2), c->stream>>>(Gh, c->Ns, c->plane_scale, field);
+    const size_t smem = (size_t)3 * N2 * sizeof(double2);
+    const int ept = plane_ept(N2);
+    if (ept == 1) ulk::k_plane_idft<1><<<dim3(r_max, 12), N2, smem, c->stream>>>(Gh, c->Ns, c->plane_scale, field);
+    else if (ept == 2) ulk::k_plane_idft<2><<<dim3(r_max, 12), N2 / 2, smem, c->stream>>>(Gh, c->Ns, c->plane_scale, field);
+    else ulk::k_plane_idft<4><<<dim3(r_max, 12), N2 / 4, smem, c->stream>>>(Gh, c->Ns, c->plane_scale, field);
     c->launches += 1;
     c->plane_fresh = true;
     return cudaGetLastError() == cudaSuccess ? UL_OK : fail(c, UL_ECUDA, "k_plane_idft launch");

@@ -839,7 +839,7 @@ __global__ void __launch_bounds__(256) k_replay_reduce(const ReplayArgs P) {
     }
 }
 
-constexpr int PLANE_MAX_NS = 32;   // the DFT route runs one block of Ns^2 threads per plane
+constexpr int PLANE_MAX_NS = 64;   // the DFT route keeps three Ns^2 planes of complex doubles in shared memory (196 KB at Ns = 64)
 
 // ---------------------------------------------------------------- full-plane maps through the transverse DFT
 // When the field points are a FULL transverse plane, fp = b + Ns c <-> offset (a, b, c) with one a (BJ config 4's "full
@@ -848,11 +848,12 @@ constexpr int PLANE_MAX_NS = 32;   // the DFT route runs one block of Ns^2 threa
 // G(b,c) = sum_{p,q} Z(p,q) O(p+b, q+c)  <=>  Ghat(k,l) = Zhat(-k,-l) Ohat(k,l)  with the 2-d DFT over the transverse plane:
 // 2 Ns^3 complex MACs per plane for the transforms instead of Ns^4 per plane and channel for the direct sum.  The DFT is
 // done as two small dense matrix products with the Ns x Ns matrix W[j][k] = e^{-2 pi i jk/Ns} (any Ns, no radix
-// restriction), in fp64, one block of Ns^2 threads per plane (Ns <= 32).  Ohat of the 12 channels of one direction mu is
-// tabulated first (k_plane_dft_o); k_plane_spectral transforms Z = W T of every plane of its group, multiplies with the
-// 12 Ohat planes and keeps 12 complex sums per (k,l) in registers; k_plane_gh_accum adds the groups' partial sums to
-// Ghat; k_plane_idft turns Ghat into the map once per measurement.  Everything is owned by one thread per entry and
-// summed in a fixed order: bitwise reproducible.
+// restriction), in fp64, one thread block per plane whose threads own EPT = 1, 2 or 4 entries each (Ns^2 / EPT <= 1024
+// threads: Ns <= 64).  Ohat of the 12 channels of one direction mu is tabulated first (k_plane_dft_o); k_plane_spectral
+// transforms Z = W T of every plane of its group, multiplies with CHB = 6 / EPT (at least 1) of the 12 Ohat planes and keeps
+// those complex sums per (k,l) in registers; k_plane_gh_accum adds the groups' partial sums to Ghat; k_plane_idft turns
+// Ghat into the map once per measurement.  Everything is owned by one thread per entry and summed in a fixed order:
+// bitwise reproducible.
 __device__ __forceinline__ void dft_matrix_to_smem(double2* Wm, int Ns, bool conjugate) {
     for (int e = threadIdx.x; e < Ns * Ns; e += blockDim.x) {
         const int j = e / Ns, k = e - j * Ns;
@@ -861,28 +862,38 @@ __device__ __forceinline__ void dft_matrix_to_smem(double2* Wm, int Ns, bool con
         Wm[e] = make_double2(cs, conjugate ? sn : -sn);
     }
 }
-// Ahat = M A M for the plane in A (thread e = k*Ns + l); M symmetric; T is scratch.  Returns the thread's own entry.
-__device__ __forceinline__ double2 dft2_entry(const double2* A, double2* T, const double2* M, int Ns) {
-    const int e = threadIdx.x, k = e / Ns, l = e - k * Ns;
-    double2 t = make_double2(0.0, 0.0);
-    for (int p = 0; p < Ns; ++p) {                                       // T[k][l] = sum_p M[k][p] A[p][l]
-        const double2 m = M[k * Ns + p], a = A[p * Ns + l];
-        t.x = fma(m.x, a.x, fma(-m.y, a.y, t.x));
-        t.y = fma(m.x, a.y, fma(m.y, a.x, t.y));
-    }
-    T[e] = t;
-    __syncthreads();
-    double2 r = make_double2(0.0, 0.0);
-    for (int q = 0; q < Ns; ++q) {                                       // R[k][l] = sum_q T[k][q] M[q][l]
-        const double2 a = T[k * Ns + q], m = M[q * Ns + l];
-        r.x = fma(a.x, m.x, fma(-a.y, m.y, r.x));
-        r.y = fma(a.x, m.y, fma(a.y, m.x, r.y));
+// Ahat = M A M for the plane in A; M symmetric; T is scratch.  Thread x owns the entries e = x + i blockDim.x, i < EPT
+// (e = k*Ns + l); their values are returned in r[].
+template <int EPT>
+__device__ __forceinline__ void dft2_entries(const double2* A, double2* T, const double2* M, int Ns, double2 r[EPT]) {
+#pragma unroll
+    for (int i = 0; i < EPT; ++i) {
+        const int e = threadIdx.x + i * blockDim.x, k = e / Ns, l = e - k * Ns;
+        double2 t = make_double2(0.0, 0.0);
+        for (int p = 0; p < Ns; ++p) {                                   // T[k][l] = sum_p M[k][p] A[p][l]
+            const double2 m = M[k * Ns + p], a = A[p * Ns + l];
+            t.x = fma(m.x, a.x, fma(-m.y, a.y, t.x));
+            t.y = fma(m.x, a.y, fma(m.y, a.x, t.y));
+        }
+        T[e] = t;
     }
     __syncthreads();
-    return r;
+#pragma unroll
+    for (int i = 0; i < EPT; ++i) {
+        const int e = threadIdx.x + i * blockDim.x, k = e / Ns, l = e - k * Ns;
+        double2 v = make_double2(0.0, 0.0);
+        for (int q = 0; q < Ns; ++q) {                                   // R[k][l] = sum_q T[k][q] M[q][l]
+            const double2 a = T[k * Ns + q], m = M[q * Ns + l];
+            v.x = fma(a.x, m.x, fma(-a.y, m.y, v.x));
+            v.y = fma(a.x, m.y, fma(a.y, m.x, v.y));
+        }
+        r[i] = v;
+    }
+    __syncthreads();
 }
 
-// Ohat[ch][plane][k*Ns + l] for direction mu; grid (n_planes, 12), block Ns^2, dynamic smem 3 Ns^2 double2
+// Ohat[ch][plane][k*Ns + l] for direction mu; grid (n_planes, 12), block Ns^2 / EPT, dynamic smem 3 Ns^2 double2
+template <int EPT>
 __global__ void __launch_bounds__(1024, 1) k_plane_dft_o(const ReplayArgs P, int mu, double2* __restrict__ Oh) {
     extern __shared__ double2 sh[];
     const Geom& g = P.g;
@@ -897,17 +908,25 @@ __global__ void __launch_bounds__(1024, 1) k_plane_dft_o(const ReplayArgs P, int
     comp_dirs(mu, ch >> 1, pa, pb);
     orient_of(pa, pb, o, sgn);
     dft_matrix_to_smem(Wm, Ns, false);
-    const int e = threadIdx.x, p = e / Ns, q = e - p * Ns;
-    const long long zs = (long long)s * g.Vs + xm * stride[mu] + p * stride[nu] + q * stride[rho];
-    const float v = P.Ot[(long long)(2 * o + (ch & 1)) * n + zs];
-    A[e] = make_double2((double)((ch & 1) ? sgn * v : v), 0.0);
+#pragma unroll
+    for (int i = 0; i < EPT; ++i) {
+        const int e = threadIdx.x + i * blockDim.x, p = e / Ns, q = e - p * Ns;
+        const long long zs = (long long)s * g.Vs + xm * stride[mu] + p * stride[nu] + q * stride[rho];
+        const float v = P.Ot[(long long)(2 * o + (ch & 1)) * n + zs];
+        A[e] = make_double2((double)((ch & 1) ? sgn * v : v), 0.0);
+    }
     __syncthreads();
-    Oh[((long long)ch * gridDim.x + pl) * N2 + e] = dft2_entry(A, T, Wm, Ns);
+    double2 r[EPT];
+    dft2_entries<EPT>(A, T, Wm, Ns, r);
+#pragma unroll
+    for (int i = 0; i < EPT; ++i) Oh[((long long)ch * gridDim.x + pl) * N2 + threadIdx.x + i * blockDim.x] = r[i];
 }
 
 // partial[(group*r_max + r-1)*12 + ch][k*Ns + l] = sum over the planes of the group of Zhat(-k,-l) Ohat_ch(k,l);
-// grid (r_max, groups, 2 channel halves), block Ns^2 (<= 1024 threads: 64 registers each, hence 6 channels per block)
+// grid (r_max, groups, 12 / CHB), block Ns^2 / EPT (<= 1024 threads with 64 registers each: CHB * EPT <= 6 complex sums)
+template <int EPT>
 __global__ void __launch_bounds__(1024, 1) k_plane_spectral(const ReplayArgs P, int mu, int fa, const double2* __restrict__ Oh, double2* __restrict__ Ghp) {
+    constexpr int CHB = EPT >= 4 ? 1 : 6 / EPT;
     extern __shared__ double2 sh[];
     const Geom& g = P.g;
     const int Ns = g.Ns, N2 = Ns * Ns;
@@ -918,31 +937,42 @@ __global__ void __launch_bounds__(1024, 1) k_plane_spectral(const ReplayArgs P, 
     const int r = blockIdx.x + 1, n_planes = P.n_slab * Ns;
     const double2* Wm = P.W + ((long long)(mu - 1) * P.r_max + (r - 1)) * n;
     dft_matrix_to_smem(Wc, Ns, true);                                    // conj(W): Zhat(-k,-l)
-    const int e = threadIdx.x, p = e / Ns, q = e - p * Ns;
-    const int ch0 = 6 * blockIdx.z;
-    double2 acc[6];
+    const int ch0 = CHB * blockIdx.z;
+    double2 acc[CHB][EPT];
 #pragma unroll
-    for (int ch = 0; ch < 6; ++ch) acc[ch] = make_double2(0.0, 0.0);
+    for (int ch = 0; ch < CHB; ++ch)
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) acc[ch][i] = make_double2(0.0, 0.0);
     for (int pl = blockIdx.y; pl < n_planes; pl += gridDim.y) {
         const int s = pl / Ns, xm = pl - s * Ns;
-        const int xs = xm * stride[mu] + p * stride[nu] + q * stride[rho];
-        const int ys = wrapc(xm + r, Ns) * stride[mu] + p * stride[nu] + q * stride[rho];
-        const long long j = (long long)s * g.Vs + xs;
-        const double2 u = P.U[j], v = P.U[(long long)s * g.Vs + ys];
-        const double2 Tj = make_double2(fma(v.x, u.x, v.y * u.y), fma(v.y, u.x, -(v.x * u.y)));
-        A[e] = cmul(Wm[j], Tj);
+#pragma unroll
+        for (int i = 0; i < EPT; ++i) {
+            const int e = threadIdx.x + i * blockDim.x, p = e / Ns, q = e - p * Ns;
+            const int xs = xm * stride[mu] + p * stride[nu] + q * stride[rho];
+            const int ys = wrapc(xm + r, Ns) * stride[mu] + p * stride[nu] + q * stride[rho];
+            const long long j = (long long)s * g.Vs + xs;
+            const double2 u = P.U[j], v = P.U[(long long)s * g.Vs + ys];
+            const double2 Tj = make_double2(fma(v.x, u.x, v.y * u.y), fma(v.y, u.x, -(v.x * u.y)));
+            A[e] = cmul(Wm[j], Tj);
+        }
         __syncthreads();
-        const double2 zh = dft2_entry(A, T, Wc, Ns);
+        double2 zh[EPT];
+        dft2_entries<EPT>(A, T, Wc, Ns, zh);
         const int plo = s * Ns + modc(xm + r / 2 + fa, Ns);              // plane of the plaquettes (anchor, DESIGN R10)
 #pragma unroll
-        for (int ch = 0; ch < 6; ++ch) {
-            const double2 oh = Oh[((long long)(ch0 + ch) * n_planes + plo) * N2 + e];
-            acc[ch].x = fma(zh.x, oh.x, fma(-zh.y, oh.y, acc[ch].x));
-            acc[ch].y = fma(zh.x, oh.y, fma(zh.y, oh.x, acc[ch].y));
-        }
+        for (int ch = 0; ch < CHB; ++ch)
+#pragma unroll
+            for (int i = 0; i < EPT; ++i) {
+                const double2 oh = Oh[((long long)(ch0 + ch) * n_planes + plo) * N2 + threadIdx.x + i * blockDim.x];
+                acc[ch][i].x = fma(zh[i].x, oh.x, fma(-zh[i].y, oh.y, acc[ch][i].x));
+                acc[ch][i].y = fma(zh[i].x, oh.y, fma(zh[i].y, oh.x, acc[ch][i].y));
+            }
     }
 #pragma unroll
-    for (int ch = 0; ch < 6; ++ch) Ghp[(((long long)blockIdx.y * P.r_max + (r - 1)) * 12 + ch0 + ch) * N2 + e] = acc[ch];
+    for (int ch = 0; ch < CHB; ++ch)
+#pragma unroll
+        for (int i = 0; i < EPT; ++i)
+            Ghp[(((long long)blockIdx.y * P.r_max + (r - 1)) * 12 + ch0 + ch) * N2 + threadIdx.x + i * blockDim.x] = acc[ch][i];
 }
 
 // Gh[(r-1)*12 + ch][kl] += sum_groups Ghp[group][...]; one thread per entry
@@ -954,19 +984,25 @@ __global__ void __launch_bounds__(256) k_plane_gh_accum(const double2* __restric
     Gh[i] = a;
 }
 
-// field[((r-1)*Ns^2 + (b + Ns c))*12 + ch] = scale/Ns^2 * sum_{k,l} Gh(k,l) e^{+2 pi i (kb + lc)/Ns}; grid (r_max, 12), block Ns^2
+// field[((r-1)*Ns^2 + (b + Ns c))*12 + ch] = scale/Ns^2 * sum_{k,l} Gh(k,l) e^{+2 pi i (kb + lc)/Ns}; grid (r_max, 12), block Ns^2 / EPT
+template <int EPT>
 __global__ void __launch_bounds__(1024, 1) k_plane_idft(const double2* __restrict__ Gh, int Ns, double scale, double2* __restrict__ field) {
     extern __shared__ double2 sh[];
     const int N2 = Ns * Ns;
     double2 *Wc = sh, *A = sh + N2, *T = sh + 2 * N2;
-    const int r1 = blockIdx.x, ch = blockIdx.y, e = threadIdx.x;
+    const int r1 = blockIdx.x, ch = blockIdx.y;
     dft_matrix_to_smem(Wc, Ns, true);
-    A[e] = Gh[((long long)r1 * 12 + ch) * N2 + e];
+#pragma unroll
+    for (int i = 0; i < EPT; ++i) A[threadIdx.x + i * blockDim.x] = Gh[((long long)r1 * 12 + ch) * N2 + threadIdx.x + i * blockDim.x];
     __syncthreads();
-    const double2 v = dft2_entry(A, T, Wc, Ns);                          // entry e = b*Ns + c
-    const int b = e / Ns, c = e - b * Ns;
+    double2 v[EPT];
+    dft2_entries<EPT>(A, T, Wc, Ns, v);                                  // entry e = b*Ns + c
     const double f = scale / (double)N2;
-    field[((long long)r1 * N2 + (b + Ns * c)) * 12 + ch] = make_double2(v.x * f, v.y * f);
+#pragma unroll
+    for (int i = 0; i < EPT; ++i) {
+        const int e = threadIdx.x + i * blockDim.x, b = e / Ns, c = e - b * Ns;
+        field[((long long)r1 * N2 + (b + Ns * c)) * 12 + ch] = make_double2(v[i].x * f, v[i].y * f);
+    }
 }
 
 // vacuum[ch] = (1/(3 V n_acc)) sum_mu sgn * colsum[orient(mu, comp)][kind]

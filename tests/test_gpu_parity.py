@@ -997,6 +997,35 @@ def test_replay_full_mid_plane_against_oracle(ul, ulo):
     assert np.all(np.isfinite(g.read_correlators()[1]))
 
 
+@pytest.mark.parametrize("Ns,Nt,R", [(40, 2, 3), (64, 2, 2)])
+def test_full_plane_map_beyond_32_sampled_against_oracle(ul, ulo, Ns, Nt, R):
+    """The transverse-DFT route with several entries per thread (Ns = 40: 2, Ns = 64: 4): the FULL mid-plane map (Ns^2 field
+    points x 12 channels) of a frozen configuration, compared at sampled points with the oracle (whose stored accumulators
+    only fit a few field points at this size) to relative 1e-5, and with the library's generic per-point reduction."""
+    d = 2
+    g = ul.Lattice(Ns, Nt, 1.0, 21)
+    for _ in range(6):
+        g.sweep(1, 3)
+    links = g.get_links()
+    g.set_links(links)
+    full = [(0, b, c) for c in range(Ns) for b in range(Ns)]
+    g.multilevel_replay(d, 0, R, full)
+    cg, fg, vg = g.read_correlators()
+    pick = [(0, 0, 0), (0, 1, 0), (0, Ns - 1, 3), (0, 17, Ns // 2), (0, Ns - 2, Ns - 1)]
+    idx = [b + Ns * c for (_, b, c) in pick]
+    g.multilevel_replay(d, 0, R, pick)                              # generic path (k_replay_reduce): not a full plane
+    _, fg5, _ = g.read_correlators()
+    assert np.abs(fg[:, idx] - fg5).max() <= 1e-11 * max(1.0, np.abs(fg5).max())
+    o = ulo.Oracle(Ns, Nt, 1.0, 21)
+    o.set_links(links)
+    o.multilevel(d, 0, R, pick)
+    co, fo, vo = o.read_correlators()
+    Vs = Ns ** 3
+    for got, want, n in ((cg, co, 3 * Vs), (fg[:, idx], fo, 3 * Vs * Nt), (vg, vo, 3 * Vs * Nt)):
+        ok, worst = rel_ok(got, want, n)
+        assert ok, worst
+
+
 # ----------------------------------------------------------------------------- slab sharding (next row, SURVEY 8(e)(1))
 @pytest.mark.parametrize("world", [2, 4])
 @pytest.mark.parametrize("alg", [0, 1])
