@@ -234,6 +234,24 @@ int ul_slab_partial_product(ul_ctx* h, int s_begin, int s_end, void* dev_out);
  * outside 1..64. */
 int ul_combine_partial_products(ul_ctx* h, const void* const* dev_parts, int n_parts, double* corr);
 
+/* ---- t-sharded FULL sweeps with peer-memory halo writes ---------------------------
+ * A shard of a lattice cut in t holds ghost_layers (even, >= 2) ghost time layers below and above its own layers.  With
+ * the neighbours' link arrays set here -- DEVICE pointers to the internal-layout arrays of the shards below (t - 1 side)
+ * and above, of the same local shape: memory of the same device, or of another device of this process (peer access is
+ * enabled here; NVLink on B200) -- every unmasked sub-step kernel updates the own layers only and stores the first /
+ * last ghost_layers own layers it has just computed ALSO into the neighbours' ghost layers: one fused kernel per
+ * sub-step, no exchange step.  Ordering between neighbours is stream-ordered, without host synchronisation and without
+ * spinning kernels: before a sub-step the stream waits (cuStreamWaitValue32) until both neighbours have reported the
+ * previous sub-step complete; after it, it reports to both (cuStreamWriteValue32 into their flag words).  ul_halo_flags
+ * returns (and zeroes) this context's two flag words; ul_set_halo_peer_flags takes the neighbours' (the pointers their
+ * ul_halo_flags returned) -- without it no waits or reports are issued and the caller orders the shards (e.g. one
+ * stream).  All shards must issue the same sequence of sub-steps.  (NULL, NULL) switches the mode off.
+ * UL_EINVAL: one neighbour missing, odd or too many ghost layers, pointers that are not device memory; UL_ECUDA: no peer
+ * access between the devices; UL_ESTATE: a measurement is open / ul_halo_flags not called before ul_set_halo_peer_flags. */
+int ul_set_halo_peers(ul_ctx* h, void* dn_links, void* up_links, int ghost_layers);
+int ul_halo_flags(ul_ctx* h, void** dev_flags);
+int ul_set_halo_peer_flags(ul_ctx* h, void* dn_flags, void* up_flags);
+
 /* Results of the last measurement, HOST buffers (any may be NULL):
  * corr[r_max][2]           C(r) = (1/3Ns^3) sum_x sum_mu prod_s [T](x,s,mu,r)       (re, im)
  * field[r_max][n_fp][12][2] G(r,fp,ch) of Eq. 34; ch = 2*comp + kind, comp 0..5 = plaquette

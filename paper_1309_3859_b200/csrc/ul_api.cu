@@ -28,6 +28,13 @@ struct NvtxRange {
     ~NvtxRange() { nvtxRangePop(); }
 };
 
+// the entry points run on the context's device, whatever the caller's current device is
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(const ul_ctx* c);
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 constexpr int NBLK = 592;   // blocks of the two-stage reductions: 4 per SM on 148 SMs
 constexpr int TBLK = 8 * NBLK;   // blocks of the slab-table kernel (grid-stride; one partial per block and column)
 
@@ -129,6 +136,14 @@ struct ul_ctx {
     unsigned bar_base = 0;
     int zflip = 0;            // alternates per sub-step launch (UpdateArgs::zflip)
     bool zflip_on = true;     // UL_NO_ZFLIP=1 turns the alternation off
+    int dev = 0;              // the CUDA device of this context (entry points switch to it)
+    // peer-memory halo writes (ul_set_halo_peers): neighbours' link arrays, own-layer range, stream-ordered flags
+    int* peer_dn = nullptr; int* peer_up = nullptr;
+    int halo_gl = 0;
+    uint32_t* halo_flags = nullptr;      // [0]: sub-steps the shard below has completed, [1]: the shard above (written by them)
+    uint32_t* peer_flag_dn = nullptr;    // where this shard reports to the shard below (its flags[1]) / above (its flags[0])
+    uint32_t* peer_flag_up = nullptr;
+    uint32_t halo_seq = 0;               // sub-steps completed since the peers were set
     bool or_tma = false, or_tma_attr = false;   // UL_OR_TMA=1: overrelaxation through the bulk-copy staged kernel
     bool use_pdl = true;      // programmatic dependent launch between the update kernels (UL_NO_PDL=1 turns it off)
     cudaStream_t cap_stream = nullptr;
@@ -153,6 +168,7 @@ struct ul_ctx {
     char* plane_buf = nullptr; // full-plane maps through the transverse DFT: Ohat, group partials, Ghat (library-owned)
     size_t plane_bytes = 0;
     bool plane_fresh = true;   // Ghat holds nothing yet
+    bool plane_attr_set = false; // shared-memory limits of the plane kernels raised (per context: the attribute is per device)
     double plane_scale = 0.0;
     int plane_r_max = 0;
     bool replay = false;     // ul_multilevel_replay in progress: no TO sums, fields reduced on the fly in pass 2
@@ -168,6 +184,11 @@ struct ul_ctx {
 };
 
 namespace {
+
+DeviceGuard::DeviceGuard(const ul_ctx* c) {
+    int cur = -1;
+    if (c && cudaGetDevice(&cur) == cudaSuccess && cur != c->dev && cudaSetDevice(c->dev) == cudaSuccess) prev = cur;
+}
 
 std::string g_err;   // errors without a handle
 
@@ -225,6 +246,33 @@ cudaError_t launch_update_mu(const ul_ctx* c, int mu, const ulk::UpdateArgs& a, 
     }
 }
 
+// Stream-ordered flags between neighbouring shards (no kernel spins, no host synchronisation): cuStreamWriteValue32 /
+// cuStreamWaitValue32 on words in (peer-mapped) device memory, fetched from the driver at run time (libul.so does not link
+// against libcuda, so it still loads on a machine without a driver).
+typedef int (*StreamMemOp32)(cudaStream_t, unsigned long long, uint32_t, unsigned int);
+StreamMemOp32 stream_memop(const char* name) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult st;
+    if (cudaGetDriverEntryPoint(name, &fn, cudaEnableDefault, &st) != cudaSuccess || st != cudaDriverEntryPointSuccess) return nullptr;
+    return (StreamMemOp32)fn;
+}
+int halo_wait(ul_ctx* c) {
+    static StreamMemOp32 wait32 = stream_memop("cuStreamWaitValue32");
+    if (!wait32) return fail(c, UL_ECUDA, "cuStreamWaitValue32 not available");
+    for (int i = 0; i < 2; ++i)                                    // CU_STREAM_WAIT_VALUE_GEQ = 0
+        if (wait32(c->stream, (unsigned long long)(uintptr_t)(c->halo_flags + i), c->halo_seq, 0u) != 0) return fail(c, UL_ECUDA, "cuStreamWaitValue32");
+    return UL_OK;
+}
+int halo_signal(ul_ctx* c) {
+    static StreamMemOp32 write32 = stream_memop("cuStreamWriteValue32");
+    if (!write32) return fail(c, UL_ECUDA, "cuStreamWriteValue32 not available");
+    c->halo_seq += 1;
+    if (write32(c->stream, (unsigned long long)(uintptr_t)c->peer_flag_dn, c->halo_seq, 0u) != 0 ||
+        write32(c->stream, (unsigned long long)(uintptr_t)c->peer_flag_up, c->halo_seq, 0u) != 0)
+        return fail(c, UL_ECUDA, "cuStreamWriteValue32");
+    return UL_OK;
+}
+
 // one sub-step (kind, parity, mu), optionally slab-masked: rows a3-a6
 // s_begin <= s < s_end: the slabs (of thickness slab_d) this launch covers; the whole lattice when slab_d = 0
 int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin = 0, int s_end = -1) {
@@ -239,8 +287,16 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin = 0
         z0 = s_begin * per;
     }
     if (n_t == 0) return UL_OK;                       // thickness 1: every spatial link is frozen
+    const bool halo = c->peer_dn != nullptr && slab_d == 0;
+    if (halo) { z0 = c->halo_gl; n_t = c->Nt - 2 * c->halo_gl; }   // own layers only: the ghost layers are written by the neighbours
     ulk::UpdateArgs a;
     a.z0 = z0;
+    a.peer_dn = halo ? c->peer_dn : nullptr; a.peer_up = halo ? c->peer_up : nullptr;
+    a.halo_gl = c->halo_gl; a.halo_nt = c->Nt - 2 * c->halo_gl;
+    if (halo && c->peer_flag_dn) {                                // both neighbours have completed the previous sub-step:
+        const int rc = halo_wait(c);                              // their halo writes have landed and they no longer read what this
+        if (rc) return rc;                                        // sub-step is about to overwrite in their ghost layers
+    }
     a.zflip = c->zflip_on ? (c->zflip ^= 1) : 0;
     a.th = c->th; a.Vh = (int)c->Vh; a.Ns = c->Ns; a.Nh = c->Nh; a.Nt = c->Nt;
     a.parity = parity; a.slab_d = slab_d; a.beta = (float)c->beta;
@@ -253,7 +309,7 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin = 0
         const double units = c->met_delta * (4294967296.0 / 6.283185307179586476925286766559);
         a.met_delta_bt = units >= 2147483647.0 ? 2147483647 : (int)(units + 0.5);
     }
-    if (kind == 1 && c->or_tma && c->vec == 4 && c->bz == 1 && !c->capturing) {       // A/B partner of the direct gather (ul_update_tma.cuh)
+    if (kind == 1 && c->or_tma && c->vec == 4 && c->bz == 1 && !c->capturing && !halo) {       // A/B partner of the direct gather (ul_update_tma.cuh)
         const size_t smem = (size_t)18 * 2 * c->by * c->Nh * sizeof(int);
         if (!c->or_tma_attr) {
             cudaFuncSetAttribute(ulk::k_update_or_tma<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -291,6 +347,7 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin = 0
         if (es != cudaSuccess) return fail(c, UL_ECUDA, std::string("k_hb_stragglers launch: ") + cudaGetErrorString(es));
         c->launches += 1;
     }
+    if (halo && c->peer_flag_dn) return halo_signal(c);
     return UL_OK;
 }
 int one_sweep(ul_ctx* c, int kind, int slab_d, int s_begin = 0, int s_end = -1) {      // O5: parity outer, direction inner
@@ -350,6 +407,7 @@ int compound_persistent(ul_ctx* c, int n_hb, int n_or, int slab_d) {
 }
 
 int compound(ul_ctx* c, int n_hb, int n_or, int slab_d) {
+    if (c->peer_dn != nullptr && slab_d == 0) return compound_direct(c, n_hb, n_or, slab_d);   // halo writes: direct launches
     if (c->use_persist && n_hb + n_or > 0) return compound_persistent(c, n_hb, n_or, slab_d);
     if (!c->use_graphs || n_hb + n_or == 0) return compound_direct(c, n_hb, n_or, slab_d);
     GraphKey key{n_hb, n_or, slab_d, c->alg, c->beta, c->met_delta, c->site_offset};
@@ -602,6 +660,7 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(nullptr, UL_ECUDA, "no CUDA device");
     ul_ctx* c = new (std::nothrow) ul_ctx;
     if (!c) return fail(nullptr, UL_ENOMEM, "host allocation failed");
+    cudaGetDevice(&c->dev);
     c->Ns = Ns; c->Nt = Nt; c->Nh = Nh;
     c->Vs = (long long)Ns * Ns * Ns; c->V = c->Vs * Nt; c->Vh = c->V / 2;
     c->beta = beta; c->seed = seed;
@@ -713,6 +772,7 @@ size_t ul_workspace_bytes_replay2(int Ns, int Nt, int d_in, int d_out, int r_max
 }
 int ul_destroy(ul_ctx* c) {
     if (!c) return UL_OK;
+    DeviceGuard guard(c);
     cudaStreamSynchronize(c->stream);
     if (c->own_th && c->th) cudaFree(c->th);
     if (c->own_work && c->work) cudaFree(c->work);
@@ -722,6 +782,7 @@ int ul_destroy(ul_ctx* c) {
     if (c->scratch) cudaFree(c->scratch);
     if (c->hb_queue) cudaFree(c->hb_queue);
     if (c->d_bar) cudaFree(c->d_bar);
+    if (c->halo_flags) cudaFree(c->halo_flags);
     for (auto& e : c->graphs) if (e.exec) cudaGraphExecDestroy(e.exec);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
@@ -731,6 +792,7 @@ int ul_destroy(ul_ctx* c) {
 
 int ul_init(ul_ctx* c, int mode) {
     if (!c || (mode != 0 && mode != 1)) return fail(c, UL_EINVAL, "mode must be 0 or 1");
+    DeviceGuard guard(c);
     if (mode == 0) {
         UL_CUDA(c, cudaMemsetAsync(c->th, 0, sizeof(float) * 4 * (size_t)c->V, c->stream));
         return UL_OK;
@@ -757,6 +819,7 @@ static int ensure_staging(ul_ctx* c) {
 }
 static int links_in(ul_ctx* c, const void* host, int mode) {
     if (!c || !host) return fail(c, UL_EINVAL, "null pointer");
+    DeviceGuard guard(c);
     int rc = ensure_staging(c);
     if (rc) return rc;
     const long long n = 4 * c->V;
@@ -773,6 +836,7 @@ static int links_in(ul_ctx* c, const void* host, int mode) {
 }
 static int links_out(ul_ctx* c, void* host, int mode) {
     if (!c || !host) return fail(c, UL_EINVAL, "null pointer");
+    DeviceGuard guard(c);
     int rc = ensure_staging(c);
     if (rc) return rc;
     const long long n = 4 * c->V;
@@ -792,18 +856,21 @@ int ul_set_counter(ul_ctx* c, uint64_t v) { if (!c) return fail(c, UL_EINVAL, "n
 
 int ul_sweep(ul_ctx* c, int n_hb, int n_or) {
     if (!c || n_hb < 0 || n_or < 0) return fail(c, UL_EINVAL, "n_hb, n_or must be >= 0");
+    DeviceGuard guard(c);
     NvtxRange range("ul_sweep");
     return compound(c, n_hb, n_or, 0);
 }
 int ul_substep(ul_ctx* c, int kind, int parity, int mu, int slab_d) {
     if (!c || kind < 0 || kind > 2 || (parity != 0 && parity != 1) || mu < 0 || mu > 3 || slab_d < 0)
         return fail(c, UL_EINVAL, "bad sub-step arguments");
+    DeviceGuard guard(c);
     if (slab_d > 0 && c->Nt % slab_d != 0) return fail(c, UL_EINVAL, "Nt % slab_d != 0");
     return substep(c, kind, parity, mu, slab_d);
 }
 int ul_substep_slabs(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin, int s_end) {
     if (!c || kind < 0 || kind > 2 || (parity != 0 && parity != 1) || mu < 0 || mu > 3 || slab_d < 1 || c->Nt % slab_d != 0)
         return fail(c, UL_EINVAL, "bad sub-step arguments");
+    DeviceGuard guard(c);
     if (s_begin < 0 || s_begin > s_end || s_end > c->Nt / slab_d) return fail(c, UL_EINVAL, "bad slab range");
     return substep(c, kind, parity, mu, slab_d, s_begin, s_end);
 }
@@ -834,6 +901,7 @@ int ul_set_subupdate(ul_ctx* c, int n_hb, int n_or, int k_sweeps) {
 
 int ul_measure_begin(ul_ctx* c, int d, int r_max, const int* fps, int n_fp) {
     if (!c) return fail(c, UL_EINVAL, "null handle");
+    DeviceGuard guard(c);
     const int rc = check_meas_args(c, d, r_max, fps, n_fp);
     if (rc) return rc;
     return open_measurement(c, d, 0, r_max, fps, n_fp);
@@ -845,6 +913,7 @@ int ul_set_accum_batch(ul_ctx* c, int depth) {
 }
 int ul_accumulate(ul_ctx* c) {
     if (!c) return fail(c, UL_EINVAL, "null handle");
+    DeviceGuard guard(c);
     if (!c->open) return fail(c, UL_ESTATE, "no open measurement");
     const int rc = accumulate(c);
     if (!rc && c->d_out > 0) c->n_inner_acc += 1;
@@ -852,6 +921,7 @@ int ul_accumulate(ul_ctx* c) {
 }
 int ul_measure_end(ul_ctx* c) {
     if (!c) return fail(c, UL_EINVAL, "null handle");
+    DeviceGuard guard(c);
     if (!c->open || c->n_acc == 0 || c->d_out > 0) return fail(c, UL_ESTATE, "nothing accumulated (or a two-level measurement is open)");
     const int rc = flush(c);
     if (rc) return rc;
@@ -861,6 +931,7 @@ int ul_measure_end(ul_ctx* c) {
 
 int ul_multilevel(ul_ctx* c, int d, int n_sub, int r_max, const int* fps, int n_fp) {
     if (!c || n_sub < 0) return fail(c, UL_EINVAL, "n_sub must be >= 0");
+    DeviceGuard guard(c);
     NvtxRange range("ul_multilevel");
     int rc = ul_measure_begin(c, d, r_max, fps, n_fp);
     if (rc) return rc;
@@ -936,8 +1007,7 @@ int reduce_fields(ul_ctx* c, const ulk::ReplayArgs& ra, bool plane, int plane_a,
         if (c->plane_fresh) { UL_CUDA(c, cudaMemsetAsync(Gh, 0, gh_b, c->stream)); c->plane_fresh = false; }
         c->plane_scale = scale; c->plane_r_max = R;
         const size_t smem = (size_t)3 * N2 * sizeof(double2);
-        static bool attr_set = false;
-        if (!attr_set) {
+        if (!c->plane_attr_set) {
             const int cap = 3 * ulk::PLANE_MAX_NS * ulk::PLANE_MAX_NS * (int)sizeof(double2);
             cudaFuncSetAttribute(ulk::k_plane_dft_o<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
             cudaFuncSetAttribute(ulk::k_plane_dft_o<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
@@ -948,7 +1018,7 @@ int reduce_fields(ul_ctx* c, const ulk::ReplayArgs& ra, bool plane, int plane_a,
             cudaFuncSetAttribute(ulk::k_plane_idft<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
             cudaFuncSetAttribute(ulk::k_plane_idft<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
             cudaFuncSetAttribute(ulk::k_plane_idft<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
-            attr_set = true;
+            c->plane_attr_set = true;
         }
         const long long ne = (long long)R * 12 * N2;
         const int ept = plane_ept(N2);                                   // entries per thread: Ns^2 / ept <= 1024 threads
@@ -998,6 +1068,7 @@ int plane_finish(ul_ctx* c, int r_max) {
 // ul_multilevel (to fp64 rounding order), with 2x the sweeps and none of the per-site TO accumulators.
 int ul_multilevel_replay(ul_ctx* c, int d, int n_sub, int r_max, const int* fps, int n_fp) {
     if (!c || n_sub < 0) return fail(c, UL_EINVAL, "n_sub must be >= 0");
+    DeviceGuard guard(c);
     if (n_fp == 0) return ul_multilevel(c, d, n_sub, r_max, fps, n_fp);                  // nothing is linear in O: nothing to replay
     int rc = check_meas_args(c, d, r_max, fps, n_fp);
     if (rc) return rc;
@@ -1105,6 +1176,7 @@ static int end2(ul_ctx* c) {
 }
 int ul_multilevel2(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, int r_max, const int* fps, int n_fp) {
     if (!c || n_in < 1 || n_out < 1) return fail(c, UL_EINVAL, "n_in, n_out must be >= 1");
+    DeviceGuard guard(c);
     int rc = begin2(c, d_in, d_out, r_max, fps, n_fp);
     if (rc) return rc;
     auto bail = [&](int code) { c->open = false; return code; };
@@ -1124,15 +1196,18 @@ int ul_multilevel2(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, int r_ma
 }
 int ul_measure2_begin(ul_ctx* c, int d_in, int d_out, int r_max, const int* fps, int n_fp) {
     if (!c) return fail(c, UL_EINVAL, "null handle");
+    DeviceGuard guard(c);
     return begin2(c, d_in, d_out, r_max, fps, n_fp);
 }
 int ul_combine(ul_ctx* c) {
     if (!c) return fail(c, UL_EINVAL, "null handle");
+    DeviceGuard guard(c);
     if (!c->open || c->d_out == 0) return fail(c, UL_ESTATE, "no open two-level measurement");
     return combine2(c);
 }
 int ul_measure2_end(ul_ctx* c) {
     if (!c) return fail(c, UL_EINVAL, "null handle");
+    DeviceGuard guard(c);
     if (!c->open || c->d_out == 0) return fail(c, UL_ESTATE, "no open two-level measurement");
     return end2(c);
 }
@@ -1144,6 +1219,7 @@ int ul_measure2_end(ul_ctx* c) {
 // Wc T2 O on the fly.  About three times the sub-update sweeps of ul_multilevel2, none of its TO accumulators.
 int ul_multilevel2_replay(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, int r_max, const int* fps, int n_fp) {
     if (!c || n_in < 1 || n_out < 1) return fail(c, UL_EINVAL, "n_in, n_out must be >= 1");
+    DeviceGuard guard(c);
     if (n_fp == 0) return ul_multilevel2(c, d_in, n_in, d_out, n_out, r_max, fps, n_fp);
     int rc = check_meas_args(c, d_in, r_max, fps, n_fp);
     if (rc) return rc;
@@ -1240,6 +1316,7 @@ int ul_multilevel2_replay(ul_ctx* c, int d_in, int n_in, int d_out, int n_out, i
 
 int ul_plaquette(ul_ctx* c, double* out) {
     if (!c || !out) return fail(c, UL_EINVAL, "null pointer");
+    DeviceGuard guard(c);
     const int gx = (c->Ns * c->Ns + 255) / 256, rows = c->Nt * c->Ns;
     const int gy = rows < NBLK / gx ? rows : (NBLK / gx > 0 ? NBLK / gx : 1);
     if (gx * gy > NBLK) return fail(c, UL_EINVAL, "lattice too large for this build");
@@ -1255,6 +1332,7 @@ int ul_plaquette(ul_ctx* c, double* out) {
 }
 int ul_polyakov(ul_ctx* c, int multihit, double* out) {
     if (!c || !out || (multihit != 0 && multihit != 1)) return fail(c, UL_EINVAL, "multihit must be 0 or 1");
+    DeviceGuard guard(c);
     const int nb = (int)((c->Vs + 255) / 256) < NBLK ? (int)((c->Vs + 255) / 256) : NBLK;
     ulk::k_polyakov<<<nb, 256, 0, c->stream>>>(geom(c), c->th, c->beta, multihit, c->scratch);
     ulk::k_sum_partials<<<2, 256, 0, c->stream>>>(c->scratch, nb, c->scratch + 2 * NBLK, 1.0 / (double)c->Vs, 0);
@@ -1274,6 +1352,7 @@ int ul_read_correlators(ul_ctx* c, double* corr, double* field, double* vacuum) 
 }
 int ul_read_slab_averages(ul_ctx* c, double* out) {
     if (!c || !out) return fail(c, UL_EINVAL, "null pointer");
+    DeviceGuard guard(c);
     if (!c->have) return fail(c, UL_ESTATE, "no measurement yet");
     const size_t n = (size_t)3 * c->res_r_max * c->res_n_slab * (size_t)c->Vs * 2;
     UL_CUDA(c, cudaMemcpyAsync(out, c->res_A, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
@@ -1289,6 +1368,7 @@ int ul_set_site_offset(ul_ctx* c, int64_t offset) {
 }
 int ul_slab_partial_product(ul_ctx* c, int s_begin, int s_end, void* dev_out) {
     if (!c || !dev_out) return fail(c, UL_EINVAL, "null pointer");
+    DeviceGuard guard(c);
     if (!c->have) return fail(c, UL_ESTATE, "no measurement yet");
     if (s_begin < 0 || s_end > c->res_n_slab || s_begin > s_end) return fail(c, UL_EINVAL, "bad slab range");
     ulk::WeightArgs wa;
@@ -1302,6 +1382,7 @@ int ul_slab_partial_product(ul_ctx* c, int s_begin, int s_end, void* dev_out) {
 }
 int ul_combine_partial_products(ul_ctx* c, const void* const* dev_parts, int n_parts, double* corr) {
     if (!c || !dev_parts || !corr) return fail(c, UL_EINVAL, "null pointer");
+    DeviceGuard guard(c);
     if (n_parts < 1 || n_parts > ulk::MAX_SHARDS) return fail(c, UL_EINVAL, "need 1 <= n_parts <= 64");
     if (!c->have) return fail(c, UL_ESTATE, "no measurement yet");
     ulk::CombinePartsArgs a;
@@ -1322,6 +1403,51 @@ int ul_combine_partial_products(ul_ctx* c, const void* const* dev_parts, int n_p
     c->corr.assign(corr, corr + 2 * R);                        // ul_read_correlators now returns the global C(r)
     return UL_OK;
 }
+int ul_set_halo_peers(ul_ctx* c, void* dn_links, void* up_links, int ghost_layers) {
+    if (!c) return fail(c, UL_EINVAL, "null handle");
+    if (c->open) return fail(c, UL_ESTATE, "a measurement is open");
+    if (!dn_links && !up_links) { c->peer_dn = c->peer_up = nullptr; c->peer_flag_dn = c->peer_flag_up = nullptr; c->halo_gl = 0; return UL_OK; }
+    if (!dn_links || !up_links || ghost_layers < 2 || (ghost_layers & 1) || c->Nt - 2 * ghost_layers < ghost_layers)
+        return fail(c, UL_EINVAL, "need both neighbours, an even number >= 2 of ghost layers and at least that many own layers");
+    DeviceGuard guard(c);
+    for (void* p : {dn_links, up_links}) {                        // a neighbour on another device of this process: enable peer access
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, p) != cudaSuccess || at.type != cudaMemoryTypeDevice) { cudaGetLastError(); return fail(c, UL_EINVAL, "peer links must be device memory"); }
+        if (at.device != c->dev) {
+            int can = 0;
+            cudaDeviceCanAccessPeer(&can, c->dev, at.device);
+            if (!can) return fail(c, UL_ECUDA, "no peer access to the neighbour's device");
+            const cudaError_t e = cudaDeviceEnablePeerAccess(at.device, 0);
+            if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) return fail(c, UL_ECUDA, std::string("cudaDeviceEnablePeerAccess: ") + cudaGetErrorString(e));
+            cudaGetLastError();
+        }
+    }
+    c->peer_dn = (int*)dn_links; c->peer_up = (int*)up_links; c->halo_gl = ghost_layers;
+    return UL_OK;
+}
+int ul_halo_flags(ul_ctx* c, void** dev_flags) {
+    if (!c || !dev_flags) return fail(c, UL_EINVAL, "null pointer");
+    DeviceGuard guard(c);
+    if (!c->halo_flags) {
+        void* p = nullptr;
+        UL_CUDA(c, cudaMalloc(&p, 2 * sizeof(uint32_t)));
+        c->halo_flags = (uint32_t*)p;
+    }
+    UL_CUDA(c, cudaMemsetAsync(c->halo_flags, 0, 2 * sizeof(uint32_t), c->stream));
+    UL_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->halo_seq = 0;
+    *dev_flags = c->halo_flags;
+    return UL_OK;
+}
+int ul_set_halo_peer_flags(ul_ctx* c, void* dn_flags, void* up_flags) {
+    if (!c) return fail(c, UL_EINVAL, "null handle");
+    if (!dn_flags || !up_flags) { c->peer_flag_dn = c->peer_flag_up = nullptr; return UL_OK; }
+    if (!c->halo_flags) return fail(c, UL_ESTATE, "call ul_halo_flags first");
+    c->peer_flag_dn = (uint32_t*)dn_flags + 1;                    // the shard below hears from its upper neighbour in its flags[1]
+    c->peer_flag_up = (uint32_t*)up_flags;                        // the shard above from its lower neighbour in its flags[0]
+    c->halo_seq = 0;
+    return UL_OK;
+}
 int ul_get_launch_count(ul_ctx* c, uint64_t* n) { if (!c || !n) return fail(c, UL_EINVAL, "null pointer"); *n = c->launches; return UL_OK; }
 
 int ul_philox_selftest(const uint32_t* ctr, const uint32_t* key, uint32_t* out, int n) {
@@ -1339,6 +1465,7 @@ int ul_philox_selftest(const uint32_t* ctr, const uint32_t* key, uint32_t* out, 
 }
 int ul_sync(ul_ctx* c) {
     if (!c) return fail(c, UL_EINVAL, "null handle");
+    DeviceGuard guard(c);
     UL_CUDA(c, cudaStreamSynchronize(c->stream));
     return UL_OK;
 }

@@ -38,6 +38,12 @@ struct UpdateArgs {
     int4* queue;          // heatbath stragglers: (element offset in th[mu][parity], site, Sx, Sy), see k_hb_stragglers
     int* qcount;          // [HB_NQ] entries in each sub-queue (zero before the launch) + [1] ticket of k_hb_stragglers
     int qcap;             // capacity of a sub-queue; sub-queue i = queue[i * qcap ...]
+    // t-sharded full sweeps with peer-memory halo writes: the kernel stores the first / last halo_gl own time
+    // layers it updates also into the neighbour shards' ghost layers (their link arrays, mapped peer memory over NVLink or
+    // the same device), so no separate exchange step follows the sub-step.  Own layers: [halo_gl, halo_gl + halo_nt).
+    int* peer_dn;         // link array of the shard below (t - 1 side), or nullptr
+    int* peer_up;         // link array of the shard above
+    int halo_gl, halo_nt;
     uint32_t site_offset; // added to the local canonical site index in the Philox counter (slab sharding: t0 * Ns^3)
     int met_delta_bt;     // Metropolis proposal half-width delta as a binary angle (0 < delta <= pi -> up to 2^31 - 1)
 };
@@ -56,6 +62,7 @@ struct Site {
     int dm[4], dp[4];     // element deltas for a displacement of -1 / +1 along t, (x1: 0), x2, x3
     int dxp, dxm;         // element deltas to the extra element of a +1 / -1 shifted chunk
     int off;              // x1 = 2h + off
+    int t;                // local time layer
 };
 
 // Global loads of link angles.  COH = false: the read-only path (ld.global.nc), fine when the whole kernel only reads the
@@ -275,9 +282,17 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
                 }
         }
     }
-    if (VEC == 4) *reinterpret_cast<int4*>(own) = make_int4(out[0], out[1 % VEC], out[2 % VEC], out[3 % VEC]);
-    else if (VEC == 2) *reinterpret_cast<int2*>(own) = make_int2(out[0], out[1 % VEC]);
-    else own[0] = out[0];
+    auto store = [&](int* dst) {
+        if (VEC == 4) *reinterpret_cast<int4*>(dst) = make_int4(out[0], out[1 % VEC], out[2 % VEC], out[3 % VEC]);
+        else if (VEC == 2) *reinterpret_cast<int2*>(dst) = make_int2(out[0], out[1 % VEC]);
+        else dst[0] = out[0];
+    };
+    store(own);
+    if (P.peer_dn != nullptr) {                                   // (uniform) boundary layers also go to the neighbours' ghost layers
+        const int arr = (MU * 2 + p) * P.Vh + st.e0, shift = P.halo_nt * (P.Ns * P.Ns * P.Nh);
+        if (st.t < 2 * P.halo_gl) store(P.peer_dn + arr + shift);                // first own layers -> upper ghost of the shard below
+        if (st.t >= P.halo_nt) store(P.peer_up + arr - shift);                   // last own layers -> lower ghost of the shard above
+    }
 }
 
 
@@ -321,6 +336,7 @@ __device__ __forceinline__ void update_tile(const UpdateArgs& P, const int tx, c
     Site st;
     st.off = sel;                                     // = (p + x2 + x3 + t) & 1: x1 = 2h + off for the links of this thread
     st.e0 = ((t * Ns + x3) * Ns + x2) * Nh + h0;
+    st.t = t;
     st.dp[0] = (t == Nt - 1) ? -(Nt - 1) * stt : stt;   st.dm[0] = (t == 0) ? (Nt - 1) * stt : -stt;
     st.dp[1] = 0;                                       st.dm[1] = 0;
     st.dp[2] = (x2 == Ns - 1) ? -(Ns - 1) * sy : sy;    st.dm[2] = (x2 == 0) ? (Ns - 1) * sy : -sy;
@@ -372,7 +388,13 @@ __global__ void __launch_bounds__(256, UL_HBS_MINB) k_hb_stragglers(const Update
     for (int e = blockIdx.y * blockDim.x + threadIdx.x; e < n; e += gridDim.y * blockDim.x) {
         const int4 q = q0[e];
         // q.y = the site index, all 32 bits (ghost-layer sites of a shard wrap); (q.z, q.w) = the staple sum, (0, 0) if k = 0
-        own[q.x] = ulm::hb_straggler(__int_as_float(q.z), __int_as_float(q.w), P.beta, (uint32_t)q.y, sweep_lo, sweep_hi, c3, P.key0, P.key1);
+        const int v = ulm::hb_straggler(__int_as_float(q.z), __int_as_float(q.w), P.beta, (uint32_t)q.y, sweep_lo, sweep_hi, c3, P.key0, P.key1);
+        own[q.x] = v;
+        if (P.peer_dn != nullptr) {                                                       // as in update_links
+            const int stt = P.Ns * P.Ns * P.Nh, t = q.x / stt, arr = (mu * 2 + P.parity) * P.Vh + q.x;
+            if (t < 2 * P.halo_gl) P.peer_dn[arr + P.halo_nt * stt] = v;
+            if (t >= P.halo_nt) P.peer_up[arr - P.halo_nt * stt] = v;
+        }
     }
     __syncthreads();                                                                      // every thread of the block has read its count
     if (threadIdx.x == 0) {

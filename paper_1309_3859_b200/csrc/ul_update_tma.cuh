@@ -127,6 +127,7 @@ __global__ void __launch_bounds__(256, 3) k_update_or_tma(const UpdateArgs P) {
     Site st;
     st.off = sel;
     st.e0 = ((t * Ns + x3) * Ns + x2) * Nh + h0;
+    st.t = t;
     const int roff = (x2 - x2lo) * Nh;
     float Sx[4] = {0.0f, 0.0f, 0.0f, 0.0f}, Sy[4] = {0.0f, 0.0f, 0.0f, 0.0f};
     mbar_wait(&mbar, 0u);

@@ -222,14 +222,14 @@ class ShardedSweeper:
     """Full sweeps of one lattice cut in t.  `group`: None under torch.distributed (one shard per process), or the list
     of all shards when they live in one process (shard-after-shard emulation on one GPU: the exchange is then a copy)."""
 
-    def __init__(self, Ns, Nt, beta, seed, rank, world, links, counter=0, device="cuda:0", stage_on_host=False):
+    def __init__(self, Ns, Nt, beta, seed, rank, world, links, counter=0, device="cuda:0", stage_on_host=False, stream=None):
         from . import ul
         self.stage_on_host = stage_on_host
         if Nt % world or (Nt // world) % 2:
             raise ValueError("Nt / world must be an even number of layers")
         self.nt_loc, self.rank, self.world = Nt // world, rank, world
         self.t0 = rank * self.nt_loc
-        self.lat = ul.Lattice(Ns, self.nt_loc + 2 * GL, beta, seed, device=device)
+        self.lat = ul.Lattice(Ns, self.nt_loc + 2 * GL, beta, seed, device=device, stream=stream)
         self.lat.set_site_offset((self.t0 - GL) * Ns ** 3)
         self.lat.set_links(shard_links_halo(links, self.t0, self.nt_loc))
         self.lat.set_counter(counter)
@@ -240,9 +240,10 @@ class ShardedSweeper:
         return self.lat.get_links_raw()[:, GL:GL + self.nt_loc]
 
 
-def sharded_sweep(shards, n_hb, n_or, dist=None):
+def sharded_sweep(shards, n_hb, n_or, dist=None, peer=False):
     """n_hb stochastic sweeps then n_or overrelaxation sweeps (the order of ul_sweep) on `shards`: the list of all
-    shards in one process (emulation) or [this rank's shard] under torch.distributed."""
+    shards in one process (emulation) or [this rank's shard] under torch.distributed.  peer: the shards were connected with
+    connect_peers, the kernels write the halos themselves and nothing is exchanged here."""
     for kind, count in ((2 if shards[0].alg == 1 else 0, n_hb), (1, n_or)):
         for _ in range(count):
             for parity in range(2):
@@ -250,6 +251,8 @@ def sharded_sweep(shards, n_hb, n_or, dist=None):
                     for sh in shards:
                         sh.lat.substep(kind, parity, mu, 0)
                     arr = 2 * mu + parity
+                    if peer:
+                        continue
                     if dist is not None:
                         sh = shards[0]
                         exchange_halos(sh.view, arr, sh.nt_loc, dist, sh.rank, sh.world, sh.stage_on_host)
@@ -263,3 +266,17 @@ def sharded_sweep(shards, n_hb, n_or, dist=None):
             if kind != 1:
                 for sh in shards:
                     sh.lat.set_counter(sh.lat.get_counter() + 1)
+
+
+def connect_peers(shards, flags=True):
+    """Shards of one process (one ShardedSweeper per GPU, or several on one GPU): every shard gets its neighbours' link arrays
+    as peer memory, so that the sub-step kernels write the boundary layers straight into the neighbours' ghost layers
+    (ul_set_halo_peers; NVLink peer stores when the shards sit on different GPUs), and, with flags, their flag words for the
+    stream-ordered hand-shake between neighbours.  sharded_sweep(shards, ..., peer=True) then issues no exchange at all."""
+    n = len(shards)
+    fl = [sh.lat.halo_flags() for sh in shards] if flags else None
+    for r, sh in enumerate(shards):
+        dn, up = shards[(r - 1) % n], shards[(r + 1) % n]
+        sh.lat.set_halo_peers(dn.lat.links.data_ptr(), up.lat.links.data_ptr(), GL)
+        if flags:
+            sh.lat.set_halo_peer_flags(fl[(r - 1) % n], fl[(r + 1) % n])

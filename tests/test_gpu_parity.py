@@ -1311,6 +1311,41 @@ def test_sharded_full_sweeps_reproduce_the_unsharded_run(ul, world, alg):
     assert all(sh.lat.get_counter() == full.get_counter() for sh in shards)
 
 
+@pytest.mark.parametrize("world,flags", [(2, False), (4, False), (2, True), (4, True), (1, True)])
+@pytest.mark.parametrize("alg", [0, 1])
+def test_peer_memory_halo_writes_reproduce_the_unsharded_run(ul, world, flags, alg):
+    """Full sweeps of a t-sharded lattice with the halo exchange FUSED into the sub-step kernels (ul_set_halo_peers: the kernels
+    store their boundary layers into the neighbours' ghost layers, here peer pointers on the same device) and, with flags,
+    every shard on its own stream, ordered only by the stream-ordered flag words between neighbours
+    (cuStreamWriteValue32 / cuStreamWaitValue32: no host synchronisation, no kernel waits on another): bit-identical
+    to ul_sweep on the whole lattice."""
+    import torch
+    from paper_1309_3859_b200 import sharded
+    Ns, Nt, beta, seed = 8, 16, 0.99, 91
+    full = ul.Lattice(Ns, Nt, beta, seed)
+    full.set_update_algorithm(alg, 1.2)
+    full.sweep(2, 1)
+    links0, ctr0 = full.get_links(), full.get_counter()
+    full.set_links(links0)
+    full.sweep(2, 3)
+    want = full.get_links_raw()
+    streams = [torch.cuda.Stream() if flags else None for _ in range(world)]
+    shards = [sharded.ShardedSweeper(Ns, Nt, beta, seed, r, world, links0, ctr0, stream=streams[r]) for r in range(world)]
+    for sh in shards:
+        sh.alg = alg
+        sh.lat.set_update_algorithm(alg, 1.2)
+        sh.lat.sync()
+    sharded.connect_peers(shards, flags=flags)
+    n0 = [sh.lat.launch_count() for sh in shards]
+    sharded.sharded_sweep(shards, 2, 3, peer=True)
+    for sh in shards:
+        sh.lat.sync()
+    got = np.concatenate([sh.own_links_raw() for sh in shards], axis=1)
+    assert np.array_equal(got, want)
+    assert all(sh.lat.get_counter() == full.get_counter() for sh in shards)
+    assert all(sh.lat.launch_count() - n for sh, n in zip(shards, n0))
+
+
 TWO_PROCESS_WORKER = r"""
 import os, sys
 sys.path.insert(0, {root!r})
