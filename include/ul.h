@@ -87,8 +87,16 @@ int ul_set_counter(ul_ctx* h, uint64_t sweep_counter);
 /* n_hb heatbath sweeps, then n_or overrelaxation sweeps, of the whole lattice.  One sweep =
  * 8 sub-steps: parity outer (even, odd: P:374), direction inner (0..3), in place.  Heatbath
  * draws theta' = alpha + phi, phi ~ exp(beta k cos phi), from the staple sum k e^{i alpha}
- * (DESIGN R2: Best-Fisher rejection, Philox4x32-10 keyed by (seed; site, sweep, attempt,
- * parity, mu)); overrelaxation sets theta' = 2 alpha - theta.  Asynchronous on the stream. */
+ * (DESIGN R2: Best-Fisher rejection; R19: Philox4x32-10 keyed by (seed; site, sweep, block,
+ * parity, mu), two attempts per block); overrelaxation sets theta' = 2 alpha - theta.
+ * Asynchronous on the stream.  How the sub-steps are launched depends on the lattice and never on
+ * the result (bit-identical, tested): one kernel per sub-step with programmatic dependent launch
+ * between them; a CUDA graph per recipe on lattices of <= 2^21 sites; one cooperative launch per
+ * compound sweep on lattices of <= 256 thread-block tiles (csrc/ul_persist.cuh).  Environment
+ * switches, read when the handle is created (for A/B measurements; defaults are the fast paths):
+ * UL_NO_PDL=1, UL_NO_ZFLIP=1 (alternating traversal of the time layers), UL_NO_PERSIST=1,
+ * UL_PERSIST_VEC=1|2|4, UL_OR_TMA=1 (overrelaxation through the bulk-copy staged gather,
+ * csrc/ul_update_tma.cuh: slower). */
 int ul_sweep(ul_ctx* h, int n_hb, int n_or);
 
 /* Test hook: one sub-step.  kind 0 = heatbath (draws with the current sweep counter, does
