@@ -374,13 +374,14 @@ __global__ void __launch_bounds__(256) k_slab_tables(const TableArgs P) {
 __global__ void __launch_bounds__(256) k_slab_tables_u(const TableArgs P) {
     const Geom& g = P.g;
     const int Ns = g.Ns, Nh = g.Nh;
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;      // over (s - s0, x3, x2, h)
-    const long long total = (long long)P.n_rows * Ns * Nh;
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;                   // over (s - s0, x3, x2, h): < V/2 < 2^30, 32-bit divisions
+    const unsigned total = (unsigned)P.n_rows * Ns * Nh;
     if (i >= total) return;
-    const int h = (int)(i % Nh);
-    const long long rr = i / Nh;                                                // (s - s0, x3, x2)
-    const int x2 = (int)(rr % Ns);
-    const int row = P.row0 + (int)(rr / Ns);                                    // s * Ns + x3
+    const unsigned rr = i / (unsigned)Nh;                                       // (s - s0, x3, x2)
+    const int h = (int)(i - rr * Nh);
+    const unsigned rq = rr / (unsigned)Ns;
+    const int x2 = (int)(rr - rq * Ns);
+    const int row = P.row0 + (int)rq;                                           // s * Ns + x3
     const int s = row / Ns, x3 = row - s * Ns;
     unsigned acc0 = 0u, acc1 = 0u;                                              // parity-0 / parity-1 array element
     for (int t = s * P.d; t < (s + 1) * P.d; ++t) {
