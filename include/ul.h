@@ -259,6 +259,14 @@ int ul_combine_partial_products(ul_ctx* h, const void* const* dev_parts, int n_p
 int ul_set_halo_peers(ul_ctx* h, void* dn_links, void* up_links, int ghost_layers);
 int ul_halo_flags(ul_ctx* h, void** dev_flags);
 int ul_set_halo_peer_flags(ul_ctx* h, void* dn_flags, void* up_flags);
+/* The same between processes (one process per GPU, the shards' processes exchange the 64-byte handles through
+ * torch.distributed): ul_ipc_export writes the CUDA IPC handles (cudaIpcMemHandle_t, 64 bytes each) of the allocations
+ * that hold this context's link array and its flag words (ul_halo_flags first) and the byte offsets of the two inside
+ * them; ul_ipc_open maps a neighbour's allocation into this process (once per allocation; closed by ul_destroy) and
+ * returns the device pointer to pass to ul_set_halo_peers / ul_set_halo_peer_flags.  The exporting memory must come
+ * from cudaMalloc (ul_create, or a PyTorch tensor of the default caching allocator).  UL_ECUDA if IPC is refused. */
+int ul_ipc_export(ul_ctx* h, void* out_links_handle, uint64_t* links_offset, void* out_flags_handle, uint64_t* flags_offset);
+int ul_ipc_open(ul_ctx* h, const void* handle, uint64_t offset, void** dev_ptr);
 
 /* Results of the last measurement, HOST buffers (any may be NULL):
  * corr[r_max][2]           C(r) = (1/3Ns^3) sum_x sum_mu prod_s [T](x,s,mu,r)       (re, im)

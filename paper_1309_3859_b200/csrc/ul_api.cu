@@ -13,6 +13,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "ul_measure.cuh"
@@ -144,6 +145,7 @@ struct ul_ctx {
     uint32_t* peer_flag_dn = nullptr;    // where this shard reports to the shard below (its flags[1]) / above (its flags[0])
     uint32_t* peer_flag_up = nullptr;
     uint32_t halo_seq = 0;               // sub-steps completed since the peers were set
+    std::vector<std::pair<cudaIpcMemHandle_t, void*>> ipc_open;   // neighbours' allocations opened through CUDA IPC
     bool or_tma = false, or_tma_attr = false;   // UL_OR_TMA=1: overrelaxation through the bulk-copy staged kernel
     bool use_pdl = true;      // programmatic dependent launch between the update kernels (UL_NO_PDL=1 turns it off)
     cudaStream_t cap_stream = nullptr;
@@ -782,6 +784,7 @@ int ul_destroy(ul_ctx* c) {
     if (c->scratch) cudaFree(c->scratch);
     if (c->hb_queue) cudaFree(c->hb_queue);
     if (c->d_bar) cudaFree(c->d_bar);
+    for (auto& e : c->ipc_open) cudaIpcCloseMemHandle(e.second);
     if (c->halo_flags) cudaFree(c->halo_flags);
     for (auto& e : c->graphs) if (e.exec) cudaGraphExecDestroy(e.exec);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
@@ -1446,6 +1449,45 @@ int ul_set_halo_peer_flags(ul_ctx* c, void* dn_flags, void* up_flags) {
     c->peer_flag_dn = (uint32_t*)dn_flags + 1;                    // the shard below hears from its upper neighbour in its flags[1]
     c->peer_flag_up = (uint32_t*)up_flags;                        // the shard above from its lower neighbour in its flags[0]
     c->halo_seq = 0;
+    return UL_OK;
+}
+// ---- the same between PROCESSES (one process per GPU): CUDA IPC handles of the link array and the flag words
+int ul_ipc_export(ul_ctx* c, void* out_links_handle, uint64_t* links_offset, void* out_flags_handle, uint64_t* flags_offset) {
+    if (!c || !out_links_handle || !links_offset || !out_flags_handle || !flags_offset) return fail(c, UL_EINVAL, "null pointer");
+    DeviceGuard guard(c);
+    if (!c->halo_flags) return fail(c, UL_ESTATE, "call ul_halo_flags first");
+    typedef int (*GetRange)(unsigned long long*, size_t*, unsigned long long);
+    static GetRange get_range = [] {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult st;
+        return (cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &st) == cudaSuccess && st == cudaDriverEntryPointSuccess) ? (GetRange)fn : (GetRange) nullptr;
+    }();
+    if (!get_range) return fail(c, UL_ECUDA, "cuMemGetAddressRange not available");
+    const void* ptrs[2] = {c->th, c->halo_flags};
+    void* outs[2] = {out_links_handle, out_flags_handle};
+    uint64_t* offs[2] = {links_offset, flags_offset};
+    for (int i = 0; i < 2; ++i) {                                 // a handle names the whole allocation: pass the offset inside it along
+        unsigned long long base = 0;
+        size_t size = 0;
+        if (get_range(&base, &size, (unsigned long long)(uintptr_t)ptrs[i]) != 0) return fail(c, UL_ECUDA, "cuMemGetAddressRange");
+        cudaIpcMemHandle_t hnd;
+        UL_CUDA(c, cudaIpcGetMemHandle(&hnd, (void*)(uintptr_t)base));
+        std::memcpy(outs[i], &hnd, sizeof(hnd));
+        *offs[i] = (uint64_t)((uintptr_t)ptrs[i] - (uintptr_t)base);
+    }
+    return UL_OK;
+}
+int ul_ipc_open(ul_ctx* c, const void* handle, uint64_t offset, void** dev_ptr) {
+    if (!c || !handle || !dev_ptr) return fail(c, UL_EINVAL, "null pointer");
+    DeviceGuard guard(c);
+    cudaIpcMemHandle_t hnd;
+    std::memcpy(&hnd, handle, sizeof(hnd));
+    for (auto& e : c->ipc_open)                                    // an allocation is opened once per process
+        if (std::memcmp(&e.first, &hnd, sizeof(hnd)) == 0) { *dev_ptr = (char*)e.second + offset; return UL_OK; }
+    void* base = nullptr;
+    UL_CUDA(c, cudaIpcOpenMemHandle(&base, hnd, cudaIpcMemLazyEnablePeerAccess));
+    c->ipc_open.push_back({hnd, base});
+    *dev_ptr = (char*)base + offset;
     return UL_OK;
 }
 int ul_get_launch_count(ul_ctx* c, uint64_t* n) { if (!c || !n) return fail(c, UL_EINVAL, "null pointer"); *n = c->launches; return UL_OK; }

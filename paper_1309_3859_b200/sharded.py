@@ -280,3 +280,28 @@ def connect_peers(shards, flags=True):
         sh.lat.set_halo_peers(dn.lat.links.data_ptr(), up.lat.links.data_ptr(), GL)
         if flags:
             sh.lat.set_halo_peer_flags(fl[(r - 1) % n], fl[(r + 1) % n])
+
+
+def connect_peers_ipc(shard, dist):
+    """One shard per PROCESS (torch.distributed, any backend that can all_gather_object): the ranks exchange the CUDA IPC
+    handles of their link arrays and flag words, every rank maps its two neighbours' and sets them as halo peers; from then on
+    sharded_sweep([shard], ..., peer=True) needs no communication call at all: the kernels write the halos over NVLink (or
+    inside the GPU when the ranks share one) and the streams order themselves through the flag words."""
+    rank, world = dist.get_rank(), dist.get_world_size()
+    shard.lat.halo_flags()
+    mine = shard.lat.ipc_export()
+    everyone = [None] * world
+    dist.all_gather_object(everyone, mine)
+    dn, up = everyone[(rank - 1) % world], everyone[(rank + 1) % world]
+    if world == 1:
+        links = {0: shard.lat.links.data_ptr()}
+        shard.lat.set_halo_peers(links[0], links[0], GL)
+        f = shard.lat.halo_flags()
+        shard.lat.set_halo_peer_flags(f, f)
+        return
+    p = {}
+    for name, (hl, ol, hf, of) in (("dn", dn), ("up", up)):
+        p[name] = (shard.lat.ipc_open(hl, ol), shard.lat.ipc_open(hf, of))
+    shard.lat.set_halo_peers(p["dn"][0], p["up"][0], GL)
+    shard.lat.set_halo_peer_flags(p["dn"][1], p["up"][1])
+    dist.barrier()                                       # nobody starts before every rank has its peers (the flag words are zero)

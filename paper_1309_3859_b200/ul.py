@@ -19,7 +19,7 @@ SYMBOLS = [
     "ul_create", "ul_create_ext", "ul_workspace_bytes", "ul_destroy", "ul_init", "ul_set_beta",
     "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep", "ul_substep_slabs", "ul_set_slab_group",
     "ul_set_subupdate", "ul_set_update_algorithm", "ul_multilevel", "ul_multilevel_replay", "ul_workspace_bytes_replay", "ul_multilevel2_replay", "ul_workspace_bytes_replay2", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
-    "ul_measure_end", "ul_measure2_begin", "ul_combine", "ul_measure2_end", "ul_set_accum_batch", "ul_set_multihit", "ul_plaquette", "ul_polyakov", "ul_set_site_offset", "ul_slab_partial_product", "ul_combine_partial_products", "ul_set_halo_peers", "ul_halo_flags", "ul_set_halo_peer_flags", "ul_read_correlators", "ul_read_slab_averages",
+    "ul_measure_end", "ul_measure2_begin", "ul_combine", "ul_measure2_end", "ul_set_accum_batch", "ul_set_multihit", "ul_plaquette", "ul_polyakov", "ul_set_site_offset", "ul_slab_partial_product", "ul_combine_partial_products", "ul_set_halo_peers", "ul_halo_flags", "ul_set_halo_peer_flags", "ul_ipc_export", "ul_ipc_open", "ul_read_correlators", "ul_read_slab_averages",
     "ul_get_launch_count", "ul_philox_selftest", "ul_sync", "ul_last_error",
 ]
 
@@ -79,6 +79,8 @@ def lib():
         L.ul_set_halo_peers.argtypes = [P, P, P, C.c_int]
         L.ul_halo_flags.argtypes = [P, C.POINTER(P)]
         L.ul_set_halo_peer_flags.argtypes = [P, P, P]
+        L.ul_ipc_export.argtypes = [P, P, C.POINTER(C.c_uint64), P, C.POINTER(C.c_uint64)]
+        L.ul_ipc_open.argtypes = [P, P, C.c_uint64, C.POINTER(P)]
         L.ul_accumulate.argtypes = [P]
         L.ul_measure_end.argtypes = [P]
         L.ul_measure2_begin.argtypes = [P, C.c_int, C.c_int, C.c_int, P, C.c_int]
@@ -343,6 +345,19 @@ class Lattice:
 
     def set_halo_peer_flags(self, dn_flags_ptr, up_flags_ptr):
         self._ck(lib().ul_set_halo_peer_flags(self._h, C.c_void_p(dn_flags_ptr or None), C.c_void_p(up_flags_ptr or None)))
+
+    def ipc_export(self):
+        """(links handle bytes, offset, flags handle bytes, offset) for the neighbours' processes (after halo_flags())."""
+        hl, hf = C.create_string_buffer(64), C.create_string_buffer(64)
+        ol, of = C.c_uint64(), C.c_uint64()
+        self._ck(lib().ul_ipc_export(self._h, hl, C.byref(ol), hf, C.byref(of)))
+        return bytes(hl.raw), ol.value, bytes(hf.raw), of.value
+
+    def ipc_open(self, handle, offset):
+        """Device pointer (int) of a neighbour process's allocation + offset."""
+        p = C.c_void_p()
+        self._ck(lib().ul_ipc_open(self._h, C.c_char_p(handle), int(offset), C.byref(p)))
+        return p.value
 
     def launch_count(self):
         v = C.c_uint64()

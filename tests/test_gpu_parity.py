@@ -1388,8 +1388,18 @@ ok_C = np.abs(C - C_full).max() <= 1e-13 * max(1.0, np.abs(C_full).max())
 sw = sharded.ShardedSweeper(Ns, Nt, beta, seed, rank, world, links0, ctr0, stage_on_host=True)
 sharded.sharded_sweep([sw], 2, 2, dist)
 ok_sweep = np.array_equal(sw.own_links_raw(), after_sw[:, sw.t0:sw.t0 + sw.nt_loc]) and sw.lat.get_counter() == ctr0 + 2
+# (3) the same sweeps with peer-memory halo writes between the two PROCESSES: CUDA IPC handles of the link arrays and
+# flag words, the kernels write the neighbour's ghost layers, the streams wait on the flag words (no communication call)
+import signal
+signal.alarm(240)                                    # a lost hand-shake must not outlive the test
+pw = sharded.ShardedSweeper(Ns, Nt, beta, seed, rank, world, links0, ctr0)
+sharded.connect_peers_ipc(pw, dist)
+sharded.sharded_sweep([pw], 2, 2, peer=True)
+pw.lat.sync()
+ok_peer = np.array_equal(pw.own_links_raw(), after_sw[:, pw.t0:pw.t0 + pw.nt_loc]) and pw.lat.get_counter() == ctr0 + 2
 dist.barrier()
-print("RESULT", rank, bool(ok_links), bool(ok_C), bool(ok_sweep))
+signal.alarm(0)
+print("RESULT", rank, bool(ok_links), bool(ok_C), bool(ok_sweep), bool(ok_peer))
 dist.destroy_process_group()
 """
 
@@ -1397,7 +1407,8 @@ dist.destroy_process_group()
 def test_two_processes_on_one_gpu_sharded_multilevel_and_sweeps(ul, tmp_path):
     """The real multi-process code path of paper_1309_3859_b200/sharded.py: two ranks (two processes, both on cuda:0,
     torch.distributed over gloo with host-staged tensors; no kernel of one rank waits on the other: the waits are the
-    hosts') run ShardedLattice and ShardedSweeper and reproduce the unsharded run bit for bit / to 1e-13."""
+    hosts') run ShardedLattice and ShardedSweeper and reproduce the unsharded run bit for bit / to 1e-13; then the same
+    sweeps with peer-memory halo writes between the processes (CUDA IPC; stream-ordered flag words, no spinning kernel)."""
     import subprocess
     import sys
     script = tmp_path / "worker.py"
@@ -1407,11 +1418,16 @@ def test_two_processes_on_one_gpu_sharded_multilevel_and_sweeps(ul, tmp_path):
     for r in range(2):
         env = dict(os.environ, RANK=str(r), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
         procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True))
-    outs = [p.communicate(timeout=600) for p in procs]
+    try:
+        outs = [p.communicate(timeout=600) for p in procs]
+    finally:
+        for p in procs:
+            if p.poll() is None:
+                p.kill()
     assert all(p.returncode == 0 for p in procs), outs
     for r in range(2):
         line = [l for l in outs[r][0].splitlines() if l.startswith("RESULT")][0]
-        assert line == f"RESULT {r} True True True", (line, outs[r][1][-2000:])
+        assert line == f"RESULT {r} True True True True", (line, outs[r][1][-2000:])
 
 
 # ----------------------------------------------------------------------------- degenerate and extreme shapes
