@@ -155,15 +155,33 @@ def main():
     t = torch.tensor([e0.elapsed_time(e1), e1.elapsed_time(e2)], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    # full sweeps of the same lattice cut in t, the halos written by the kernels into the neighbours' ghost layers
+    sweep_ms = None
+    if Nt % world == 0 and (Nt // world) % 2 == 0 and Nt // world >= GL:
+        sw = ShardedSweeper(Ns, Nt, 1.0, 4, rank, world, links.cpu().numpy(), ctr, device=f"cuda:{local}")
+        if world > 1:
+            connect_peers_ipc(sw, dist)
+        else:
+            connect_peers([sw])
+        sharded_sweep([sw], 1, 4, peer=True)
+        torch.cuda.synchronize()
+        e3, e4 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e3.record()
+        for _ in range(5):
+            sharded_sweep([sw], 1, 4, peer=True)
+        e4.record()
+        torch.cuda.synchronize()
+        ts = torch.tensor([e3.elapsed_time(e4) / 5], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(ts, op=dist.ReduceOp.MAX)
+        sweep_ms = float(ts[0])
     if rank == 0:
         print({"world": world, "lattice": f"{Ns}^3x{Nt}", "d": d, "n_sub": n_sub, "subupdate_loop_ms": float(t[0]),
-               "exchange_ms": float(t[1]), "C": [complex(c) for c in C]})
+               "exchange_ms": float(t[1]), "compound_1hb_4or_sweep_peer_halo_ms": sweep_ms, "C": [complex(c) for c in C]})
     if world > 1:
         dist.destroy_process_group()
 
 
-if __name__ == "__main__":
-    main()
 
 
 # ---------------------------------------------------------------------------------------------------------------------
@@ -305,3 +323,7 @@ def connect_peers_ipc(shard, dist):
     shard.lat.set_halo_peers(p["dn"][0], p["up"][0], GL)
     shard.lat.set_halo_peer_flags(p["dn"][1], p["up"][1])
     dist.barrier()                                       # nobody starts before every rank has its peers (the flag words are zero)
+
+
+if __name__ == "__main__":
+    main()
