@@ -17,7 +17,7 @@ UL_OK, UL_EINVAL, UL_ENOMEM, UL_ECUDA, UL_ESTATE = 0, -1, -2, -3, -4
 # every symbol include/ul.h declares (tests check that the library exports exactly these)
 SYMBOLS = [
     "ul_create", "ul_create_ext", "ul_workspace_bytes", "ul_destroy", "ul_init", "ul_set_beta",
-    "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep", "ul_substep_slabs", "ul_set_slab_group",
+    "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep", "ul_substep_slabs", "ul_set_slab_group", "ul_set_slab_group_streams",
     "ul_set_subupdate", "ul_set_update_algorithm", "ul_multilevel", "ul_multilevel_replay", "ul_workspace_bytes_replay", "ul_multilevel2_replay", "ul_workspace_bytes_replay2", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
     "ul_measure_end", "ul_measure2_begin", "ul_combine", "ul_measure2_end", "ul_set_accum_batch", "ul_set_multihit", "ul_plaquette", "ul_polyakov", "ul_set_site_offset", "ul_slab_partial_product", "ul_combine_partial_products", "ul_set_halo_peers", "ul_halo_flags", "ul_set_halo_peer_flags", "ul_ipc_export", "ul_ipc_open", "ul_read_correlators", "ul_read_slab_averages",
     "ul_get_launch_count", "ul_philox_selftest", "ul_sync", "ul_last_error",
@@ -59,6 +59,7 @@ def lib():
         L.ul_substep.argtypes = [P, C.c_int, C.c_int, C.c_int, C.c_int]
         L.ul_substep_slabs.argtypes = [P] + [C.c_int] * 6
         L.ul_set_slab_group.argtypes = [P, C.c_int]
+        L.ul_set_slab_group_streams.argtypes = [P, C.c_int]
         L.ul_set_subupdate.argtypes = [P, C.c_int, C.c_int, C.c_int]
         L.ul_set_update_algorithm.argtypes = [P, C.c_int, C.c_double]
         L.ul_multilevel.argtypes = [P, C.c_int, C.c_int, C.c_int, P, C.c_int]
@@ -227,6 +228,9 @@ class Lattice:
 
     def set_slab_group(self, n_slabs):
         self._ck(lib().ul_set_slab_group(self._h, int(n_slabs)))
+
+    def set_slab_group_streams(self, n_streams):
+        self._ck(lib().ul_set_slab_group_streams(self._h, int(n_streams)))
 
     def set_update_algorithm(self, alg, delta=np.pi):
         self._ck(lib().ul_set_update_algorithm(self._h, int(alg), float(delta)))

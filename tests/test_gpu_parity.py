@@ -1479,10 +1479,13 @@ def test_beta_zero_heatbath_is_uniform_on_device(ul):
 
 
 # ----------------------------------------------------------------------------- slab-group-major order
-@pytest.mark.parametrize("Ns,Nt,d,grp,alg,n_fp", [(8, 8, 2, 1, 0, 0), (8, 12, 2, 4, 0, 3), (6, 8, 4, 1, 1, 2), (16, 16, 2, 3, 0, 0)])
-def test_slab_group_major_order_is_bit_identical(ul, Ns, Nt, d, grp, alg, n_fp):
-    """ul_set_slab_group: the n_sub loop run slab group by slab group (ragged last group, ragged last batch) gives
-    the same links, sweep counter, slab sums, C(r) and G bit for bit as the sub-update-major order; vacuum to 1e-13."""
+@pytest.mark.parametrize("Ns,Nt,d,grp,streams,alg,n_fp", [(8, 8, 2, 1, 1, 0, 0), (8, 12, 2, 4, 1, 0, 3), (6, 8, 4, 1, 1, 1, 2), (16, 16, 2, 3, 1, 0, 0),
+                                                          (8, 16, 2, 2, 2, 0, 0), (8, 12, 2, 1, 4, 1, 2), (16, 16, 2, 3, 2, 0, 3), (8, 8, 4, 1, 3, 0, 0)])
+def test_slab_group_major_order_is_bit_identical(ul, Ns, Nt, d, grp, streams, alg, n_fp):
+    """ul_set_slab_group / ul_set_slab_group_streams: the n_sub loop run slab group by slab group (ragged last group, ragged
+    last round, ragged last batch), one group after the other or several side by side on their own streams (a round's compound
+    sub-update captured as one CUDA graph with a fork and a join), gives the same links, sweep counter, slab sums, C(r) and G
+    bit for bit as the sub-update-major order; vacuum to 1e-13."""
     R, n_sub = 3, 5
     fps = FPS[:n_fp]
     res = []
@@ -1493,7 +1496,9 @@ def test_slab_group_major_order_is_bit_identical(ul, Ns, Nt, d, grp, alg, n_fp):
             g.set_update_algorithm(1, 1.3)
         g.set_accum_batch(2)
         g.set_slab_group(mode)
+        g.set_slab_group_streams(streams)
         g.multilevel(d, n_sub, R, fps)
+        g.multilevel(d, n_sub, R, fps)                               # (the second call replays the captured rounds)
         res.append((g.get_links_raw(), g.get_counter(), g.read_slab_averages(), *g.read_correlators()))
     a, b = res
     assert np.array_equal(a[0], b[0]) and a[1] == b[1]
