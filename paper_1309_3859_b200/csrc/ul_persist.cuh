@@ -49,6 +49,31 @@ __device__ __forceinline__ void grid_barrier(unsigned* bar, unsigned k, int tid)
     __syncthreads();
 }
 
+// The heatbath sub-step with the stragglers finished by the SAME thread block from a shared-memory queue (as in the persistent
+// kernel below) instead of the striped global queue + k_hb_stragglers: for the small launches of a slab group (0.5-1 M links)
+// a second launch costs more than the ~12 % of extra instructions.  Same counters and device functions: bit-identical links.
+template <int MU, int VEC, bool DEVCTR>
+__global__ void __launch_bounds__(256, UL_HB_MINB) k_update_hb_local(const UpdateArgs P) {
+    __shared__ int4 sq[PQ_CAP];
+    __shared__ int scount;
+    const uint32_t sweep_lo = DEVCTR ? __ldg(P.sweep_dev) : P.sweep_lo, sweep_hi = DEVCTR ? __ldg(P.sweep_dev + 1) : P.sweep_hi;
+    const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+    const int nthr = blockDim.x * blockDim.y * blockDim.z;
+    if (tid == 0) scount = 0;
+    __syncthreads();
+    UpdateArgs Q = P;
+    Q.queue = sq; Q.qcount = &scount; Q.qcap = PQ_CAP;            // tile index 0 -> sub-queue 0: the block's own queue
+    update_tile<0, MU, VEC, false, true>(Q, blockIdx.x, blockIdx.y, blockIdx.z, gridDim.z, 0, sweep_lo, sweep_hi);
+    __syncthreads();                                               // the tile's angles (placeholders for pending links) and its queue are written
+    const int n = min(scount, PQ_CAP);
+    int* own = P.th + (MU * 2 + P.parity) * P.Vh;
+    const uint32_t c3 = ((uint32_t)P.parity << 2) | (uint32_t)MU;
+    for (int e = tid; e < n; e += nthr) {
+        const int4 q = sq[e];
+        own[q.x] = ulm::hb_straggler(__int_as_float(q.z), __int_as_float(q.w), P.beta, (uint32_t)q.y, sweep_lo, sweep_hi, c3, P.key0, P.key1);
+    }
+}
+
 template <int KIND, int VEC>
 __device__ __forceinline__ void persist_tile(const UpdateArgs& P, int mu, int tx, int ty, int tz, int ntz, uint32_t sweep_lo, uint32_t sweep_hi) {
     switch (mu) {
