@@ -192,7 +192,7 @@ int ul_measure2_end(ul_ctx* h);
 int ul_set_slab_group(ul_ctx* h, int n_slabs);
 /* Slab groups per round of the slab-group-major loop: n_streams groups run side by side, each on its own stream (own
  * straggler queue and sweep-counter copy), one compound sub-update of a round captured once as a CUDA graph and replayed.
- * 1 = one group after the other; default 2.  Bit-identical results.  UL_EINVAL outside 1..8; UL_ESTATE: a measurement is
+ * 1 = one group after the other; default 4.  Bit-identical results.  UL_EINVAL outside 1..8; UL_ESTATE: a measurement is
  * open. */
 int ul_set_slab_group_streams(ul_ctx* h, int n_streams);
 int ul_substep_slabs(ul_ctx* h, int kind, int parity, int mu, int slab_d, int s_begin, int s_end);

@@ -106,6 +106,8 @@ struct GraphKey {
 // one compound sub-update of a ROUND of slab groups (S groups side by side, each on its own stream), captured as one graph
 struct RoundGraph {
     int g0, grp, S, n_hb, n_or, sub_k, slab_d, alg;
+    int n_sub, kb, r_max, n_fp, multihit;   // the whole round: n_sub x (sub-update of the S groups, tables) + accumulation passes
+    const void* work; size_t ws_total;     // the workspace the table and accumulation launches were captured with
     double beta, met_delta;
     uint32_t site_offset;
     cudaGraphExec_t exec = nullptr;
@@ -152,7 +154,7 @@ struct ul_ctx {
     int grp_n = 0;
     bool hb_local_groups = true;        // ... (UL_NO_HB_LOCAL=1: the group launches use the global queue + straggler kernel)
     bool hb_local = false;              // heatbath launches finish their stragglers in the kernel (slab-group rounds)
-    int group_streams_n = 2;            // groups side by side per round (ul_set_slab_group's second knob; UL_GROUP_STREAMS)
+    int group_streams_n = 4;            // groups side by side per round (ul_set_slab_group's second knob; UL_GROUP_STREAMS)
     std::vector<RoundGraph> round_graphs;
     int dev = 0;              // the CUDA device of this context (entry points switch to it)
     // peer-memory halo writes (ul_set_halo_peers): neighbours' link arrays, own-layer range, stream-ordered flags
@@ -502,39 +504,59 @@ int group_streams(ul_ctx* c, int S) {
     return UL_OK;
 }
 
-// One compound sub-update of the round of slab groups that starts at slab g0: S groups of grp slabs side by side, each on its
-// own stream with its own straggler queue and sweep-counter copy, captured ONCE as a graph with a fork and a join and replayed
-// on the caller's stream (the kernels read the sweep counter from device memory, so the graph never changes).
-int round_subupdate(ul_ctx* c, int d, int g0, int grp, int S) {
+int accumulate(ul_ctx* c, int s_begin = 0, int s_end = -1);
+int flush(ul_ctx* c, int s_begin = 0, int s_end = -1);
+
+// The whole n_sub loop of one ROUND of slab groups (slabs g0 <= s < g1: S groups of grp slabs side by side), captured ONCE as a
+// graph and replayed: per sub-update a fork to the group streams (each with its own straggler queue and sweep-counter copy; the
+// kernels read the sweep counter from device memory, so the graph never changes), the compound sub-update of every group, a
+// join, the round's tables, and an accumulation pass whenever the batch is full.  Leaves the host state as the launches would.
+int round_run(ul_ctx* c, int d, int g0, int g1, int grp, int S, int n_sub) {
     RoundGraph* g = nullptr;
     for (auto& e : c->round_graphs)
         if (e.g0 == g0 && e.grp == grp && e.S == S && e.n_hb == c->sub_hb && e.n_or == c->sub_or && e.sub_k == c->sub_k && e.slab_d == d &&
-            e.alg == c->alg && e.beta == c->beta && e.met_delta == c->met_delta && e.site_offset == c->site_offset) g = &e;
+            e.alg == c->alg && e.beta == c->beta && e.met_delta == c->met_delta && e.site_offset == c->site_offset && e.n_sub == n_sub &&
+            e.kb == c->ws.kb && e.r_max == c->r_max && e.n_fp == c->n_fp && e.multihit == (c->multihit ? 1 : 0) && e.work == c->work &&
+            e.ws_total == c->ws.total) g = &e;
+    const bool deferred = c->n_fp == 0 && !c->multihit;             // accumulate(): the vacuum sums are then taken at the end
     if (!g) {
         if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(c, UL_ECUDA, "capture stream");
         cudaStream_t user = c->stream;
         int4* q0 = c->hb_queue; int* qc0 = c->hb_qcount; uint32_t* ds0 = c->d_sweep;
-        const uint64_t launches0 = c->launches;
+        const uint64_t launches0 = c->launches, sweep_keep = c->sweep;
         cudaGraph_t graph = nullptr;
         int rc = UL_OK;
         if (cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) rc = UL_ECUDA;
         c->capturing = true;
-        c->hb_local = c->hb_local_groups;
-        if (!rc && cudaEventRecord(c->grp_ev[0], c->cap_stream) != cudaSuccess) rc = UL_ECUDA;
-        for (int k = 0; k < S && !rc; ++k) {
-            const int s0 = g0 + k * grp;
-            if (s0 >= c->n_slab) break;
-            const int s1 = s0 + grp < c->n_slab ? s0 + grp : c->n_slab;
-            if (cudaStreamWaitEvent(c->grp_stream[k], c->grp_ev[0], 0) != cudaSuccess) { rc = UL_ECUDA; break; }
-            c->stream = c->grp_stream[k]; c->hb_queue = c->grp_queue[k]; c->hb_qcount = c->grp_qcount[k]; c->d_sweep = c->grp_sweep[k];
-            for (int kk = 0; kk < c->sub_k && !rc; ++kk) rc = compound_direct(c, c->sub_hb, c->sub_or, d, s0, s1);
-            if (!rc && (cudaEventRecord(c->grp_ev[1 + k], c->grp_stream[k]) != cudaSuccess ||
-                        cudaStreamWaitEvent(c->cap_stream, c->grp_ev[1 + k], 0) != cudaSuccess)) rc = UL_ECUDA;
+        c->acc_fresh = true; c->n_pending = 0;
+        for (int j = 0; j < n_sub && !rc; ++j) {
+            c->hb_local = c->hb_local_groups;
+            if (cudaEventRecord(c->grp_ev[0], c->cap_stream) != cudaSuccess) rc = UL_ECUDA;
+            for (int k = 0; k < S && !rc; ++k) {
+                const int s0 = g0 + k * grp;
+                if (s0 >= g1) break;
+                const int s1 = s0 + grp < g1 ? s0 + grp : g1;
+                if (cudaStreamWaitEvent(c->grp_stream[k], c->grp_ev[0], 0) != cudaSuccess) { rc = UL_ECUDA; break; }
+                c->stream = c->grp_stream[k]; c->hb_queue = c->grp_queue[k]; c->hb_qcount = c->grp_qcount[k]; c->d_sweep = c->grp_sweep[k];
+                for (int kk = 0; kk < c->sub_k && !rc; ++kk) rc = compound_direct(c, c->sub_hb, c->sub_or, d, s0, s1);
+                if (!rc && (cudaEventRecord(c->grp_ev[1 + k], c->grp_stream[k]) != cudaSuccess ||
+                            cudaStreamWaitEvent(c->cap_stream, c->grp_ev[1 + k], 0) != cudaSuccess)) rc = UL_ECUDA;
+            }
+            c->hb_local = false;
+            c->stream = c->cap_stream; c->hb_queue = q0; c->hb_qcount = qc0; c->d_sweep = ds0;
+            if (!rc) rc = accumulate(c, g0, g1);                    // the round's tables while its links are still in L2
+            if (!rc) {
+                c->n_pending += 1;
+                if (c->n_pending == c->ws.kb || j == n_sub - 1) rc = flush(c, g0, g1);
+            }
         }
         const cudaError_t ee = cudaStreamEndCapture(c->cap_stream, &graph);
         c->stream = user; c->hb_queue = q0; c->hb_qcount = qc0; c->d_sweep = ds0; c->capturing = false; c->hb_local = false;
+        c->sweep = sweep_keep;
         RoundGraph ng;
         ng.g0 = g0; ng.grp = grp; ng.S = S; ng.n_hb = c->sub_hb; ng.n_or = c->sub_or; ng.sub_k = c->sub_k; ng.slab_d = d; ng.alg = c->alg;
+        ng.n_sub = n_sub; ng.kb = c->ws.kb; ng.r_max = c->r_max; ng.n_fp = c->n_fp; ng.multihit = c->multihit ? 1 : 0;
+        ng.work = c->work; ng.ws_total = c->ws.total;
         ng.beta = c->beta; ng.met_delta = c->met_delta; ng.site_offset = c->site_offset;
         ng.launches = c->launches - launches0;
         c->launches = launches0;
@@ -544,7 +566,7 @@ int round_subupdate(ul_ctx* c, int d, int g0, int grp, int S) {
             return fail(c, UL_ECUDA, "slab-group round: graph capture failed");
         }
         cudaGraphDestroy(graph);
-        if (c->round_graphs.size() >= 64) {                            // bounded cache
+        if (c->round_graphs.size() >= 32) {                            // bounded cache
             cudaStreamSynchronize(c->stream);
             cudaGraphExecDestroy(c->round_graphs.front().exec);
             c->round_graphs.erase(c->round_graphs.begin());
@@ -553,8 +575,10 @@ int round_subupdate(ul_ctx* c, int d, int g0, int grp, int S) {
         g = &c->round_graphs.back();
     }
     if (cudaGraphLaunch(g->exec, c->stream) != cudaSuccess) return fail(c, UL_ECUDA, "cudaGraphLaunch (slab-group round)");
-    c->sweep += (uint64_t)c->sub_hb * (uint64_t)c->sub_k;
+    c->sweep += (uint64_t)c->sub_hb * (uint64_t)c->sub_k * (uint64_t)n_sub;
     c->launches += g->launches;
+    c->n_pending = 0; c->acc_fresh = false;
+    if (deferred) c->vac_deferred = true;
     return UL_OK;
 }
 
@@ -617,7 +641,7 @@ double* res_vacuum(ul_ctx* c) { return wsp<double>(c, c->ws.result) + 2 * (size_
 
 // adds the tabulated configurations (slots 0..n_pending-1) to the accumulators: rows a7, a8
 // (restricted to the slabs s_begin <= s < s_end when s_end >= 0: slab-group-major order)
-int flush(ul_ctx* c, int s_begin = 0, int s_end = -1) {
+int flush(ul_ctx* c, int s_begin, int s_end) {
     if (c->n_pending == 0) return UL_OK;
     NvtxRange range("ul:accumulate_batch");
     if (s_end < 0) s_end = c->n_slab;
@@ -686,7 +710,7 @@ int vacuum_pass(ul_ctx* c) {
 // tabulates the current configuration (U, Ot, column sums of O) into the next batch slot; the batch is
 // added to the accumulators when it is full, and before anything reads them.  With a slab range (s_end >= 0) only
 // those slabs are tabulated, and the caller counts the configuration and flushes (slab-group-major order).
-int accumulate(ul_ctx* c, int s_begin = 0, int s_end = -1) {
+int accumulate(ul_ctx* c, int s_begin, int s_end) {
     NvtxRange range("ul:slab_tables");
     const bool ranged = s_end >= 0;
     if (!ranged) s_end = c->n_slab;
@@ -1085,13 +1109,13 @@ int ul_multilevel(ul_ctx* c, int d, int n_sub, int r_max, const int* fps, int n_
                     ulk::k_set_sweep<<<1, 1, 0, c->stream>>>(c->grp_sweep[k], (uint32_t)(sweep0 & 0xffffffffu), (uint32_t)(sweep0 >> 32));
             c->acc_fresh = true;
             c->n_pending = 0;
+            if (S > 1) {                                               // the whole round is one graph replay
+                rc = round_run(c, d, g0, g1, grp, S, n_sub);
+                if (rc) return bail(rc);
+                continue;
+            }
             for (int j = 0; j < n_sub; ++j) {
-                if (S > 1) {
-                    rc = round_subupdate(c, d, g0, grp, S);
-                    if (rc) return bail(rc);
-                } else {
-                    for (int k = 0; k < c->sub_k; ++k) { rc = compound_direct(c, c->sub_hb, c->sub_or, d, g0, g1); if (rc) return bail(rc); }
-                }
+                for (int k = 0; k < c->sub_k; ++k) { rc = compound_direct(c, c->sub_hb, c->sub_or, d, g0, g1); if (rc) return bail(rc); }
                 rc = accumulate(c, g0, g1);                            // the round's tables while its links are still in L2
                 if (rc) return bail(rc);
                 c->n_pending += 1;
