@@ -1479,9 +1479,10 @@ def test_beta_zero_heatbath_is_uniform_on_device(ul):
 
 
 # ----------------------------------------------------------------------------- slab-group-major order
-@pytest.mark.parametrize("Ns,Nt,d,grp,streams,alg,n_fp", [(8, 8, 2, 1, 1, 0, 0), (8, 12, 2, 4, 1, 0, 3), (6, 8, 4, 1, 1, 1, 2), (16, 16, 2, 3, 1, 0, 0),
-                                                          (8, 16, 2, 2, 2, 0, 0), (8, 12, 2, 1, 4, 1, 2), (16, 16, 2, 3, 2, 0, 3), (8, 8, 4, 1, 3, 0, 0)])
-def test_slab_group_major_order_is_bit_identical(ul, Ns, Nt, d, grp, streams, alg, n_fp):
+@pytest.mark.parametrize("Ns,Nt,d,grp,streams,alg,n_fp,mh", [(8, 8, 2, 1, 1, 0, 0, 0), (8, 12, 2, 4, 1, 0, 3, 0), (6, 8, 4, 1, 1, 1, 2, 0), (16, 16, 2, 3, 1, 0, 0, 0),
+                                                             (8, 16, 2, 2, 2, 0, 0, 0), (8, 12, 2, 1, 4, 1, 2, 0), (16, 16, 2, 3, 2, 0, 3, 0), (8, 8, 4, 1, 3, 0, 0, 0),
+                                                             (8, 12, 2, 2, 2, 0, 2, 1), (8, 8, 2, 1, 4, 0, 0, 1)])
+def test_slab_group_major_order_is_bit_identical(ul, Ns, Nt, d, grp, streams, alg, n_fp, mh):
     """ul_set_slab_group / ul_set_slab_group_streams: the n_sub loop run slab group by slab group (ragged last group, ragged
     last round, ragged last batch), one group after the other or several side by side on their own streams (a round's compound
     sub-update captured as one CUDA graph with a fork and a join), gives the same links, sweep counter, slab sums, C(r) and G
@@ -1495,6 +1496,7 @@ def test_slab_group_major_order_is_bit_identical(ul, Ns, Nt, d, grp, streams, al
         if alg:
             g.set_update_algorithm(1, 1.3)
         g.set_accum_batch(2)
+        g.set_multihit(mh)
         g.set_slab_group(mode)
         g.set_slab_group_streams(streams)
         g.multilevel(d, n_sub, R, fps)
@@ -1504,6 +1506,27 @@ def test_slab_group_major_order_is_bit_identical(ul, Ns, Nt, d, grp, streams, al
     assert np.array_equal(a[0], b[0]) and a[1] == b[1]
     assert np.array_equal(a[2], b[2]) and np.array_equal(a[3], b[3]) and np.array_equal(a[4], b[4])
     assert np.allclose(a[5], b[5], rtol=0, atol=1e-13)
+
+
+def test_default_slab_groups_at_bench_size_are_bit_identical(ul):
+    """64^4, the bench's multilevel call in its default form (rounds of 4 groups x 2 slabs side by side, graph-replayed, heatbath
+    stragglers finished in the kernel) against the one-launch-over-all-slabs form: same links, counter and C(r) bit for bit."""
+    Ns = Nt = 64
+    R = 16
+    g = ul.Lattice(Ns, Nt, 0.98, 5, workspace_bytes=ul.workspace_bytes(Ns, Nt, 2, 0, R, 0))
+    g.sweep(1, 2)
+    g.set_subupdate(1, 4, 1)
+    raw, ctr = g.get_links_raw(), g.get_counter()
+    res = []
+    for mode in (-1, 0):
+        g.set_slab_group(mode)
+        g.set_links_raw(raw)
+        g.set_counter(ctr)
+        n0 = g.launch_count()
+        g.multilevel(2, 9, R)                                      # a full batch and a ragged one
+        res.append((g.get_links_raw(), g.get_counter(), g.read_correlators()[0], g.launch_count() - n0))
+    assert np.array_equal(res[0][0], res[1][0]) and res[0][1] == res[1][1] and np.array_equal(res[0][2], res[1][2])
+    assert res[0][3] > 4 * res[1][3] // 2                           # the grouped form really ran (many small launches)
 
 
 def test_substep_slabs_covers_the_masked_substep(ul):
