@@ -152,8 +152,8 @@ struct ul_ctx {
     int4* grp_queue[8] = {}; int* grp_qcount[8] = {};
     uint32_t* grp_sweep[8] = {};        // per-stream device copies of the sweep counter (graph replays)
     int grp_n = 0;
-    bool hb_local_groups = true;        // ... (UL_NO_HB_LOCAL=1: the group launches use the global queue + straggler kernel)
-    bool hb_local = false;              // heatbath launches finish their stragglers in the kernel (slab-group rounds)
+    bool hb_local_on = true;            // heatbath launches finish their stragglers in the kernel from a shared-memory queue
+                                        // (UL_NO_HB_LOCAL=1, and always with peer halo writes: global queue + k_hb_stragglers)
     int group_streams_n = 4;            // groups side by side per round (ul_set_slab_group's second knob; UL_GROUP_STREAMS)
     std::vector<RoundGraph> round_graphs;
     int dev = 0;              // the CUDA device of this context (entry points switch to it)
@@ -351,7 +351,7 @@ int substep(ul_ctx* c, int kind, int parity, int mu, int slab_d, int s_begin = 0
         c->launches += 1;
         return UL_OK;
     }
-    if (kind == 0 && c->hb_local && !halo) {                      // slab-group launches: stragglers finished inside the kernel
+    if (kind == 0 && c->hb_local_on && !halo) {                   // stragglers finished inside the kernel (ul_persist.cuh)
         cudaError_t el = cudaSuccess;
 #define UL_HBL(MU_, VEC_)                                                                                                     \
         el = c->capturing ? launch_pdl(c, ulk::k_update_hb_local<MU_, VEC_, true>, grid, block, a)                            \
@@ -530,7 +530,6 @@ int round_run(ul_ctx* c, int d, int g0, int g1, int grp, int S, int n_sub) {
         c->capturing = true;
         c->acc_fresh = true; c->n_pending = 0;
         for (int j = 0; j < n_sub && !rc; ++j) {
-            c->hb_local = c->hb_local_groups;
             if (cudaEventRecord(c->grp_ev[0], c->cap_stream) != cudaSuccess) rc = UL_ECUDA;
             for (int k = 0; k < S && !rc; ++k) {
                 const int s0 = g0 + k * grp;
@@ -542,7 +541,6 @@ int round_run(ul_ctx* c, int d, int g0, int g1, int grp, int S, int n_sub) {
                 if (!rc && (cudaEventRecord(c->grp_ev[1 + k], c->grp_stream[k]) != cudaSuccess ||
                             cudaStreamWaitEvent(c->cap_stream, c->grp_ev[1 + k], 0) != cudaSuccess)) rc = UL_ECUDA;
             }
-            c->hb_local = false;
             c->stream = c->cap_stream; c->hb_queue = q0; c->hb_qcount = qc0; c->d_sweep = ds0;
             if (!rc) rc = accumulate(c, g0, g1);                    // the round's tables while its links are still in L2
             if (!rc) {
@@ -551,7 +549,7 @@ int round_run(ul_ctx* c, int d, int g0, int g1, int grp, int S, int n_sub) {
             }
         }
         const cudaError_t ee = cudaStreamEndCapture(c->cap_stream, &graph);
-        c->stream = user; c->hb_queue = q0; c->hb_qcount = qc0; c->d_sweep = ds0; c->capturing = false; c->hb_local = false;
+        c->stream = user; c->hb_queue = q0; c->hb_qcount = qc0; c->d_sweep = ds0; c->capturing = false;
         c->sweep = sweep_keep;
         RoundGraph ng;
         ng.g0 = g0; ng.grp = grp; ng.S = S; ng.n_hb = c->sub_hb; ng.n_or = c->sub_or; ng.sub_k = c->sub_k; ng.slab_d = d; ng.alg = c->alg;
@@ -842,7 +840,7 @@ int create_common(ul_ctx** h, int Ns, int Nt, double beta, uint64_t seed, void* 
     if (cudaMemset(c->hb_qcount, 0, sizeof(int) * (ulk::HB_NQ + 1)) != cudaSuccess) { ul_destroy(c); return fail(nullptr, UL_ECUDA, "memset straggler counters"); }
     c->d_sweep = (uint32_t*)(c->d_bad + 2);
     { const char* e = getenv("UL_NO_ZFLIP"); if (e && e[0] == '1') c->zflip_on = false; }
-    { const char* e = getenv("UL_NO_HB_LOCAL"); if (e && e[0] == '1') c->hb_local_groups = false; }
+    { const char* e = getenv("UL_NO_HB_LOCAL"); if (e && e[0] == '1') c->hb_local_on = false; }
     { const char* e = getenv("UL_GROUP_STREAMS"); if (e) { const int v = atoi(e); c->group_streams_n = v < 1 ? 1 : (v > 8 ? 8 : v); } }
     { const char* e = getenv("UL_OR_TMA"); if (e && e[0] == '1' && 18 * 2 * c->by * c->Nh * 4 <= 200 * 1024) c->or_tma = true; }
     { const char* e = getenv("UL_NO_PDL"); if (e && e[0] == '1') c->use_pdl = false; }

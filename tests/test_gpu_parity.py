@@ -1120,6 +1120,26 @@ def test_graph_replayed_sweeps_equal_directly_launched_substeps(ul, monkeypatch,
         assert np.array_equal(a.get_links_raw(), b.get_links_raw()) and a.get_counter() == b.get_counter()
 
 
+@pytest.mark.parametrize("Ns,Nt", [(16, 4), (8, 8), (6, 4)])
+def test_global_straggler_queue_equals_in_kernel_stragglers(ul, monkeypatch, Ns, Nt):
+    """Heatbath links that rejected both attempts of their first Philox block are finished either by the same thread block
+    from a shared-memory queue (default) or through the striped global queue + k_hb_stragglers (UL_NO_HB_LOCAL=1; always
+    with peer-memory halo writes): same links bit for bit, full and slab-masked, directly launched sub-steps."""
+    a = ul.Lattice(Ns, Nt, 1.0, 17)
+    monkeypatch.setenv("UL_NO_HB_LOCAL", "1")
+    monkeypatch.setenv("UL_NO_PERSIST", "1")
+    b = ul.Lattice(Ns, Nt, 1.0, 17)
+    for L in (a, b):
+        for it in range(3):
+            for d in (0, 2):
+                for parity in (0, 1):
+                    for mu in range(4):
+                        L.substep(0, parity, mu, d)
+                L.set_counter(L.get_counter() + 1)
+    assert b.launch_count() > a.launch_count()                      # (the straggler launches)
+    assert np.array_equal(a.get_links_raw(), b.get_links_raw())
+
+
 def test_tma_staged_overrelaxation_equals_direct_gather(ul, ulo, monkeypatch):
     """The bulk-copy (TMA) staged overrelaxation kernel (UL_OR_TMA=1; ul_update_tma.cuh), the A/B partner of the direct
     gather: same links bit for bit after full and slab-masked sweeps on a lattice whose tiles have its shape (Ns = 64), and one
