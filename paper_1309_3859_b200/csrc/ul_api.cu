@@ -538,11 +538,12 @@ int round_run(ul_ctx* c, int d, int g0, int g1, int grp, int S, int n_sub) {
                 if (cudaStreamWaitEvent(c->grp_stream[k], c->grp_ev[0], 0) != cudaSuccess) { rc = UL_ECUDA; break; }
                 c->stream = c->grp_stream[k]; c->hb_queue = c->grp_queue[k]; c->hb_qcount = c->grp_qcount[k]; c->d_sweep = c->grp_sweep[k];
                 for (int kk = 0; kk < c->sub_k && !rc; ++kk) rc = compound_direct(c, c->sub_hb, c->sub_or, d, s0, s1);
+                if (!rc && deferred) rc = accumulate(c, s0, s1);    // U table only: the group's own table launch, on its stream
                 if (!rc && (cudaEventRecord(c->grp_ev[1 + k], c->grp_stream[k]) != cudaSuccess ||
                             cudaStreamWaitEvent(c->cap_stream, c->grp_ev[1 + k], 0) != cudaSuccess)) rc = UL_ECUDA;
             }
             c->stream = c->cap_stream; c->hb_queue = q0; c->hb_qcount = qc0; c->d_sweep = ds0;
-            if (!rc) rc = accumulate(c, g0, g1);                    // the round's tables while its links are still in L2
+            if (!rc && !deferred) rc = accumulate(c, g0, g1);       // tables with plaquettes (shared partial sums): after the join
             if (!rc) {
                 c->n_pending += 1;
                 if (c->n_pending == c->ws.kb || j == n_sub - 1) rc = flush(c, g0, g1);
