@@ -312,8 +312,9 @@ __global__ void k_set_sweep(uint32_t* sweep, uint32_t lo, uint32_t hi) { sweep[0
 #define UL_HB_MINB 4
 #endif
 #ifndef UL_OR_MINB
-#define UL_OR_MINB 0   // 0 = unspecified
-#endif
+#define UL_OR_MINB 5   // overrelaxation / Metropolis launches over the whole lattice (HBM-bound): 48 registers, 5 blocks per SM (OR sweep
+#endif                 // 440 -> 417 us on 64^4); the graph-replayed launches (DEVCTR: small lattices, slab groups out of L2) are left to
+                       // the compiler (46-62 registers, 4 blocks: measured 1-5 % faster there than with the cap)
 // One tile (= one thread block's worth) of a sub-step: tile coordinates (tx, ty, tz) of a (gx, gy, ntz) tile grid, blk = the
 // tile's linear index (picks the straggler sub-queue).
 template <int KIND, int MU, int VEC, bool COH, bool PDL>
@@ -361,7 +362,7 @@ __device__ __forceinline__ void update_tile(const UpdateArgs& P, const int tx, c
 }
 
 template <int KIND, int MU, int VEC, bool DEVCTR>
-__global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : UL_OR_MINB) k_update(const UpdateArgs P) {
+__global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : (DEVCTR ? 0 : UL_OR_MINB)) k_update(const UpdateArgs P) {
     // the sweep counter: a kernel argument (uniform registers), or, for launches replayed from a CUDA graph, device memory
     const uint32_t sweep_lo = DEVCTR ? __ldg(P.sweep_dev) : P.sweep_lo, sweep_hi = DEVCTR ? __ldg(P.sweep_dev + 1) : P.sweep_hi;
     update_tile<KIND, MU, VEC, false, true>(P, blockIdx.x, blockIdx.y, blockIdx.z, gridDim.z, blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z),
