@@ -311,6 +311,9 @@ __global__ void k_set_sweep(uint32_t* sweep, uint32_t lo, uint32_t hi) { sweep[0
 #ifndef UL_HB_MINB
 #define UL_HB_MINB 4
 #endif
+#ifndef UL_ORG_MINB
+#define UL_ORG_MINB 3   // graph-replayed overrelaxation launches (small lattices, slab groups out of L2): up to 80 registers, 3 blocks per SM
+#endif
 #ifndef UL_OR_MINB
 #define UL_OR_MINB 5   // overrelaxation / Metropolis launches over the whole lattice (HBM-bound): 48 registers, 5 blocks per SM (OR sweep
 #endif                 // 440 -> 417 us on 64^4); the graph-replayed launches (DEVCTR: small lattices, slab groups out of L2) are left to
@@ -362,7 +365,7 @@ __device__ __forceinline__ void update_tile(const UpdateArgs& P, const int tx, c
 }
 
 template <int KIND, int MU, int VEC, bool DEVCTR>
-__global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : (DEVCTR ? 0 : UL_OR_MINB)) k_update(const UpdateArgs P) {
+__global__ void __launch_bounds__(256, KIND == 0 ? UL_HB_MINB : (DEVCTR ? UL_ORG_MINB : UL_OR_MINB)) k_update(const UpdateArgs P) {
     // the sweep counter: a kernel argument (uniform registers), or, for launches replayed from a CUDA graph, device memory
     const uint32_t sweep_lo = DEVCTR ? __ldg(P.sweep_dev) : P.sweep_lo, sweep_hi = DEVCTR ? __ldg(P.sweep_dev + 1) : P.sweep_hi;
     update_tile<KIND, MU, VEC, false, true>(P, blockIdx.x, blockIdx.y, blockIdx.z, gridDim.z, blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z),
