@@ -217,6 +217,16 @@ int ul_set_accum_batch(ul_ctx* h, int depth);
 /* Mean of cos theta_P (Eq. 6) over all 6V plaquettes, over the 3V time-like and the
  * 3V space-like ones: HOST double[3].  Synchronises. */
 int ul_plaquette(ul_ctx* h, double* mean_cos);
+/* The same numbers (bit for bit: same kernels, same order of additions) for callers that must not allocate -- code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Input: the handle's current links; output:
+ * DEVICE double[3] (caller-owned), written asynchronously on the handle's stream (no synchronisation, no host copy).
+ * Calls no cudaMalloc / cudaFree / allocating routine: the block partials live in a fixed file-scope device array of
+ * 2 * 592 + 4 doubles (9.5 KB, held by every GPU that loads the library until exit).  Limit: ceil(Ns^2 / 256) <= 592,
+ * i.e. Ns <= 389 (any Nt); beyond it UL_EINVAL with a message that says so.  The first call on a device looks the array's
+ * address up (cudaGetSymbolAddress: make one call outside capture first).  EVERY call on a device, of any handle, shares
+ * that array, which keeps the last call's contents (each call overwrites all it reads, nothing needs clearing): calls that
+ * can overlap on the GPU (different streams) race -- order them.  UL_EINVAL: null pointers, device index beyond 63. */
+int ul_plaquette_noalloc(ul_ctx* h, double* dev_mean_cos);
 
 /* Polyakov-loop average <P> = (1/Ns^3) sum_x prod_t U_0(x,t) (Eqs. 15-16): HOST double[2] = (Re, Im).
  * multihit = 1: analytic multihit, every temporal link replaced by its mean over its local weight with the

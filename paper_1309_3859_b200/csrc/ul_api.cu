@@ -1494,6 +1494,44 @@ int ul_plaquette(ul_ctx* c, double* out) {
     out[0] = 0.5 * (v[0] + v[1]); out[1] = v[0]; out[2] = v[1];
     return UL_OK;
 }
+// ---- the plaquette average without any allocation (include/ul.h: ul_plaquette_noalloc) -------------------------------------
+// The block partials and the two sums of k_plaquette / k_sum_partials live in a file-scope device array instead of the
+// cudaMalloc'ed scratch of the handle: 2 NBLK + 4 doubles = 9.5 KB, held by every GPU that loads the library until it exits.
+// In host code the NAME of the array is a host-side stand-in, not a device address: the address the kernels get comes from
+// cudaGetSymbolAddress, taken once per device with that device current (device code of this file could name the array directly).
+static __device__ __align__(256) double g_plaq_scratch[2 * NBLK + 4];
+static double* g_plaq_scratch_ptr[64] = {};                        // per device, resolved on the first call for that device
+
+// (mean over all, time-like, space-like) from the two sums; out = caller's device buffer
+static __global__ void k_plaquette_out(const double* __restrict__ sums, double* __restrict__ out) {
+    if (threadIdx.x == 0) { const double t = sums[0], sp = sums[1]; out[0] = 0.5 * (t + sp); out[1] = t; out[2] = sp; }
+}
+
+int ul_plaquette_noalloc(ul_ctx* c, double* dev_out) {
+    if (!c || !dev_out) return fail(c, UL_EINVAL, "null pointer");
+    if (c->dev < 0 || c->dev >= 64) return fail(c, UL_EINVAL, "ul_plaquette_noalloc: device index beyond 63");
+    // the fixed scratch holds one partial per block and sum, at most NBLK blocks: ceil(Ns^2 / 256) <= NBLK, i.e. Ns <= 389
+    const int gx = (c->Ns * c->Ns + 255) / 256, rows = c->Nt * c->Ns;
+    if (gx > NBLK)
+        return fail(c, UL_EINVAL, "ul_plaquette_noalloc: lattice beyond the fixed scratch (need ceil(Ns^2 / 256) <= 592 blocks, i.e. Ns <= 389)");
+    const int gy = rows < NBLK / gx ? rows : NBLK / gx;             // gx gy <= NBLK
+    DeviceGuard guard(c);                                            // the context's device is current from here on
+    double* scratch = g_plaq_scratch_ptr[c->dev];
+    if (!scratch) {                                                  // set-up, once per device: no allocation, a symbol lookup
+        void* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_plaq_scratch);
+        if (e != cudaSuccess || !p) return fail(c, UL_ECUDA, std::string("cudaGetSymbolAddress(g_plaq_scratch): ") + cudaGetErrorString(e));
+        scratch = g_plaq_scratch_ptr[c->dev] = (double*)p;
+    }
+    // every element read below is written by this call first (gx gy partials per sum, then the two sums), so nothing has to
+    // start at zero although the array keeps the last call's contents
+    ulk::k_plaquette<<<dim3(gx, gy), 256, 0, c->stream>>>(geom(c), c->th, scratch);
+    ulk::k_sum_partials<<<2, 256, 0, c->stream>>>(scratch, gx * gy, scratch + 2 * NBLK, 1.0 / (3.0 * (double)c->V), 0);
+    k_plaquette_out<<<1, 32, 0, c->stream>>>(scratch + 2 * NBLK, dev_out);
+    UL_CUDA(c, cudaGetLastError());
+    c->launches += 3;
+    return UL_OK;
+}
 int ul_polyakov(ul_ctx* c, int multihit, double* out) {
     if (!c || !out || (multihit != 0 && multihit != 1)) return fail(c, UL_EINVAL, "multihit must be 0 or 1");
     DeviceGuard guard(c);

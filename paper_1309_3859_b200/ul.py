@@ -19,7 +19,7 @@ SYMBOLS = [
     "ul_create", "ul_create_ext", "ul_workspace_bytes", "ul_destroy", "ul_init", "ul_set_beta",
     "ul_set_links", "ul_get_links", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep", "ul_substep_slabs", "ul_set_slab_group", "ul_set_slab_group_streams",
     "ul_set_subupdate", "ul_set_update_algorithm", "ul_multilevel", "ul_multilevel_replay", "ul_workspace_bytes_replay", "ul_multilevel2_replay", "ul_workspace_bytes_replay2", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
-    "ul_measure_end", "ul_measure2_begin", "ul_combine", "ul_measure2_end", "ul_set_accum_batch", "ul_set_multihit", "ul_plaquette", "ul_polyakov", "ul_set_site_offset", "ul_slab_partial_product", "ul_combine_partial_products", "ul_set_halo_peers", "ul_halo_flags", "ul_set_halo_peer_flags", "ul_ipc_export", "ul_ipc_open", "ul_read_correlators", "ul_read_slab_averages",
+    "ul_measure_end", "ul_measure2_begin", "ul_combine", "ul_measure2_end", "ul_set_accum_batch", "ul_set_multihit", "ul_plaquette", "ul_plaquette_noalloc", "ul_polyakov", "ul_set_site_offset", "ul_slab_partial_product", "ul_combine_partial_products", "ul_set_halo_peers", "ul_halo_flags", "ul_set_halo_peer_flags", "ul_ipc_export", "ul_ipc_open", "ul_read_correlators", "ul_read_slab_averages",
     "ul_get_launch_count", "ul_philox_selftest", "ul_sync", "ul_last_error",
 ]
 
@@ -88,6 +88,7 @@ def lib():
         L.ul_combine.argtypes = [P]
         L.ul_measure2_end.argtypes = [P]
         L.ul_plaquette.argtypes = [P, P]
+        L.ul_plaquette_noalloc.argtypes = [P, P]
         L.ul_read_correlators.argtypes = [P, P, P, P]
         L.ul_read_slab_averages.argtypes = [P, P]
         L.ul_get_launch_count.argtypes = [P, C.POINTER(C.c_uint64)]
@@ -289,6 +290,13 @@ class Lattice:
     def plaquette(self):
         out = np.zeros(3)
         self._ck(lib().ul_plaquette(self._h, _ptr(out)))
+        return out
+
+    def plaquette_noalloc(self, out):
+        """out: caller's float64 CUDA tensor of 3 elements; written asynchronously on the lattice's stream (ul_plaquette_noalloc)."""
+        if not out.is_cuda or out.dtype != self._torch.float64 or out.numel() < 3 or not out.is_contiguous():
+            raise ValueError("out must be a contiguous float64 CUDA tensor with 3 elements")
+        self._ck(lib().ul_plaquette_noalloc(self._h, C.c_void_p(out.data_ptr())))
         return out
 
     def read_correlators(self):
