@@ -1528,6 +1528,28 @@ def test_slab_group_major_order_is_bit_identical(ul, Ns, Nt, d, grp, streams, al
     assert np.allclose(a[5], b[5], rtol=0, atol=1e-13)
 
 
+def test_slab_group_rounds_follow_a_changed_measurement(ul):
+    """The captured rounds are keyed by everything their launches were recorded with: a second measurement with another r_max
+    (the library-owned workspace grows and moves), another n_sub, another beta and another sub-update recipe must not replay a
+    stale graph: every call equals the one-launch form bit for bit."""
+    Ns, Nt, d = 8, 16, 2
+    res = {}
+    for mode in (0, 2):
+        g = ul.Lattice(Ns, Nt, 1.0, 23)
+        g.sweep(2, 2)
+        g.set_slab_group(mode)
+        g.set_slab_group_streams(2)
+        out = []
+        for R, n_sub, beta, recipe in ((2, 5, 1.0, (1, 3)), (4, 5, 1.0, (1, 3)), (4, 3, 0.9, (1, 3)), (3, 9, 0.9, (2, 1)), (2, 5, 1.0, (1, 3))):
+            g.set_beta(beta)
+            g.set_subupdate(*recipe, 1)
+            g.multilevel(d, n_sub, R)
+            out.append((g.get_links_raw(), g.get_counter(), g.read_correlators()[0]))
+        res[mode] = out
+    for a, b in zip(res[0], res[2]):
+        assert np.array_equal(a[0], b[0]) and a[1] == b[1] and np.array_equal(a[2], b[2])
+
+
 def test_default_slab_groups_at_bench_size_are_bit_identical(ul):
     """64^4, the bench's multilevel call in its default form (rounds of 4 groups x 2 slabs side by side, graph-replayed, heatbath
     stragglers finished in the kernel) against the one-launch-over-all-slabs form: same links, counter and C(r) bit for bit."""
