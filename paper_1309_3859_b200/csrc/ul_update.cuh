@@ -87,14 +87,14 @@ __device__ __forceinline__ void load_row(const int* __restrict__ th, int idx, co
     }
     if (D1 > 0) {
         if (OFF) {                                    // shift by +1: need element h0 + VEC
-            const int x = ld1<COH>(th + idx + st.dxp);
+            const int x = ld1<COH>(th + (idx + st.dxp));
 #pragma unroll
             for (int i = 0; i < VEC - 1; ++i) v[i] = v[i + 1];
             v[VEC - 1] = x;
         }
     } else if (D1 < 0) {
         if (!OFF) {                                   // shift by -1: need element h0 - 1
-            const int x = ld1<COH>(th + idx + st.dxm);
+            const int x = ld1<COH>(th + (idx + st.dxm));
 #pragma unroll
             for (int i = VEC - 1; i > 0; --i) v[i] = v[i - 1];
             v[0] = x;
@@ -181,8 +181,14 @@ __device__ __forceinline__ void update_links(const UpdateArgs& P, const Site& st
         else if (VEC == 2) { const int2 q = COH ? __ldcg(reinterpret_cast<const int2*>(own)) : *reinterpret_cast<const int2*>(own); old[0] = q.x; old[1 % VEC] = q.y; }
         else old[0] = COH ? __ldcg(own) : own[0];
 #pragma unroll
-        for (int i = 0; i < VEC; ++i)                 // overrelaxation (O2): theta' = 2 alpha - theta, exact mod 2 pi
-            out[i] = (int)(2u * (unsigned)ulm::atan2_bt(Sy[i], Sx[i]) - (unsigned)old[i]);
+        for (int i = 0; i < VEC; i += 2) {            // overrelaxation (O2): theta' = 2 alpha - theta, exact mod 2 pi
+            int al[2];
+            if (i + 1 < VEC) ulm::atan2_bt2(Sy[i], Sx[i], Sy[(i + 1) % VEC], Sx[(i + 1) % VEC], al[0], al[1]);   // two links per FFMA2
+            else al[0] = ulm::atan2_bt(Sy[i], Sx[i]);
+#pragma unroll
+            for (int j = 0; j < 2 && i + j < VEC; ++j)
+                out[(i + j) % VEC] = (int)(2u * (unsigned)al[j] - (unsigned)old[(i + j) % VEC]);
+        }
     } else if (KIND == 2) {
         // Metropolis (DESIGN R21): one hit, theta' = theta + delta (2 u1 - 1), accept iff
         // u2 <= exp(beta k [cos(theta' - alpha) - cos(theta - alpha)]).  With d = theta' - theta (an exact integer
@@ -331,7 +337,10 @@ __device__ __forceinline__ void update_tile(const UpdateArgs& P, const int tx, c
     int t = (P.zflip ? ntz - 1 - tz : tz) + P.z0;
     if (MU != 0 && P.slab_d > 0) {                    // enumerate only the non-frozen layers
         const int dm = P.slab_d - 1;
-        const int s = t / dm;
+        // s = t / dm without the ~25 instructions of an integer division in every thread: nothing to do at thickness 2;
+        // otherwise the truncated float quotient of t + 1/2, exact while t dm < 2^21 (the fractional part of (t + 1/2) / dm
+        // is at least 1 / (2 dm) away from an integer, the approximate division is off by < 2^-21 relative)
+        const int s = dm == 1 ? t : __float2int_rz(__fdividef(__int2float_rn(t) + 0.5f, __int2float_rn(dm)));
         t = s * P.slab_d + 1 + (t - s * dm);
     }
     const int p = P.parity;
