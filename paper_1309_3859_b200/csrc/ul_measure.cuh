@@ -457,23 +457,30 @@ __global__ void __launch_bounds__(256, FIELD ? UL_ACCF_MINB : UL_ACC_MINB) k_acc
     const long long idx = P.idx0 + (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= P.idx0 + P.n_idx) return;
     const int s = (int)(idx / g.Vs);
-    const int xs = (int)(idx - (long long)s * g.Vs);
+    const int xs_lin = (int)(idx - (long long)s * g.Vs);
     const int Ns = g.Ns;
-    int x[4];
-    x[0] = 0;
-    x[1] = xs % Ns;
-    x[2] = (xs / Ns) % Ns;
-    x[3] = xs / (Ns * Ns);
     const int stride[4] = {0, 1, Ns, Ns * Ns};
     const double2* __restrict__ Us = P.U + (long long)s * g.Vs;
     const long long stepA = (long long)P.n_slab * g.Vs;                  // A[mu][r] -> A[mu][r+1]
-    double2 u0[KB];
-#pragma unroll
-    for (int k = 0; k < KB; ++k)
-        if (FULL || k < P.nk) u0[k] = Us[k * n + xs];
 #pragma unroll
     for (int mu = 1; mu <= 3; ++mu) {
         const int nu = 1 + (mu % 3), rho = 1 + ((mu + 1) % 3);
+        // The site this thread owns for the charge axis mu.  For mu = 3 it is the thread's linear site with x2 and x3 exchanged
+        // (a bijection of the slab's sites), so that the consecutive x2 rows of a thread block become consecutive x3 rows: the
+        // rows U(x + r 3^) a block reads are then shared between its rows through L1, as they are for mu = 2 (without the
+        // exchange every one of them is read from L2 once per row and separation: half of the kernel's L2 traffic).  Every
+        // accumulator entry still sees the same additions in the same order.
+        int x[4];
+        x[0] = 0;
+        x[1] = xs_lin % Ns;
+        x[2] = (xs_lin / Ns) % Ns;
+        x[3] = xs_lin / (Ns * Ns);
+        if (mu == 3) { const int t_ = x[2]; x[2] = x[3]; x[3] = t_; }
+        const int xs = x[1] + Ns * (x[2] + Ns * x[3]);
+        double2 u0[KB];
+#pragma unroll
+        for (int k = 0; k < KB; ++k)
+            if (FULL || k < P.nk) u0[k] = Us[k * n + xs];
         double2* Ap = P.A + (((long long)(mu - 1) * P.r_max + (P.r_begin - 1)) * P.n_slab + s) * g.Vs + xs;
         // the accumulator entries of the NEXT step are requested before the current ones are worked on (software pipelining:
         // the kernel is bound by the latency of these reads, not by bandwidth or arithmetic)
