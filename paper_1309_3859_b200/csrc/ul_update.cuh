@@ -339,9 +339,10 @@ __device__ __forceinline__ void update_tile(const UpdateArgs& P, const int tx, c
     if (MU != 0 && P.slab_d > 0) {                    // enumerate only the non-frozen layers
         const int dm = P.slab_d - 1;
         // s = t / dm without the ~25 instructions of an integer division in every thread: nothing to do at thickness 2;
-        // otherwise the truncated float quotient of t + 1/2, exact while t dm < 2^21 (the fractional part of (t + 1/2) / dm
-        // is at least 1 / (2 dm) away from an integer, the approximate division is off by < 2^-21 relative)
-        const int s = dm == 1 ? t : __float2int_rz(__fdividef(__int2float_rn(t) + 0.5f, __int2float_rn(dm)));
+        // otherwise the truncated float quotient of t + 1/2, exact for t < 2^20 (the fractional part of (t + 1/2) / dm is
+        // at least 1 / (2 dm) away from an integer, the approximate quotient is off by < 2^-21 (t / dm)); beyond that
+        // (no lattice that fits a GPU has 2^20 time layers) the division
+        const int s = dm == 1 ? t : (t < (1 << 20) ? __float2int_rz(__fdividef(__int2float_rn(t) + 0.5f, __int2float_rn(dm))) : t / dm);
         t = s * P.slab_d + 1 + (t - s * dm);
     }
     const int p = P.parity;

@@ -1457,10 +1457,12 @@ def test_two_processes_on_one_gpu_sharded_multilevel_and_sweeps(ul, tmp_path):
 
 
 # ----------------------------------------------------------------------------- degenerate and extreme shapes
-@pytest.mark.parametrize("Ns,Nt,d", [(2, 2, 2), (2, 4, 1), (4, 2, 2), (6, 6, 6), (4, 8, 8), (10, 4, 2)])
+@pytest.mark.parametrize("Ns,Nt,d", [(2, 2, 2), (2, 4, 1), (4, 2, 2), (6, 6, 6), (4, 8, 8), (10, 4, 2), (4, 12, 3), (4, 30, 5), (4, 24, 8),
+                                     (2, 126, 7)])
 def test_degenerate_shapes_against_oracle(ul, ulo, Ns, Nt, d):
     """Smallest lattice (2^4 sites wrap onto themselves), a single slab (d = Nt), thickness 1 (every spatial link
-    frozen), r_max = Ns/2 (the largest separation), rows that are not a multiple of the vector width (Ns = 6, 10):
+    frozen), several slabs of thickness 3, 5, 7, 8 (the masked spatial launches enumerate the d - 1 non-frozen layers of every
+    slab), r_max = Ns/2 (the largest separation), rows that are not a multiple of the vector width (Ns = 6, 10):
     one heatbath and one overrelaxation sweep link by link, then the frozen-configuration estimator, stored and replay."""
     beta, R = 0.9, Ns // 2
     o = ulo.Oracle(Ns, Nt, beta, 8)
