@@ -9,7 +9,7 @@ One STEP = one pass of the whole hot path over a 64^4 lattice (beta = 0.98, hot 
                                               + T^(2) accumulation}, slab product, reduction (a6, a7, a10, a13)
     ul_plaquette()                                                          (row a11)
 metric = link updates per second (full + masked updates) over the whole step, inputs resident in HBM.
-`e2e` = the same step through the C ABI with HOST link buffers (ul_set_links + step + ul_get_links).
+`e2e` = the same step through the C ABI with HOST link buffers (ul_set_links + step + ul_get_links_async, waited for at the end).
 `roofline` = the overrelaxation sub-step kernel (4 of every 5 sweeps), timed with CUDA events inside
 the timed region, against its algorithmic 36 B per link update.
 `cpu_baseline` = the oracle (oracle/ulo.cpp, single thread) on a bounded sample of the same workload: one slab-masked
@@ -254,15 +254,20 @@ def run_ours(args, rank, local_rank, world):
     host_out = torch.empty(4 * V, dtype=torch.float32).pin_memory()
     lat.get_links(host_in)
     e2e_steps = max(2, min(args.steps, 5))
+    # every step: its links host -> device (pinned), the step, its links device -> host and the correlators; the read-back is
+    # ul_get_links_async, so that it shares the host link with the next step's ul_set_links (the last one is waited for inside
+    # the timed region)
     for _ in range(2):
-        lat.set_links(host_in); step(); lat.get_links(host_out)
+        lat.set_links(host_in); step(); lat.get_links_async(host_out)
+    lat.get_links_wait()
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         lat.set_links(host_in)
         step()
-        lat.get_links(host_out)
+        lat.get_links_async(host_out)
         lat.read_correlators()
+    lat.get_links_wait()
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3
     if dist is not None:

@@ -72,6 +72,16 @@ int ul_set_beta(ul_ctx* h, double beta);
 int ul_set_links(ul_ctx* h, const float* host_links);
 int ul_get_links(ul_ctx* h, float* host_links);
 
+/* ul_get_links without waiting for the copy (row a1; a serving loop that reads every configuration back): the
+ * canonical copy is formed on the context's stream into a library-owned device buffer of its own (4 V floats, allocated on
+ * the first call) and copied to host_links on a second stream, so it runs beside whatever is enqueued next, e.g. the
+ * ul_set_links of the next configuration (both directions of the host link busy at once).  host_links is caller-owned,
+ * should be pinned (with pageable memory the call itself waits), and must not be read or freed before ul_get_links_wait
+ * returns UL_OK.  A second call before the wait is allowed: it waits on the stream for the first copy (the buffer is
+ * reused), so one wait covers both.  UL_EINVAL on null pointers, UL_ECUDA on a CUDA failure. */
+int ul_get_links_async(ul_ctx* h, float* host_links);
+int ul_get_links_wait(ul_ctx* h);
+
 /* The same arrays as raw binary angles, HOST int32[4][Nt][Ns][Ns][Ns], bit for bit: the exact
  * state for checkpoint / resume (with ul_get_counter / ul_set_counter and the seed). */
 int ul_set_links_raw(ul_ctx* h, const int32_t* host_links);

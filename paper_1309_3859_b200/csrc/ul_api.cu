@@ -186,6 +186,11 @@ struct ul_ctx {
     int slab_group = -1;     // ul_set_slab_group: slabs per group of the slab-group-major sub-update loop (0 = off, -1 = auto)
     bool skip_colsum = false; // replayed configurations: their plaquette column sums are already in the vacuum sums
     float* staging2 = nullptr; // second configuration copy (two-level replay)
+    float* staging_out = nullptr;        // ul_get_links_async: its own canonical copy, a copy stream and two events, so that the
+    cudaStream_t copy_stream = nullptr;  // device-to-host copy runs beside whatever the caller enqueues next (ul_set_links of the
+    cudaEvent_t ev_repacked = nullptr;   // next configuration: both directions of the link to the host are busy at once)
+    cudaEvent_t ev_out_done = nullptr;
+    bool out_pending = false;
     char* plane_buf = nullptr; // full-plane maps through the transverse DFT: Ohat, group partials, Ghat (library-owned)
     size_t plane_bytes = 0;
     bool plane_fresh = true;   // Ghat holds nothing yet
@@ -916,6 +921,10 @@ int ul_destroy(ul_ctx* c) {
     if (c->own_work && c->work) cudaFree(c->work);
     if (c->staging) cudaFree(c->staging);
     if (c->staging2) cudaFree(c->staging2);
+    if (c->copy_stream) { cudaStreamSynchronize(c->copy_stream); cudaStreamDestroy(c->copy_stream); }
+    if (c->ev_repacked) cudaEventDestroy(c->ev_repacked);
+    if (c->ev_out_done) cudaEventDestroy(c->ev_out_done);
+    if (c->staging_out) cudaFree(c->staging_out);
     if (c->plane_buf) cudaFree(c->plane_buf);
     if (c->scratch) cudaFree(c->scratch);
     if (c->hb_queue) cudaFree(c->hb_queue);
@@ -992,6 +1001,39 @@ static int links_out(ul_ctx* c, void* host, int mode) {
     c->launches += 1;
     UL_CUDA(c, cudaMemcpyAsync(host, c->staging, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, c->stream));
     UL_CUDA(c, cudaStreamSynchronize(c->stream));
+    return UL_OK;
+}
+// The read-back without waiting for it: repack on the context's stream into a buffer of its own, the copy to the host on a
+// second stream behind an event.  A following call waits (on the stream) for the previous copy before it overwrites the buffer.
+int ul_get_links_async(ul_ctx* c, float* host) {
+    if (!c || !host) return fail(c, UL_EINVAL, "null pointer");
+    DeviceGuard guard(c);
+    const long long n = 4 * c->V;
+    if (!c->staging_out) {
+        void* p = nullptr;
+        UL_CUDA(c, cudaMalloc(&p, sizeof(float) * (size_t)n));
+        c->staging_out = (float*)p;
+        UL_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        UL_CUDA(c, cudaEventCreateWithFlags(&c->ev_repacked, cudaEventDisableTiming));
+        UL_CUDA(c, cudaEventCreateWithFlags(&c->ev_out_done, cudaEventDisableTiming));
+    }
+    if (c->out_pending) UL_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_out_done, 0));
+    ulk::k_repack<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(geom(c), c->th, c->staging_out, 0, c->d_bad);
+    UL_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    UL_CUDA(c, cudaEventRecord(c->ev_repacked, c->stream));
+    UL_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->ev_repacked, 0));
+    UL_CUDA(c, cudaMemcpyAsync(host, c->staging_out, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, c->copy_stream));
+    UL_CUDA(c, cudaEventRecord(c->ev_out_done, c->copy_stream));
+    c->out_pending = true;
+    return UL_OK;
+}
+int ul_get_links_wait(ul_ctx* c) {
+    if (!c) return fail(c, UL_EINVAL, "null handle");
+    if (!c->out_pending) return UL_OK;
+    DeviceGuard guard(c);
+    UL_CUDA(c, cudaEventSynchronize(c->ev_out_done));
+    c->out_pending = false;
     return UL_OK;
 }
 int ul_set_links(ul_ctx* c, const float* host) { return links_in(c, host, 1); }

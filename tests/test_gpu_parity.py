@@ -1456,6 +1456,39 @@ def test_two_processes_on_one_gpu_sharded_multilevel_and_sweeps(ul, tmp_path):
         assert line == f"RESULT {r} True True True True", (line, outs[r][1][-2000:])
 
 
+# ----------------------------------------------------------------------------- asynchronous read-back
+def test_get_links_async_equals_get_links(ul):
+    """ul_get_links_async / ul_get_links_wait return the same bytes as ul_get_links: one call, two calls before one wait (the
+    second waits on the stream for the first copy), and a call overtaken by the next ul_set_links and sweeps (the copy reads its
+    own buffer, not the link array that is being overwritten)."""
+    import torch
+    Ns, Nt = 16, 8
+    g = ul.Lattice(Ns, Nt, 0.99, 17)
+    g.sweep(1, 2)
+    want = g.get_links()
+    a = torch.empty(4 * g.V, dtype=torch.float32).pin_memory()
+    b = torch.empty(4 * g.V, dtype=torch.float32).pin_memory()
+    g.get_links_async(a)
+    g.get_links_wait()
+    assert np.array_equal(a.numpy().reshape(want.shape), want)
+    g.get_links_wait()                                              # nothing pending: returns at once
+    a.zero_()
+    g.get_links_async(a)
+    g.sweep(1, 1)
+    want2 = g.get_links()
+    g.get_links_async(b)                                            # second call before the wait
+    g.set_links(want)                                               # overtakes the copies
+    g.sweep(0, 3)
+    g.get_links_wait()
+    assert np.array_equal(a.numpy().reshape(want.shape), want)
+    assert np.array_equal(b.numpy().reshape(want.shape), want2)
+    c = np.empty(4 * g.V, dtype=np.float32)                         # pageable memory: still correct
+    g.set_links(want2)
+    g.get_links_async(torch.from_numpy(c))
+    g.get_links_wait()
+    assert np.array_equal(c.reshape(want.shape), want2)
+
+
 # ----------------------------------------------------------------------------- degenerate and extreme shapes
 @pytest.mark.parametrize("Ns,Nt,d", [(2, 2, 2), (2, 4, 1), (4, 2, 2), (6, 6, 6), (4, 8, 8), (10, 4, 2), (4, 12, 3), (4, 30, 5), (4, 24, 8),
                                      (2, 126, 7)])
