@@ -9,7 +9,7 @@ One STEP = one pass of the whole hot path over a 64^4 lattice (beta = 0.98, hot 
                                               + T^(2) accumulation}, slab product, reduction (a6, a7, a10, a13)
     ul_plaquette()                                                          (row a11)
 metric = link updates per second (full + masked updates) over the whole step, inputs resident in HBM.
-`e2e` = the same step through the C ABI with HOST link buffers (ul_set_links + step + ul_get_links_async, waited for at the end).
+`e2e` = the same step through the C ABI with HOST link buffers (ul_set_links_async / _commit + step + ul_get_links_async: the copies of neighbouring steps overlap the work).
 `roofline` = the overrelaxation sub-step kernel (4 of every 5 sweeps), timed with CUDA events inside
 the timed region, against its algorithmic 36 B per link update.
 `cpu_baseline` = the oracle (oracle/ulo.cpp, single thread) on a bounded sample of the same workload: one slab-masked
@@ -253,20 +253,25 @@ def run_ours(args, rank, local_rank, world):
     host_in = torch.empty(4 * V, dtype=torch.float32).pin_memory()
     host_out = torch.empty(4 * V, dtype=torch.float32).pin_memory()
     lat.get_links(host_in)
-    e2e_steps = max(2, min(args.steps, 5))
+    e2e_steps = max(2, min(args.steps, 20))
     # every step: its links host -> device (pinned), the step, its links device -> host and the correlators; the read-back is
     # ul_get_links_async, so that it shares the host link with the next step's ul_set_links (the last one is waited for inside
     # the timed region)
+    # the upload of a step's links is ul_set_links_async + ul_set_links_commit: the copy of step i + 1 is started before step i
+    # runs (on the library's upload stream) and committed when step i is over, so e2e_steps + 1 uploads are inside the timed
+    # region for e2e_steps steps
     for _ in range(2):
         lat.set_links(host_in); step(); lat.get_links_async(host_out)
     lat.get_links_wait()
     barrier()
     t0 = time.perf_counter()
+    lat.set_links_async(host_in)
     for _ in range(e2e_steps):
-        lat.set_links(host_in)
+        lat.set_links_commit()
+        lat.set_links_async(host_in)                  # the next step's input
         step()
+        lat.read_correlators()                        # before the read-back of the links: a small copy queues behind a large one
         lat.get_links_async(host_out)
-        lat.read_correlators()
     lat.get_links_wait()
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3

@@ -82,6 +82,16 @@ int ul_get_links(ul_ctx* h, float* host_links);
 int ul_get_links_async(ul_ctx* h, float* host_links);
 int ul_get_links_wait(ul_ctx* h);
 
+/* ul_set_links in two parts, for the same loop: ul_set_links_async copies host_links (caller-owned, pinned, untouched until
+ * the commit returns) into a library-owned device buffer of its own (4 V floats, allocated on the first call) on a second
+ * stream -- nothing the context's stream is doing is touched, so the upload of the NEXT configuration runs beside the work on
+ * the current one; ul_set_links_commit then makes it the configuration: the repack and the validation of ul_set_links on the
+ * context's stream, behind the upload (its validation flag sits in mapped host memory: reading it queues no copy behind a
+ * ul_get_links_async still in flight).  A second ul_set_links_async before the commit replaces the first.  ul_set_links_commit
+ * returns UL_ESTATE without a pending upload, UL_EINVAL for an invalid angle (as ul_set_links; the links are then undefined). */
+int ul_set_links_async(ul_ctx* h, const float* host_links);
+int ul_set_links_commit(ul_ctx* h);
+
 /* The same arrays as raw binary angles, HOST int32[4][Nt][Ns][Ns][Ns], bit for bit: the exact
  * state for checkpoint / resume (with ul_get_counter / ul_set_counter and the seed). */
 int ul_set_links_raw(ul_ctx* h, const int32_t* host_links);

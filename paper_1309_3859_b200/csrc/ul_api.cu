@@ -191,6 +191,12 @@ struct ul_ctx {
     cudaEvent_t ev_repacked = nullptr;   // next configuration: both directions of the link to the host are busy at once)
     cudaEvent_t ev_out_done = nullptr;
     bool out_pending = false;
+    float* staging_in = nullptr;         // ul_set_links_async: the upload of the NEXT configuration on a stream of its own while the
+    cudaStream_t in_stream = nullptr;    // current one is being worked on; ul_set_links_commit turns it into the link array
+    cudaEvent_t ev_in_done = nullptr;
+    bool in_pending = false;
+    int* bad_host = nullptr;             // the validation flag of ul_set_links_commit in mapped pinned host memory: reading it back must
+    int* bad_dev = nullptr;              // not queue a copy behind a ul_get_links_async that is still using the copy engine
     char* plane_buf = nullptr; // full-plane maps through the transverse DFT: Ohat, group partials, Ghat (library-owned)
     size_t plane_bytes = 0;
     bool plane_fresh = true;   // Ghat holds nothing yet
@@ -925,6 +931,10 @@ int ul_destroy(ul_ctx* c) {
     if (c->ev_repacked) cudaEventDestroy(c->ev_repacked);
     if (c->ev_out_done) cudaEventDestroy(c->ev_out_done);
     if (c->staging_out) cudaFree(c->staging_out);
+    if (c->in_stream) { cudaStreamSynchronize(c->in_stream); cudaStreamDestroy(c->in_stream); }
+    if (c->ev_in_done) cudaEventDestroy(c->ev_in_done);
+    if (c->staging_in) cudaFree(c->staging_in);
+    if (c->bad_host) cudaFreeHost(c->bad_host);
     if (c->plane_buf) cudaFree(c->plane_buf);
     if (c->scratch) cudaFree(c->scratch);
     if (c->hb_queue) cudaFree(c->hb_queue);
@@ -1034,6 +1044,42 @@ int ul_get_links_wait(ul_ctx* c) {
     DeviceGuard guard(c);
     UL_CUDA(c, cudaEventSynchronize(c->ev_out_done));
     c->out_pending = false;
+    return UL_OK;
+}
+// The upload ahead of time: host -> a buffer of its own on a second stream (nothing the context's stream does is touched), and
+// the commit that makes it the configuration (repack + validation on the context's stream, behind the upload's event).
+int ul_set_links_async(ul_ctx* c, const float* host) {
+    if (!c || !host) return fail(c, UL_EINVAL, "null pointer");
+    DeviceGuard guard(c);
+    const long long n = 4 * c->V;
+    if (!c->staging_in) {
+        void* p = nullptr;
+        UL_CUDA(c, cudaMalloc(&p, sizeof(float) * (size_t)n));
+        c->staging_in = (float*)p;
+        UL_CUDA(c, cudaStreamCreateWithFlags(&c->in_stream, cudaStreamNonBlocking));
+        UL_CUDA(c, cudaEventCreateWithFlags(&c->ev_in_done, cudaEventDisableTiming));
+        UL_CUDA(c, cudaHostAlloc((void**)&c->bad_host, sizeof(int), cudaHostAllocMapped));
+        UL_CUDA(c, cudaHostGetDevicePointer((void**)&c->bad_dev, c->bad_host, 0));
+    }
+    UL_CUDA(c, cudaMemcpyAsync(c->staging_in, host, sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, c->in_stream));
+    UL_CUDA(c, cudaEventRecord(c->ev_in_done, c->in_stream));
+    c->in_pending = true;
+    return UL_OK;
+}
+int ul_set_links_commit(ul_ctx* c) {
+    if (!c) return fail(c, UL_EINVAL, "null handle");
+    if (!c->in_pending) return fail(c, UL_ESTATE, "no ul_set_links_async to commit");
+    DeviceGuard guard(c);
+    const long long n = 4 * c->V;
+    c->in_pending = false;
+    UL_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_in_done, 0));
+    *(volatile int*)c->bad_host = 0;                                // nothing on the device writes it before the launch below
+    ulk::k_repack<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(geom(c), c->th, c->staging_in, 1, c->bad_dev);
+    UL_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    UL_CUDA(c, cudaStreamSynchronize(c->stream));
+    const int bad = *(volatile int*)c->bad_host;
+    if (bad) return fail(c, UL_EINVAL, "link angles must be finite with |theta| <= 3.2 (wrap them to [-pi, pi] first)");
     return UL_OK;
 }
 int ul_set_links(ul_ctx* c, const float* host) { return links_in(c, host, 1); }

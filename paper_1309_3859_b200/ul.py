@@ -17,7 +17,7 @@ UL_OK, UL_EINVAL, UL_ENOMEM, UL_ECUDA, UL_ESTATE = 0, -1, -2, -3, -4
 # every symbol include/ul.h declares (tests check that the library exports exactly these)
 SYMBOLS = [
     "ul_create", "ul_create_ext", "ul_workspace_bytes", "ul_destroy", "ul_init", "ul_set_beta",
-    "ul_set_links", "ul_get_links", "ul_get_links_async", "ul_get_links_wait", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep", "ul_substep_slabs", "ul_set_slab_group", "ul_set_slab_group_streams",
+    "ul_set_links", "ul_get_links", "ul_get_links_async", "ul_get_links_wait", "ul_set_links_async", "ul_set_links_commit", "ul_set_links_raw", "ul_get_links_raw", "ul_get_counter", "ul_set_counter", "ul_sweep", "ul_substep", "ul_substep_slabs", "ul_set_slab_group", "ul_set_slab_group_streams",
     "ul_set_subupdate", "ul_set_update_algorithm", "ul_multilevel", "ul_multilevel_replay", "ul_workspace_bytes_replay", "ul_multilevel2_replay", "ul_workspace_bytes_replay2", "ul_multilevel2", "ul_measure_begin", "ul_accumulate",
     "ul_measure_end", "ul_measure2_begin", "ul_combine", "ul_measure2_end", "ul_set_accum_batch", "ul_set_multihit", "ul_plaquette", "ul_plaquette_noalloc", "ul_polyakov", "ul_set_site_offset", "ul_slab_partial_product", "ul_combine_partial_products", "ul_set_halo_peers", "ul_halo_flags", "ul_set_halo_peer_flags", "ul_ipc_export", "ul_ipc_open", "ul_read_correlators", "ul_read_slab_averages",
     "ul_get_launch_count", "ul_philox_selftest", "ul_sync", "ul_last_error",
@@ -53,6 +53,8 @@ def lib():
         L.ul_get_links.argtypes = [P, P]
         L.ul_get_links_async.argtypes = [P, P]
         L.ul_get_links_wait.argtypes = [P]
+        L.ul_set_links_async.argtypes = [P, P]
+        L.ul_set_links_commit.argtypes = [P]
         L.ul_set_links_raw.argtypes = [P, P]
         L.ul_get_links_raw.argtypes = [P, P]
         L.ul_get_counter.argtypes = [P, C.POINTER(C.c_uint64)]
@@ -209,6 +211,14 @@ class Lattice:
 
     def get_links_wait(self):
         self._ck(lib().ul_get_links_wait(self._h))
+
+    def set_links_async(self, src):
+        """src: contiguous CPU float32 tensor of 4 V elements (pinned), untouched until set_links_commit() returns."""
+        assert src.device.type == "cpu" and src.is_contiguous() and src.numel() == 4 * self.V
+        self._ck(lib().ul_set_links_async(self._h, C.c_void_p(src.data_ptr())))
+
+    def set_links_commit(self):
+        self._ck(lib().ul_set_links_commit(self._h))
 
     def set_links_raw(self, raw):
         """raw: canonical host array int32[4][Nt][Ns][Ns][Ns] of binary angles (exact state)."""

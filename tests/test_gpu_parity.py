@@ -1482,6 +1482,19 @@ def test_get_links_async_equals_get_links(ul):
     g.get_links_wait()
     assert np.array_equal(a.numpy().reshape(want.shape), want)
     assert np.array_equal(b.numpy().reshape(want.shape), want2)
+    # the upload in two parts: started while sweeps run, committed afterwards; equals ul_set_links
+    src = torch.from_numpy(want.reshape(-1).copy()).pin_memory()
+    g.set_links(want2)
+    g.set_links_async(src)
+    g.sweep(1, 1)                                                   # works on want2 while the upload is in flight
+    g.set_links_commit()
+    assert np.array_equal(g.get_links(), want)
+    with pytest.raises(Exception):
+        g.set_links_commit()                                        # nothing pending
+    src[5] = float("nan")
+    g.set_links_async(src)
+    with pytest.raises(Exception):
+        g.set_links_commit()                                        # validation as in ul_set_links
     c = np.empty(4 * g.V, dtype=np.float32)                         # pageable memory: still correct
     g.set_links(want2)
     g.get_links_async(torch.from_numpy(c))
