@@ -322,9 +322,9 @@ __global__ void k_set_sweep(uint32_t* sweep, uint32_t lo, uint32_t hi) { sweep[0
                         // shorter instruction sequence of the gather 1-5 % faster than 3 blocks of up to 80 registers: bench step 49.9 -> 49.2 ms)
 #endif
 #ifndef UL_OR_MINB
-#define UL_OR_MINB 5   // overrelaxation / Metropolis launches over the whole lattice (HBM-bound): 48 registers, 5 blocks per SM (OR sweep
-#endif                 // 440 -> 417 us on 64^4); the graph-replayed launches (DEVCTR: small lattices, slab groups out of L2) are left to
-                       // the compiler (46-62 registers, 4 blocks: measured 1-5 % faster there than with the cap)
+#define UL_OR_MINB 4   // overrelaxation / Metropolis launches over the whole lattice (HBM-bound): 64 registers, 4 blocks per SM.  With the
+#endif                 // shorter instruction sequence of the gather this is the optimum again (OR sweep on 64^4: 3 blocks 429 us, 4 blocks
+                       // 406 us, 5 blocks of 48 registers 418 us, 6 blocks spill; before the cuts 5 blocks won, 440 -> 417 us)
 // One tile (= one thread block's worth) of a sub-step: tile coordinates (tx, ty, tz) of a (gx, gy, ntz) tile grid, blk = the
 // tile's linear index (picks the straggler sub-queue).
 template <int KIND, int MU, int VEC, bool COH, bool PDL>
