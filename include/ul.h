@@ -116,7 +116,9 @@ int ul_set_counter(ul_ctx* h, uint64_t sweep_counter);
  * switches, read when the handle is created (for A/B measurements; defaults are the fast paths):
  * UL_NO_PDL=1, UL_NO_ZFLIP=1 (alternating traversal of the time layers), UL_NO_PERSIST=1,
  * UL_PERSIST_VEC=1|2|4, UL_OR_TMA=1 (overrelaxation through the bulk-copy staged gather,
- * csrc/ul_update_tma.cuh: slower). */
+ * csrc/ul_update_tma.cuh: slower), UL_BLOCK_BY=n (x2 row pairs per thread
+ * block, the rest of its 128 row pairs along x3; default: an even split), UL_NO_HB_LOCAL=1,
+ * UL_GROUP_STREAMS=n. */
 int ul_sweep(ul_ctx* h, int n_hb, int n_or);
 
 /* Test hook: one sub-step.  kind 0 = heatbath (draws with the current sweep counter, does
